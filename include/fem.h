@@ -1,0 +1,152 @@
+/*
+ * fem.h -- C ABI of the B200-native Free-Energy Machine annealing path (arxiv 2412.09285).
+ *
+ * The library runs, entirely in hand-written CUDA kernels for sm_100a, the replica-parallel
+ * mean-field annealing step of the paper (Fig.2): marginals from local fields,
+ * the explicit gradient of F_MF = U_MF(P) - S_MF(P)/beta (S18-S30), an Adam
+ * update of the fields under an annealed beta, for R
+ * independent replicas, followed by rounding (Eq.4), the integer energy of every
+ * replica (Eq.6-8) and the best-replica reduction (Eq.5).
+ * There is no CPU fallback: without a CUDA device every compute entry point fails with FEM_ECUDA.
+ *
+ * Conventions
+ *   - All pointers in fem_problem / fem_schedule and all result pointers are HOST pointers.
+ *     fem_create validates the problem on the host and uploads the device formats it builds.
+ *     The only DEVICE pointer in this ABI is `workspace` (caller-owned, e.g. a torch tensor).
+ *   - The library allocates no device memory: all state lives in the caller's workspace, which
+ *     must stay alive and untouched until fem_destroy.  Host-side bookkeeping is freed by
+ *     fem_destroy.
+ *   - Work is enqueued on the caller's CUDA stream (`cuda_stream` is a cudaStream_t cast to
+ *     void*, NULL = legacy default stream).  fem_anneal and fem_readout are ASYNCHRONOUS; the
+ *     fem_result / fem_get_* / fem_energy_of calls synchronise that stream before returning.
+ *     Host arrays passed to fem_anneal are consumed before it returns.
+ *   - Logical host layouts are replica-outermost, row-major: fields h[R][n][F] with F = q for
+ *     FEM_BMINCUT and F = 1 otherwise (the two-state kinds keep h_i = h_i(+1) - h_i(-1),
+ *     PAPER.md:661); configurations cfg[R][n] with states 0..q-1 (two-state: 1 <=> sigma = +1 /
+ *     Boolean true).  The device layout (replica-innermost n x R rows) is private.
+ *   - Determinism: same inputs and seed give bit-identical outputs run to run (no float atomics).
+ *   - Errors: status codes only.  Argument errors are reported synchronously (FEM_EINVAL) and
+ *     leave the handle unchanged; CUDA errors surface as FEM_ECUDA at the call that observes
+ *     them.  fem_last_error returns a static or handle-owned message.
+ */
+#ifndef FEM_H_
+#define FEM_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fem_handle fem_handle; /* opaque */
+
+typedef enum { FEM_OK = 0, FEM_EINVAL = 1, FEM_ENOMEM = 2, FEM_ECUDA = 3, FEM_ESTATE = 4 } fem_status;
+
+typedef enum {
+    FEM_MAXCUT = 0,  /* E = -sum_{(i,j) in E} W_ij [1 - delta(s_i,s_j)]          Eq.6  */
+    FEM_ISING = 1,   /* E = -sum_{i<j} J_ij s_i s_j, s = +-1 (sparse CSR or dense) PAPER.md:43         */
+    FEM_BMINCUT = 2, /* E = cut + lambda * sum_k (n_k - n/q)^2, q-state Potts      Eq.7  */
+    FEM_MAXSAT = 3   /* E = number of unsatisfied clauses                          Eq.8  */
+} fem_kind;
+
+/* Problem description; every pointer is a HOST pointer, read only during fem_create /
+ * fem_workspace_bytes. */
+typedef struct {
+    int32_t kind; /* fem_kind */
+    int32_t n;    /* number of variables, >= 1 */
+    int32_t q;    /* states per variable: 2 for MAXCUT / ISING / MAXSAT, 2..32 for BMINCUT */
+    /* Graph kinds (MAXCUT, BMINCUT, sparse ISING): symmetric CSR with BOTH directions stored, no self
+     * loops, no repeated entries, columns ascending in each row.  weight NULL = all +1.  For BMINCUT
+     * the weights must be > 0. */
+    const int64_t *row_ptr; /* [n+1] */
+    const int32_t *col_idx; /* [row_ptr[n]] */
+    const float *weight;    /* [row_ptr[n]] or NULL */
+    /* ISING only, instead of the CSR: dense n*n row-major symmetric couplings, zero diagonal. */
+    const float *dense_J;
+    /* MAXSAT: m clauses; clause c holds lits[clause_ptr[c] .. clause_ptr[c+1]) as signed 1-based
+     * literals (+v = variable v, -v = NOT v, i.e. W_mi = 1 / 0 in Eq.8).  A clause must not repeat a
+     * variable (S15); clause length 1..8. */
+    int32_t m;
+    const int64_t *clause_ptr; /* [m+1] */
+    const int32_t *lits;       /* [clause_ptr[m]] */
+    double lambda;             /* BMINCUT balance weight when the schedule gives no per-step lambda */
+} fem_problem;
+
+/* Annealing schedule and optimiser.  Step t = 0..steps-1 uses beta[t]
+ * (inverse temperature) and Adam step count t+1. */
+typedef struct {
+    int32_t steps;
+    const double *beta;   /* HOST [steps], > 0 */
+    const double *lambda; /* HOST [steps] per-step balance weight, or NULL */
+    double lr, beta1, beta2, eps, weight_decay; /* Adam, PyTorch semantics */
+    double init_scale;     /* h(0) = init_scale * N(0,1); used when fields were not injected */
+    int32_t precise_steps; /* the first K steps do their arithmetic in fp64 registers (storage stays fp32) */
+} fem_schedule;
+
+/* Bytes of device workspace fem_create needs for this problem with up to R_cap replicas
+ * (0 on invalid arguments).  Pure host arithmetic. */
+size_t fem_workspace_bytes(const fem_problem *problem, int32_t R_cap);
+
+/* Validate `problem`, build the device formats inside `workspace` (DEVICE pointer, 256-byte aligned,
+ * >= fem_workspace_bytes) and return a handle.  Synchronises `cuda_stream` once at the end.
+ * FEM_EINVAL: bad sizes, asymmetric CSR, self loop, unsorted/repeated column, literal out of range,
+ * repeated variable in a clause, q out of range, workspace too small or misaligned. */
+fem_status fem_create(const fem_problem *problem, int32_t R_cap, void *workspace, size_t workspace_bytes,
+                      void *cuda_stream, fem_handle **out);
+
+/* Run steps [t_done, stop_after) of the schedule on R replicas, where t_done is the number of steps
+ * already run since the last reset.  When t_done == 0 the Adam moments are zeroed and, unless fields
+ * were injected with fem_set_fields, the fields are drawn from `seed` with the counter-based
+ * generator of DESIGN.md section 3 (R4).  Asynchronous.  FEM_EINVAL: R < 1 or > R_cap, R differs
+ * from the R of the steps already run, stop_after outside [t_done, steps], beta[t] <= 0.
+ * One launch of the fused step kernel per step and replica block (one iteration
+ * of the listing's loop). */
+fem_status fem_anneal(fem_handle *h, const fem_schedule *schedule, int32_t R, uint64_t seed, int32_t stop_after);
+
+/* Forget the trajectory: t_done = 0, injected fields dropped. */
+fem_status fem_reset(fem_handle *h);
+
+/* Enqueue rounding (Eq.4), per-replica energies (Eq.6-8) and the best-replica argmin (Eq.5) on the
+ * current fields.  Asynchronous; results stay on the device until fem_result. */
+fem_status fem_readout(fem_handle *h);
+
+/* Run fem_readout if the fields changed since the last one, copy the results to the host and
+ * synchronise.  Any output pointer may be NULL.
+ *   best_replica : argmin_a energy[a], lowest a on ties
+ *   best_config  : HOST [n], configuration of the best replica
+ *   energy_int   : HOST [R]; MAXCUT: -cut, BMINCUT: cut, MAXSAT: unsat count, with weights rounded to
+ *                  nearest integer (exact when they are integral); ISING: 0
+ *   energy       : HOST [R] fp64; MAXCUT/MAXSAT: (double)energy_int when weights are integral, else the
+ *                  fp64 sum; BMINCUT: cut + lambda*sum_k (n_k - n/q)^2; ISING: -sum_{i<j} J_ij s_i s_j
+ *   part_sizes   : HOST [R][q] (BMINCUT; zeros otherwise) */
+fem_status fem_result(fem_handle *h, int32_t *best_replica, int32_t *best_config, int64_t *energy_int,
+                      double *energy, int32_t *part_sizes);
+
+/* ---- parity hooks (logical layouts, HOST pointers, synchronous) ---- */
+fem_status fem_set_fields(fem_handle *h, int32_t R, const float *fields /* [R][n][F] */); /* resets t_done */
+fem_status fem_get_fields(fem_handle *h, float *fields /* [R][n][F] */);
+fem_status fem_get_moments(fem_handle *h, float *m1, float *m2 /* [R][n][F] each, may be NULL */);
+/* marginals computed on the device from the current fields; two-state kinds: [R][n] = P(state 1) */
+fem_status fem_get_marginals(fem_handle *h, float *marginals /* [R][n][F] */);
+fem_status fem_get_configs(fem_handle *h, int32_t *cfg /* [R][n] */);
+/* energies of caller-supplied configurations (count <= R_cap), same definitions as fem_result */
+fem_status fem_energy_of(fem_handle *h, const int32_t *cfg /* [count][n] */, int32_t count, int64_t *energy_int,
+                         double *energy, int32_t *part_sizes /* [count][q] or NULL */);
+
+/* Tuning knobs (all optional): "replica_block" (replicas per L2-resident block, 0 = all),
+ * "steps_per_block" (steps run on one replica block before moving to the next, 0 = whole anneal
+ * per block when blocking is on, 1 = step-major).  Unknown key: FEM_EINVAL. */
+fem_status fem_set_option(fem_handle *h, const char *key, int64_t value);
+/* Introspection for benchmarks: "launches" (kernels enqueued so far), "t_done", "R", "nnz",
+ * "step_bytes" (algorithmic HBM bytes of one fused step). */
+int64_t fem_get_info(const fem_handle *h, const char *key);
+
+const char *fem_last_error(const fem_handle *h); /* h may be NULL: last create-time error */
+void fem_destroy(fem_handle *h);
+int32_t fem_abi_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FEM_H_ */

@@ -1,0 +1,136 @@
+// Device helpers shared by the step kernels: vector row access and the two-state / Adam arithmetic.
+#pragma once
+#include <type_traits>
+
+#include "fem_internal.cuh"
+
+namespace fem {
+
+// ---- VEC-wide row access (VEC = 1, 2 or 4 consecutive replicas) of storage type T ----
+// T = float: the bulk of the anneal.  T = double: the "wide" phase (first precise_steps steps), where
+// both the arithmetic and the stored state are fp64.
+template <typename T, int VEC>
+struct Row {
+    T v[VEC];
+    // 16-byte vector type that carries the row
+    using V16 = typename std::conditional<sizeof(T) == 4, float4, double2>::type;
+    static constexpr int kPer16 = 16 / sizeof(T);
+    static constexpr int kBytes = VEC * sizeof(T);
+
+    __device__ __forceinline__ static Row ld(const T *p) {  // read-only path (gathers)
+        Row r;
+        if constexpr (kBytes >= 16) {
+#pragma unroll
+            for (int k = 0; k < kBytes / 16; ++k) {
+                const V16 t = __ldg(reinterpret_cast<const V16 *>(p) + k);
+                memcpy(&r.v[k * kPer16], &t, 16);
+            }
+        } else if constexpr (kBytes == 8) {
+            const float2 t = __ldg(reinterpret_cast<const float2 *>(p));
+            memcpy(&r.v[0], &t, 8);
+        } else {
+            r.v[0] = __ldg(p);
+        }
+        return r;
+    }
+    __device__ __forceinline__ static Row ld_stream(const T *p) {  // streamed once: evict-first
+        Row r;
+        if constexpr (kBytes >= 16) {
+#pragma unroll
+            for (int k = 0; k < kBytes / 16; ++k) {
+                const V16 t = __ldcs(reinterpret_cast<const V16 *>(p) + k);
+                memcpy(&r.v[k * kPer16], &t, 16);
+            }
+        } else if constexpr (kBytes == 8) {
+            const float2 t = __ldcs(reinterpret_cast<const float2 *>(p));
+            memcpy(&r.v[0], &t, 8);
+        } else {
+            r.v[0] = __ldcs(p);
+        }
+        return r;
+    }
+    __device__ __forceinline__ void st(T *p) const {
+        if constexpr (kBytes >= 16) {
+#pragma unroll
+            for (int k = 0; k < kBytes / 16; ++k) {
+                V16 t;
+                memcpy(&t, &v[k * kPer16], 16);
+                reinterpret_cast<V16 *>(p)[k] = t;
+            }
+        } else if constexpr (kBytes == 8) {
+            float2 t;
+            memcpy(&t, &v[0], 8);
+            *reinterpret_cast<float2 *>(p) = t;
+        } else {
+            *p = v[0];
+        }
+    }
+    __device__ __forceinline__ void st_stream(T *p) const {
+        if constexpr (kBytes >= 16) {
+#pragma unroll
+            for (int k = 0; k < kBytes / 16; ++k) {
+                V16 t;
+                memcpy(&t, &v[k * kPer16], 16);
+                __stcs(reinterpret_cast<V16 *>(p) + k, t);
+            }
+        } else if constexpr (kBytes == 8) {
+            float2 t;
+            memcpy(&t, &v[0], 8);
+            __stcs(reinterpret_cast<float2 *>(p), t);
+        } else {
+            __stcs(p, v[0]);
+        }
+    }
+};
+
+// ---- scalars narrowed to the compute type ----
+template <typename T>
+struct Sc {
+    T inv_beta, step_size, rsqrt_bc2, eps, b1, b2, omb1, omb2, wd, two_lambda;
+    __device__ __forceinline__ explicit Sc(const StepScalars &s)
+        : inv_beta((T)s.inv_beta), step_size((T)s.step_size), rsqrt_bc2((T)s.rsqrt_bc2), eps((T)s.eps), b1((T)s.b1),
+          b2((T)s.b2), omb1((T)s.one_minus_b1), omb2((T)s.one_minus_b2), wd((T)s.wd), two_lambda((T)s.two_lambda) {}
+};
+
+__device__ __forceinline__ float fexp(float x) { return expf(x); }
+__device__ __forceinline__ double fexp(double x) { return exp(x); }
+__device__ __forceinline__ float fsqrt(float x) { return sqrtf(x); }
+__device__ __forceinline__ double fsqrt(double x) { return sqrt(x); }
+__device__ __forceinline__ float flog(float x) { return logf(x); }
+__device__ __forceinline__ double flog(double x) { return log(x); }
+
+__device__ __forceinline__ float ftanh(float x) { return tanhf(x); }
+__device__ __forceinline__ double ftanh(double x) { return tanh(x); }
+
+// Two-state pieces from one field h = h(+1) - h(-1), each free of cancellation:
+//   p(1-p) = e/(1+e)^2 with e = exp(-|h|)   (exact in the saturated tails, where 1 - m^2 would round to 0)
+//   m = 2p - 1 = tanh(h/2)                   (library tanh: relative accuracy also for |h| -> 0, where the
+//                                             deviation from the uniform marginal is all the signal there is)
+template <typename T>
+__device__ __forceinline__ T p1mp_of(T h) {
+    const T e = fexp(-fabs(h));
+    const T r = (T)1 / ((T)1 + e);
+    return e * r * r;
+}
+template <typename T>
+__device__ __forceinline__ T mag_of(T h) {
+    return ftanh((T)0.5 * h);
+}
+template <typename T>
+__device__ __forceinline__ T sigmoid_of(T h) {
+    const T e = fexp(-fabs(h));
+    const T r = (T)1 / ((T)1 + e);
+    return h < (T)0 ? e * r : r;
+}
+
+// Adam (Kingma & Ba as arranged by torch.optim.Adam): returns the new field.
+template <typename T>
+__device__ __forceinline__ T adam_update(T h, T g, T &m1, T &m2, const Sc<T> &sc) {
+    g = g + sc.wd * h;
+    m1 = sc.b1 * m1 + sc.omb1 * g;
+    m2 = sc.b2 * m2 + sc.omb2 * g * g;
+    T denom = fsqrt(m2) * sc.rsqrt_bc2 + sc.eps;
+    return h - sc.step_size * (m1 / denom);
+}
+
+}  // namespace fem

@@ -1,0 +1,639 @@
+// C ABI of libfem_b200 (include/fem.h): validation, workspace carve-up, step scheduling, result copies.
+// All arithmetic of the method runs in the kernels (k_*.cu); the host only computes the per-step
+// scalars (1/beta_t and Adam's bias corrections) in double, as DESIGN.md section 6 states.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <new>
+
+#include "fem_internal.cuh"
+
+namespace fem {
+
+// launchers defined in the kernel files
+void launch_step_q2(Handle *hd, const StepScalars &sc, bool wide, int blk_begin, int blk_count);
+void launch_prepare_q2(Handle *hd, bool wide);
+void launch_potts(Handle *hd, const StepScalars &sc, bool wide, bool step, int blk_begin, int blk_count);
+void launch_sigmoid(Handle *hd, float *out);
+int potts_vec(const Handle *hd);
+void launch_potts_softmax(Handle *hd, float *out);
+
+static std::string g_create_error;
+
+struct Layout {
+    size_t row_ptr, col, w, J, field, occ_ptr, occ, clause_ptr, lits;
+    size_t h, m1, m2, g0, g1, stage, hW, m1W, m2W, gW0, gW1, colsum0, colsum1, colpart, cfg, e_part_i, e_part_d, part_part, e_int, e_real, part,
+        best, total;
+};
+
+static size_t align_up(size_t x) { return (x + 255) & ~size_t(255); }
+
+struct ProblemShape {
+    int64_t nnz = 0, nlits = 0, nocc = 0;
+    int kmax = 0;
+    bool weighted = false, dense = false;
+};
+
+static bool shape_of(const fem_problem *pb, ProblemShape *s, std::string *err) {
+    if (!pb) return *err = "problem is NULL", false;
+    if (pb->n < 1) return *err = "n must be >= 1", false;
+    if (pb->kind < FEM_MAXCUT || pb->kind > FEM_MAXSAT) return *err = "unknown kind", false;
+    if (pb->kind == FEM_BMINCUT) {
+        if (pb->q < 2 || pb->q > kMaxQ) return *err = "q must be in 2..32 for BMINCUT", false;
+    } else if (pb->q != 2) {
+        return *err = "q must be 2 for MAXCUT / ISING / MAXSAT", false;
+    }
+    if (pb->kind == FEM_MAXSAT) {
+        if (pb->m < 1 || !pb->clause_ptr || !pb->lits) return *err = "MAXSAT needs m >= 1, clause_ptr and lits", false;
+        if (pb->clause_ptr[0] != 0) return *err = "clause_ptr[0] must be 0", false;
+        for (int c = 0; c < pb->m; ++c) {
+            const int64_t len = pb->clause_ptr[c + 1] - pb->clause_ptr[c];
+            if (len < 1 || len > kMaxClauseLen) return *err = "clause length must be in 1..8", false;
+            s->kmax = std::max<int>(s->kmax, (int)len);
+        }
+        s->nlits = s->nocc = pb->clause_ptr[pb->m];
+        if (s->nlits >= (int64_t)1 << 30) return *err = "too many literals", false;
+        if (pb->n >= (1 << 29)) return *err = "too many variables", false;
+        return true;
+    }
+    if (pb->kind == FEM_ISING && pb->dense_J) {
+        if (pb->row_ptr || pb->col_idx) return *err = "give either dense_J or a CSR, not both", false;
+        if (pb->n > 32768) return *err = "dense n too large", false;
+        s->dense = true;
+        return true;
+    }
+    if (!pb->row_ptr || (!pb->col_idx && pb->row_ptr[pb->n] != 0)) return *err = "graph kinds need row_ptr and col_idx", false;
+    if (pb->row_ptr[0] != 0) return *err = "row_ptr[0] must be 0", false;
+    s->nnz = pb->row_ptr[pb->n];
+    if (s->nnz < 0 || s->nnz >= (int64_t)1 << 31) return *err = "nnz out of range", false;
+    s->weighted = pb->weight != nullptr;
+    return true;
+}
+
+static Layout make_layout(const fem_problem *pb, const ProblemShape &s, int R_cap) {
+    Layout L{};
+    size_t o = 0;
+    auto take = [&](size_t bytes) {
+        size_t at = o;
+        o = align_up(o + bytes);
+        return at;
+    };
+    const int F = pb->kind == FEM_BMINCUT ? pb->q : 1;
+    const size_t rows = (size_t)pb->n * F + 1;
+    const size_t state = rows * (size_t)R_cap * sizeof(float);
+    L.row_ptr = take(((size_t)pb->n + 1) * 4);
+    L.col = take((size_t)s.nnz * 4);
+    L.w = take(s.weighted ? (size_t)s.nnz * 4 : 0);
+    L.J = take(s.dense ? (size_t)pb->n * pb->n * 4 : 0);
+    L.field = take(s.dense ? 2 * state : 0);  // fp64 in the wide phase
+    L.occ_ptr = take(pb->kind == FEM_MAXSAT ? ((size_t)pb->n + 1) * 4 : 0);
+    L.occ = take((size_t)s.nocc * std::max(1, s.kmax - 1) * 4);
+    L.clause_ptr = take(pb->kind == FEM_MAXSAT ? ((size_t)pb->m + 1) * 4 : 0);
+    L.lits = take((size_t)s.nlits * 4);
+    L.h = take(state);
+    L.m1 = take(state);
+    L.m2 = take(state);
+    L.g0 = take(state);
+    L.g1 = take(state);
+    L.stage = take(state);
+    L.hW = take(2 * state);  // wide phase: the same five arrays in fp64
+    L.m1W = take(2 * state);
+    L.m2W = take(2 * state);
+    L.gW0 = take(2 * state);
+    L.gW1 = take(2 * state);
+    const size_t qR = (size_t)pb->q * R_cap;
+    const bool potts = pb->kind == FEM_BMINCUT;
+    L.colsum0 = take(potts ? qR * 8 : 0);
+    L.colsum1 = take(potts ? qR * 8 : 0);
+    L.colpart = take(potts ? (size_t)kColBlocks * qR * 8 : 0);
+    L.cfg = take((size_t)pb->n * R_cap);
+    L.e_part_i = take((size_t)kEnergyChunks * R_cap * 8);
+    L.e_part_d = take((size_t)kEnergyChunks * R_cap * 8);
+    L.part_part = take(potts ? (size_t)kEnergyChunks * qR * 4 : 0);
+    L.e_int = take((size_t)R_cap * 8);
+    L.e_real = take((size_t)R_cap * 8);
+    L.part = take(qR * 4);
+    L.best = take(((size_t)pb->n + 1) * 4);
+    L.total = o;
+    return L;
+}
+
+static bool cuda_ok(Handle *hd, cudaError_t e, const char *what) {
+    if (e == cudaSuccess) return true;
+    hd->err = std::string(what) + ": " + cudaGetErrorString(e);
+    return false;
+}
+
+static fem_status fail(Handle *hd, fem_status st, const char *msg) {
+    if (hd) hd->err = msg;
+    else g_create_error = msg;
+    return st;
+}
+
+// Validate the symmetric CSR and report whether all weights are integral.
+static bool validate_graph(const fem_problem *pb, int64_t nnz, bool *integral, int *uniform_deg, std::string *err) {
+    const int n = pb->n;
+    *integral = true;
+    int64_t d0 = pb->row_ptr[1] - pb->row_ptr[0];
+    bool uniform = true;
+    for (int i = 0; i < n; ++i) {
+        const int64_t a = pb->row_ptr[i], b = pb->row_ptr[i + 1];
+        if (b < a || b > nnz) return *err = "row_ptr must be non-decreasing and end at nnz", false;
+        if (b - a != d0) uniform = false;
+        for (int64_t e = a; e < b; ++e) {
+            const int j = pb->col_idx[e];
+            if (j < 0 || j >= n) return *err = "column index out of range", false;
+            if (j == i) return *err = "self loop", false;
+            if (e > a && pb->col_idx[e - 1] >= j) return *err = "columns must be strictly ascending in each row", false;
+            const float w = pb->weight ? pb->weight[e] : 1.0f;
+            if (!std::isfinite(w)) return *err = "non-finite weight", false;
+            if (pb->kind == FEM_BMINCUT && !(w > 0.f)) return *err = "BMINCUT weights must be > 0", false;
+            if (w != std::nearbyint(w) || std::fabs(w) > 1e6f) *integral = false;
+        }
+    }
+    for (int i = 0; i < n; ++i)
+        for (int64_t e = pb->row_ptr[i]; e < pb->row_ptr[i + 1]; ++e) {
+            const int j = pb->col_idx[e];
+            const int32_t *lo = pb->col_idx + pb->row_ptr[j], *hi = pb->col_idx + pb->row_ptr[j + 1];
+            const int32_t *it = std::lower_bound(lo, hi, i);
+            if (it == hi || *it != i) return *err = "CSR is not symmetric", false;
+            if (pb->weight && pb->weight[it - pb->col_idx] != pb->weight[e]) return *err = "weights are not symmetric", false;
+        }
+    *uniform_deg = (uniform && d0 > 0 && d0 <= 64) ? (int)d0 : 0;
+    return true;
+}
+
+static void configure_R(Handle *hd, int R) {
+    hd->R = R;
+    int Rb = R;
+    if (hd->opt_replica_block > 0 && hd->opt_replica_block < R && R % hd->opt_replica_block == 0)
+        Rb = (int)hd->opt_replica_block;
+    hd->Rb = Rb;
+    if (hd->dp.kind == FEM_BMINCUT) {  // one variable's replicas must fit one CTA pass
+        for (;;) {
+            const int vec = potts_vec(hd);
+            if (hd->Rb / vec <= kThreads) break;
+            int nb = R / hd->Rb + 1;
+            while (R % nb) ++nb;
+            hd->Rb = R / nb;
+        }
+    }
+}
+
+}  // namespace fem
+
+using namespace fem;
+
+extern "C" {
+
+int32_t fem_abi_version(void) { return 1; }
+
+const char *fem_last_error(const fem_handle *h) {
+    return h ? reinterpret_cast<const Handle *>(h)->err.c_str() : g_create_error.c_str();
+}
+
+size_t fem_workspace_bytes(const fem_problem *problem, int32_t R_cap) {
+    ProblemShape s;
+    std::string err;
+    if (R_cap < 1 || !shape_of(problem, &s, &err)) return 0;
+    return make_layout(problem, s, R_cap).total;
+}
+
+fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, size_t workspace_bytes, void *cuda_stream,
+                      fem_handle **out) {
+    if (!out) return fail(nullptr, FEM_EINVAL, "out is NULL");
+    *out = nullptr;
+    ProblemShape s;
+    std::string err;
+    if (R_cap < 1) return fail(nullptr, FEM_EINVAL, "R_cap must be >= 1");
+    if (!shape_of(pb, &s, &err)) return fail(nullptr, FEM_EINVAL, err.c_str());
+    const Layout L = make_layout(pb, s, R_cap);
+    if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255)) return fail(nullptr, FEM_EINVAL, "workspace must be a 256-byte aligned device pointer");
+    if (workspace_bytes < L.total) return fail(nullptr, FEM_EINVAL, "workspace too small (see fem_workspace_bytes)");
+
+    Handle *hd = new (std::nothrow) Handle();
+    if (!hd) return fail(nullptr, FEM_ENOMEM, "out of host memory");
+    hd->pb = *pb;
+    hd->pb.row_ptr = nullptr;
+    hd->pb.col_idx = nullptr;
+    hd->pb.weight = nullptr;
+    hd->pb.dense_J = nullptr;
+    hd->pb.clause_ptr = nullptr;
+    hd->pb.lits = nullptr;
+    hd->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    hd->R_cap = R_cap;
+    DevProblem &dp = hd->dp;
+    dp.kind = pb->kind;
+    dp.n = pb->n;
+    dp.q = pb->q;
+    dp.F = pb->kind == FEM_BMINCUT ? pb->q : 1;
+    dp.nnz = s.nnz;
+    hd->rows = (int64_t)dp.n * dp.F + 1;
+    char *base = static_cast<char *>(workspace);
+    auto at = [&](size_t off) { return base + off; };
+
+    // host staging vectors must outlive the async copies: they die after the synchronise below
+    std::vector<int> h_row, h_occ_ptr, h_occ, h_cptr;
+    bool ok = true;
+    bool device_checked = false;
+    auto up = [&](void *dst, const void *src, size_t bytes, const char *what) {
+        if (!device_checked) {  // argument errors are reported before the device is touched
+            device_checked = true;
+            int ndev = 0;
+            if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+                hd->err = "no CUDA device: libfem_b200 has no CPU fallback";
+                ok = false;
+            }
+        }
+        if (ok && bytes) ok = cuda_ok(hd, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, hd->stream), what);
+    };
+
+    if (pb->kind == FEM_MAXSAT) {
+        const int n = pb->n, m = pb->m;
+        const int ks = std::max(1, s.kmax - 1);
+        dp.m = m;
+        dp.kstride = ks;
+        h_occ_ptr.assign((size_t)n + 1, 0);
+        for (int c = 0; c < m; ++c) {
+            for (int64_t x = pb->clause_ptr[c]; x < pb->clause_ptr[c + 1]; ++x) {
+                const int lit = pb->lits[x];
+                const int v = (lit > 0 ? lit : -lit) - 1;
+                if (lit == 0 || v >= n) {
+                    delete hd;
+                    return fail(nullptr, FEM_EINVAL, "literal out of range");
+                }
+                for (int64_t y = pb->clause_ptr[c]; y < x; ++y) {
+                    const int l2 = pb->lits[y];
+                    if ((l2 > 0 ? l2 : -l2) - 1 == v) {
+                        delete hd;
+                        return fail(nullptr, FEM_EINVAL, "a clause repeats a variable");
+                    }
+                }
+                h_occ_ptr[(size_t)v + 1]++;
+            }
+        }
+        for (int i = 0; i < n; ++i) h_occ_ptr[(size_t)i + 1] += h_occ_ptr[i];
+        h_occ.assign((size_t)s.nocc * ks, (n << 1) | 1);  // padding: the constant-1 row, read as "p"
+        std::vector<int> fill(h_occ_ptr.begin(), h_occ_ptr.end() - 1);
+        for (int c = 0; c < m; ++c) {  // clause order inside each variable's list == the oracle's summation order
+            const int64_t a = pb->clause_ptr[c], b = pb->clause_ptr[c + 1];
+            for (int64_t x = a; x < b; ++x) {
+                const int lit = pb->lits[x];
+                const int v = (lit > 0 ? lit : -lit) - 1;
+                int *ent = h_occ.data() + (size_t)fill[v]++ * ks;
+                int k = 0;
+                for (int64_t y = a; y < b; ++y) {
+                    if (y == x) continue;
+                    const int l2 = pb->lits[y];
+                    ent[k++] = (((l2 > 0 ? l2 : -l2) - 1) << 1) | (l2 < 0 ? 1 : 0);
+                }
+                if (lit > 0) ent[0] |= 0x80000000;
+            }
+        }
+        h_cptr.resize((size_t)m + 1);
+        for (int c = 0; c <= m; ++c) h_cptr[c] = (int)pb->clause_ptr[c];
+        up(at(L.occ_ptr), h_occ_ptr.data(), h_occ_ptr.size() * 4, "upload occ_ptr");
+        up(at(L.occ), h_occ.data(), h_occ.size() * 4, "upload occ");
+        up(at(L.clause_ptr), h_cptr.data(), h_cptr.size() * 4, "upload clause_ptr");
+        up(at(L.lits), pb->lits, (size_t)s.nlits * 4, "upload lits");
+        dp.occ_ptr = reinterpret_cast<int *>(at(L.occ_ptr));
+        dp.occ = reinterpret_cast<int *>(at(L.occ));
+        dp.clause_ptr = reinterpret_cast<int *>(at(L.clause_ptr));
+        dp.lits = reinterpret_cast<int *>(at(L.lits));
+        hd->integral_weights = true;
+        hd->structure_bytes = 4 * ((int64_t)n + 1) + 4 * (int64_t)s.nocc * ks;
+    } else if (s.dense) {
+        const int n = pb->n;
+        for (int i = 0; i < n; ++i) {
+            if (pb->dense_J[(size_t)i * n + i] != 0.f) {
+                delete hd;
+                return fail(nullptr, FEM_EINVAL, "dense_J must have a zero diagonal");
+            }
+            for (int j = i + 1; j < n; ++j)
+                if (pb->dense_J[(size_t)i * n + j] != pb->dense_J[(size_t)j * n + i] ||
+                    !std::isfinite(pb->dense_J[(size_t)i * n + j])) {
+                    delete hd;
+                    return fail(nullptr, FEM_EINVAL, "dense_J must be symmetric and finite");
+                }
+        }
+        up(at(L.J), pb->dense_J, (size_t)n * n * 4, "upload J");
+        dp.J = reinterpret_cast<float *>(at(L.J));
+        hd->field = reinterpret_cast<float *>(at(L.field));
+        hd->integral_weights = false;
+        hd->structure_bytes = 4 * (int64_t)n * n;
+    } else {
+        if (!validate_graph(pb, s.nnz, &hd->integral_weights, &dp.uniform_deg, &err)) {
+            delete hd;
+            return fail(nullptr, FEM_EINVAL, err.c_str());
+        }
+        h_row.resize((size_t)pb->n + 1);
+        for (int i = 0; i <= pb->n; ++i) h_row[i] = (int)pb->row_ptr[i];
+        up(at(L.row_ptr), h_row.data(), h_row.size() * 4, "upload row_ptr");
+        up(at(L.col), pb->col_idx, (size_t)s.nnz * 4, "upload col_idx");
+        if (s.weighted) up(at(L.w), pb->weight, (size_t)s.nnz * 4, "upload weight");
+        dp.row_ptr = reinterpret_cast<int *>(at(L.row_ptr));
+        dp.col = reinterpret_cast<int *>(at(L.col));
+        dp.w = s.weighted ? reinterpret_cast<float *>(at(L.w)) : nullptr;
+        if (pb->kind == FEM_ISING) hd->integral_weights = false;
+        hd->structure_bytes = (dp.uniform_deg > 0 ? 0 : 4 * ((int64_t)pb->n + 1)) + (s.weighted ? 8 : 4) * s.nnz;
+    }
+    hd->lambda_last = pb->lambda;
+    hd->h = reinterpret_cast<float *>(at(L.h));
+    hd->m1 = reinterpret_cast<float *>(at(L.m1));
+    hd->m2 = reinterpret_cast<float *>(at(L.m2));
+    hd->g[0] = reinterpret_cast<float *>(at(L.g0));
+    hd->g[1] = reinterpret_cast<float *>(at(L.g1));
+    hd->stage = reinterpret_cast<float *>(at(L.stage));
+    hd->hW = reinterpret_cast<double *>(at(L.hW));
+    hd->m1W = reinterpret_cast<double *>(at(L.m1W));
+    hd->m2W = reinterpret_cast<double *>(at(L.m2W));
+    hd->gW[0] = reinterpret_cast<double *>(at(L.gW0));
+    hd->gW[1] = reinterpret_cast<double *>(at(L.gW1));
+    hd->colsum[0] = reinterpret_cast<double *>(at(L.colsum0));
+    hd->colsum[1] = reinterpret_cast<double *>(at(L.colsum1));
+    hd->colpart = reinterpret_cast<double *>(at(L.colpart));
+    hd->cfg = reinterpret_cast<int8_t *>(at(L.cfg));
+    hd->e_part_i = reinterpret_cast<long long *>(at(L.e_part_i));
+    hd->e_part_d = reinterpret_cast<double *>(at(L.e_part_d));
+    hd->part_part = reinterpret_cast<int *>(at(L.part_part));
+    hd->e_int = reinterpret_cast<long long *>(at(L.e_int));
+    hd->e_real = reinterpret_cast<double *>(at(L.e_real));
+    hd->part = reinterpret_cast<int *>(at(L.part));
+    hd->best = reinterpret_cast<int *>(at(L.best));
+    if (ok) ok = cuda_ok(hd, cudaMemsetAsync(hd->part, 0, (size_t)pb->q * R_cap * 4, hd->stream), "memset");
+    if (ok) ok = cuda_ok(hd, cudaStreamSynchronize(hd->stream), "fem_create synchronize");
+    if (!ok) {
+        g_create_error = hd->err;
+        delete hd;
+        return FEM_ECUDA;
+    }
+    *out = reinterpret_cast<fem_handle *>(hd);
+    return FEM_OK;
+}
+
+void fem_destroy(fem_handle *h) { delete reinterpret_cast<Handle *>(h); }
+
+fem_status fem_reset(fem_handle *h) {
+    Handle *hd = reinterpret_cast<Handle *>(h);
+    if (!hd) return FEM_EINVAL;
+    hd->t_done = 0;
+    hd->injected = false;
+    hd->gather_valid = false;
+    hd->readout_valid = false;
+    hd->wide_live = false;
+    return FEM_OK;
+}
+
+fem_status fem_set_option(fem_handle *h, const char *key, int64_t value) {
+    Handle *hd = reinterpret_cast<Handle *>(h);
+    if (!hd || !key) return FEM_EINVAL;
+    if (hd->t_done != 0 || hd->injected) return fail(hd, FEM_ESTATE, "options can only change before fields exist (fem_reset first)");
+    if (!strcmp(key, "replica_block")) {
+        if (value < 0) return fail(hd, FEM_EINVAL, "replica_block must be >= 0");
+        hd->opt_replica_block = value;
+    } else if (!strcmp(key, "steps_per_block")) {
+        if (value < 0) return fail(hd, FEM_EINVAL, "steps_per_block must be >= 0");
+        hd->opt_steps_per_block = value;
+    } else {
+        return fail(hd, FEM_EINVAL, "unknown option");
+    }
+    return FEM_OK;
+}
+
+int64_t fem_get_info(const fem_handle *h, const char *key) {
+    const Handle *hd = reinterpret_cast<const Handle *>(h);
+    if (!hd || !key) return -1;
+    if (!strcmp(key, "launches")) return hd->launches;
+    if (!strcmp(key, "t_done")) return hd->t_done;
+    if (!strcmp(key, "R")) return hd->R;
+    if (!strcmp(key, "replica_block")) return hd->Rb;
+    if (!strcmp(key, "nnz")) return hd->dp.kind == FEM_MAXSAT ? hd->pb.m : hd->dp.nnz;
+    if (!strcmp(key, "uniform_degree")) return hd->dp.uniform_deg;
+    if (!strcmp(key, "integral_weights")) return hd->integral_weights;
+    if (!strcmp(key, "step_bytes")) {
+        // algorithmic HBM bytes of one fused step: 24 B per field (read and write h, m1, m2)
+        // plus the problem structure once
+        const int64_t fields = (int64_t)hd->dp.n * hd->dp.F * hd->R;
+        return 24 * fields + hd->structure_bytes;
+    }
+    return -1;
+}
+
+
+fem_status fem_set_fields(fem_handle *h, int32_t R, const float *fields) {
+    Handle *hd = reinterpret_cast<Handle *>(h);
+    if (!hd || !fields) return FEM_EINVAL;
+    if (R < 1 || R > hd->R_cap) return fail(hd, FEM_EINVAL, "R must be in 1..R_cap");
+    configure_R(hd, R);
+    const size_t bytes = (size_t)hd->dp.n * hd->dp.F * R * sizeof(float);
+    if (!cuda_ok(hd, cudaMemcpyAsync(hd->stage, fields, bytes, cudaMemcpyHostToDevice, hd->stream), "upload fields")) return FEM_ECUDA;
+    launch_transpose_in(hd, hd->stage, hd->h);
+    if (!cuda_ok(hd, cudaStreamSynchronize(hd->stream), "fem_set_fields")) return FEM_ECUDA;
+    hd->t_done = 0;
+    hd->injected = true;
+    hd->gather_valid = false;
+    hd->readout_valid = false;
+    hd->wide_live = false;
+    return FEM_OK;
+}
+
+// device-layout array (fp32 `src`, or its fp64 twin `srcW` while the wide phase is live) -> logical host array
+static fem_status fetch_state(Handle *hd, const float *src, const double *srcW, float *dst_host) {
+    if (hd->R < 1) return fail(hd, FEM_ESTATE, "no fields yet");
+    if (hd->wide_live && srcW) launch_transpose_out_wide(hd, srcW, hd->stage);
+    else launch_transpose_out(hd, src, hd->stage);
+    const size_t bytes = (size_t)hd->dp.n * hd->dp.F * hd->R * sizeof(float);
+    if (!cuda_ok(hd, cudaMemcpyAsync(dst_host, hd->stage, bytes, cudaMemcpyDeviceToHost, hd->stream), "download")) return FEM_ECUDA;
+    if (!cuda_ok(hd, cudaStreamSynchronize(hd->stream), "synchronize")) return FEM_ECUDA;
+    return FEM_OK;
+}
+
+fem_status fem_get_fields(fem_handle *h, float *fields) {
+    Handle *hd = reinterpret_cast<Handle *>(h);
+    if (!hd || !fields) return FEM_EINVAL;
+    return fetch_state(hd, hd->h, hd->hW, fields);
+}
+
+fem_status fem_get_moments(fem_handle *h, float *m1, float *m2) {
+    Handle *hd = reinterpret_cast<Handle *>(h);
+    if (!hd) return FEM_EINVAL;
+    fem_status st = FEM_OK;
+    if (m1) st = fetch_state(hd, hd->m1, hd->m1W, m1);
+    if (st == FEM_OK && m2) st = fetch_state(hd, hd->m2, hd->m2W, m2);
+    return st;
+}
+
+static void ensure_gather(Handle *hd) {
+    if (hd->gather_valid) return;
+    StepScalars sc{};
+    if (hd->dp.kind == FEM_BMINCUT) launch_potts(hd, sc, hd->wide_live, /*step=*/false, 0, hd->R / hd->Rb);
+    else launch_prepare_q2(hd, hd->wide_live);
+    hd->gather_valid = true;
+}
+
+fem_status fem_get_marginals(fem_handle *h, float *marginals) {
+    Handle *hd = reinterpret_cast<Handle *>(h);
+    if (!hd || !marginals) return FEM_EINVAL;
+    if (hd->R < 1) return fail(hd, FEM_ESTATE, "no fields yet");
+    // the fp32 g[cur ^ 1] is scratch here: the next step (or the narrowing) overwrites it anyway
+    if (hd->dp.kind == FEM_BMINCUT) launch_potts_softmax(hd, hd->g[hd->cur ^ 1]);
+    else launch_sigmoid(hd, hd->g[hd->cur ^ 1]);
+    return fetch_state(hd, hd->g[hd->cur ^ 1], nullptr, marginals);
+}
+
+fem_status fem_anneal(fem_handle *h, const fem_schedule *sch, int32_t R, uint64_t seed, int32_t stop_after) {
+    Handle *hd = reinterpret_cast<Handle *>(h);
+    if (!hd || !sch) return FEM_EINVAL;
+    if (R < 1 || R > hd->R_cap) return fail(hd, FEM_EINVAL, "R must be in 1..R_cap");
+    if (sch->steps < 0 || (sch->steps > 0 && !sch->beta)) return fail(hd, FEM_EINVAL, "schedule needs beta[steps]");
+    if (stop_after < hd->t_done || stop_after > sch->steps) return fail(hd, FEM_EINVAL, "stop_after must be in [t_done, steps]");
+    if ((hd->t_done > 0 || hd->injected) && R != hd->R) return fail(hd, FEM_EINVAL, "R differs from the replicas already in flight");
+    if (!(sch->lr > 0) || !(sch->beta1 >= 0 && sch->beta1 < 1) || !(sch->beta2 >= 0 && sch->beta2 < 1) || !(sch->eps >= 0))
+        return fail(hd, FEM_EINVAL, "bad Adam parameters");
+    for (int t = hd->t_done; t < stop_after; ++t)
+        if (!(sch->beta[t] > 0) || !std::isfinite(sch->beta[t])) return fail(hd, FEM_EINVAL, "beta[t] must be finite and > 0");
+
+    const int K = std::max(0, sch->precise_steps);
+    if (hd->t_done == 0) {
+        if (!hd->injected) {
+            configure_R(hd, R);
+            launch_init_fields(hd, seed, sch->init_scale);
+        }
+        if (K > 0) {  // wide phase: fp64 arithmetic and fp64 storage for the first K steps
+            launch_widen(hd);
+            hd->wide_live = true;
+        } else {
+            launch_zero_moments(hd);
+            hd->wide_live = false;
+        }
+        hd->gather_valid = false;
+    }
+    ensure_gather(hd);
+    const int nb = hd->R / hd->Rb;
+    auto scalars = [&](int t) {
+        StepScalars sc;
+        sc.inv_beta = 1.0 / sch->beta[t];
+        sc.step_size = sch->lr / (1.0 - std::pow(sch->beta1, (double)(t + 1)));
+        sc.rsqrt_bc2 = 1.0 / std::sqrt(1.0 - std::pow(sch->beta2, (double)(t + 1)));
+        sc.eps = sch->eps;
+        sc.b1 = sch->beta1;
+        sc.b2 = sch->beta2;
+        sc.one_minus_b1 = 1.0 - sch->beta1;
+        sc.one_minus_b2 = 1.0 - sch->beta2;
+        sc.wd = sch->weight_decay;
+        sc.two_lambda = 2.0 * (sch->lambda ? sch->lambda[t] : hd->pb.lambda);
+        return sc;
+    };
+    auto one_step = [&](int t, int b0, int bc) {
+        if (hd->dp.kind == FEM_BMINCUT) launch_potts(hd, scalars(t), hd->wide_live, true, b0, bc);
+        else launch_step_q2(hd, scalars(t), hd->wide_live, b0, bc);
+    };
+    const int t0 = hd->t_done;
+    int t = t0;
+    for (; t < stop_after && hd->wide_live && t < K; ++t) {  // wide phase, step-major over all blocks
+        one_step(t, 0, nb);
+        hd->cur ^= 1;
+    }
+    if (hd->wide_live && t < stop_after) {  // leave the wide phase only when fp32 steps follow
+        launch_narrow(hd, false);
+        hd->wide_live = false;
+    }
+    if (nb == 1 || hd->opt_steps_per_block == 1) {
+        for (; t < stop_after; ++t) {
+            one_step(t, 0, nb);
+            hd->cur ^= 1;
+        }
+    } else if (t < stop_after) {
+        // replica blocks are independent: run a run of steps on one block while its state is L2-resident
+        const int span = hd->opt_steps_per_block > 0 ? (int)hd->opt_steps_per_block : std::max(1, stop_after - t);
+        for (int ta = t; ta < stop_after; ta += span) {
+            const int tb = std::min(stop_after, ta + span);
+            const int cur0 = hd->cur;
+            for (int b = 0; b < nb; ++b) {
+                hd->cur = cur0;
+                for (int tt = ta; tt < tb; ++tt) {
+                    one_step(tt, b, 1);
+                    hd->cur ^= 1;
+                }
+            }
+            hd->cur = cur0 ^ ((tb - ta) & 1);
+        }
+    }
+    if (stop_after > t0) {
+        hd->lambda_last = sch->lambda ? sch->lambda[stop_after - 1] : hd->pb.lambda;
+        hd->readout_valid = false;
+    }
+    hd->t_done = stop_after;
+    if (!cuda_ok(hd, cudaGetLastError(), "kernel launch")) return FEM_ECUDA;
+    return FEM_OK;
+}
+
+fem_status fem_readout(fem_handle *h) {
+    Handle *hd = reinterpret_cast<Handle *>(h);
+    if (!hd) return FEM_EINVAL;
+    if (hd->R < 1) return fail(hd, FEM_ESTATE, "no fields yet");
+    launch_readout(hd, hd->lambda_last);
+    hd->readout_valid = true;
+    if (!cuda_ok(hd, cudaGetLastError(), "kernel launch")) return FEM_ECUDA;
+    return FEM_OK;
+}
+
+fem_status fem_result(fem_handle *h, int32_t *best_replica, int32_t *best_config, int64_t *energy_int, double *energy,
+                      int32_t *part_sizes) {
+    Handle *hd = reinterpret_cast<Handle *>(h);
+    if (!hd) return FEM_EINVAL;
+    if (!hd->readout_valid) {
+        fem_status st = fem_readout(h);
+        if (st != FEM_OK) return st;
+    }
+    bool ok = true;
+    auto down = [&](void *dst, const void *src, size_t bytes) {
+        if (ok && dst) ok = cuda_ok(hd, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, hd->stream), "download result");
+    };
+    down(best_replica, hd->best, 4);
+    down(best_config, hd->best + 1, (size_t)hd->dp.n * 4);
+    down(energy_int, hd->e_int, (size_t)hd->R * 8);
+    down(energy, hd->e_real, (size_t)hd->R * 8);
+    down(part_sizes, hd->part, (size_t)hd->R * hd->dp.q * 4);
+    if (ok) ok = cuda_ok(hd, cudaStreamSynchronize(hd->stream), "fem_result synchronize");
+    return ok ? FEM_OK : FEM_ECUDA;
+}
+
+fem_status fem_get_configs(fem_handle *h, int32_t *cfg) {
+    Handle *hd = reinterpret_cast<Handle *>(h);
+    if (!hd || !cfg) return FEM_EINVAL;
+    if (!hd->readout_valid) {
+        fem_status st = fem_readout(h);
+        if (st != FEM_OK) return st;
+    }
+    int *logical = reinterpret_cast<int *>(hd->stage);
+    launch_cfg_out(hd, logical);
+    if (!cuda_ok(hd, cudaMemcpyAsync(cfg, logical, (size_t)hd->dp.n * hd->R * 4, cudaMemcpyDeviceToHost, hd->stream), "download configs")) return FEM_ECUDA;
+    if (!cuda_ok(hd, cudaStreamSynchronize(hd->stream), "synchronize")) return FEM_ECUDA;
+    return FEM_OK;
+}
+
+fem_status fem_energy_of(fem_handle *h, const int32_t *cfg, int32_t count, int64_t *energy_int, double *energy,
+                         int32_t *part_sizes) {
+    Handle *hd = reinterpret_cast<Handle *>(h);
+    if (!hd || !cfg) return FEM_EINVAL;
+    if (count < 1 || count > hd->R_cap) return fail(hd, FEM_EINVAL, "count must be in 1..R_cap");
+    for (int64_t k = 0; k < (int64_t)count * hd->dp.n; ++k)
+        if (cfg[k] < 0 || cfg[k] >= hd->dp.q) return fail(hd, FEM_EINVAL, "state out of range");
+    int *logical = reinterpret_cast<int *>(hd->stage);
+    bool ok = cuda_ok(hd, cudaMemcpyAsync(logical, cfg, (size_t)count * hd->dp.n * 4, cudaMemcpyHostToDevice, hd->stream), "upload configs");
+    if (!ok) return FEM_ECUDA;
+    launch_cfg_in(hd, logical, count);
+    launch_energy_of(hd, count, hd->lambda_last);
+    hd->readout_valid = false;  // the device configuration buffer now holds the caller's configurations
+    auto down = [&](void *dst, const void *src, size_t bytes) {
+        if (ok && dst) ok = cuda_ok(hd, cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, hd->stream), "download energies");
+    };
+    down(energy_int, hd->e_int, (size_t)count * 8);
+    down(energy, hd->e_real, (size_t)count * 8);
+    down(part_sizes, hd->part, (size_t)count * hd->dp.q * 4);
+    if (ok) ok = cuda_ok(hd, cudaStreamSynchronize(hd->stream), "fem_energy_of synchronize");
+    return ok ? FEM_OK : FEM_ECUDA;
+}
+
+}  // extern "C"

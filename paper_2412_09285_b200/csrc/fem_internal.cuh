@@ -1,0 +1,135 @@
+// Internal declarations of libfem_b200 (not part of the ABI; see include/fem.h).
+//
+// Device layout.  R replicas are split into NB = R / Rb replica blocks of
+// Rb replicas (Rb = R unless the "replica_block" option is set).  Inside a block a field
+// (variable i, state s, replica r) lives at  (i*F + s)*Rb + r  -- replica innermost, so the row
+// of a variable is F*Rb contiguous floats and a neighbour gather is one coalesced, vectorised row
+// (north_star subsystem 1; the paper's listing keeps replicas outermost).  Every
+// per-block array has (n*F + 1) rows: the extra last row of the gather buffers is the constant 1
+// that pads short Max-SAT clauses.  Blocks are blk_stride = (n*F+1)*Rb floats apart.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/fem.h"
+
+namespace fem {
+
+constexpr int kThreads = 256;
+constexpr int kMaxQ = 32;
+constexpr int kMaxClauseLen = 8;
+
+// Per-step scalars, computed on the host in double and narrowed in-kernel.
+struct StepScalars {
+    double inv_beta;   // 1 / beta_t
+    double step_size;  // lr / (1 - beta1^(t+1))
+    double rsqrt_bc2;  // 1 / sqrt(1 - beta2^(t+1))
+    double eps, b1, b2, one_minus_b1, one_minus_b2, wd;
+    double two_lambda;  // Potts balance term 2*lambda_t
+};
+
+// Device view of the problem (pointers into the workspace).
+struct DevProblem {
+    int kind, n, q, F;
+    // graph kinds
+    const int *row_ptr;  // [n+1]
+    const int *col;      // [nnz]
+    const float *w;      // [nnz] or nullptr (= +1)
+    int uniform_deg;     // > 0 when every row has this many entries
+    int64_t nnz;
+    const float *J;  // dense Ising, n*n
+    // Max-SAT, variable-centric: occurrences of variable i are occ_ptr[i]..occ_ptr[i+1]; occurrence o
+    // holds kstride = kmax-1 packed entries: (var << 1 | negated) of the OTHER literals of its clause,
+    // padded with (n << 1 | 1) (the constant-1 row); bit 31 of entry 0 = own literal is positive.
+    int m, kstride;
+    const int *occ_ptr;
+    const int *occ;
+    const int *clause_ptr;  // [m+1], for the unsat count
+    const int *lits;        // signed 1-based
+};
+
+// One replica block's state arrays (block base pointers; a launch with gridDim.y > 1 walks blocks).
+// T = float (bulk) or double (wide phase).
+template <typename T>
+struct BlockArrays {
+    T *h, *m1, *m2;
+    const T *g_in;  // gathered quantity of step t: m = tanh(h/2) (two-state kinds), D = P - 1/q (Potts)
+    T *g_out;       // same for step t+1
+    int64_t blk_stride;
+    int Rb;
+};
+
+struct Handle {
+    fem_problem pb{};  // host copy of scalars only (pointers nulled)
+    DevProblem dp{};
+    cudaStream_t stream = nullptr;
+    int R_cap = 0, R = 0, Rb = 0;
+    int64_t rows = 0;  // n*F + 1
+    bool integral_weights = true;
+    // workspace carve-up (device pointers)
+    float *h = nullptr, *m1 = nullptr, *m2 = nullptr, *g[2] = {nullptr, nullptr}, *stage = nullptr;
+    // wide phase (first precise_steps steps): the same five arrays in fp64
+    double *hW = nullptr, *m1W = nullptr, *m2W = nullptr, *gW[2] = {nullptr, nullptr};
+    bool wide_live = false;                  // the fp64 arrays hold the current state
+    float *field = nullptr;                  // dense Ising: J*m scratch [rows*R_cap] (fp64 in the wide phase: 2x)
+    double *colsum[2] = {nullptr, nullptr};  // Potts S[q][R]
+    double *colpart = nullptr;               // [kColBlocks][q*R]
+    int8_t *cfg = nullptr;                   // [rows*R_cap]
+    long long *e_part_i = nullptr;
+    double *e_part_d = nullptr;
+    int *part_part = nullptr;
+    long long *e_int = nullptr;
+    double *e_real = nullptr;
+    int *part = nullptr;
+    int *best = nullptr;  // [0] = best replica, [1..n] = its configuration
+    int cur = 0;          // g[cur] holds the gathered quantity of the current fields
+    int t_done = 0;
+    bool injected = false, readout_valid = false, gather_valid = false;
+    int64_t opt_replica_block = 0, opt_steps_per_block = 0;
+    int64_t launches = 0;
+    int64_t structure_bytes = 0;  // problem-structure bytes one step reads (indices, weights, clause entries)
+    double lambda_last = 0.0;     // balance weight of the last executed step (readout uses it)
+    std::string err;
+};
+
+constexpr int kColBlocks = 592;     // Potts column-sum partial blocks (4 per SM)
+constexpr int kEnergyChunks = 1184;  // readout partials per replica (8 node slots x 148 blocks)
+
+// ---- launchers implemented in the .cu files (all asynchronous on hd->stream) ----
+void launch_init_fields(Handle *hd, uint64_t seed, double scale);
+void launch_zero_moments(Handle *hd);
+void launch_widen(Handle *hd);   // fp32 h -> fp64 hW, zero wide moments
+void launch_narrow(Handle *hd, bool fields_only);  // fp64 state -> fp32 arrays
+void launch_transpose_in(Handle *hd, const float *logical_dev, float *dst);  // [R][n][F] -> device layout
+void launch_transpose_out(Handle *hd, const float *src, float *logical_dev);
+void launch_transpose_out_wide(Handle *hd, const double *src, float *logical_dev);
+void launch_readout(Handle *hd, double lambda);
+void launch_energy_of(Handle *hd, int count, double lambda);  // energies of hd->cfg (count replicas)
+void launch_cfg_in(Handle *hd, const int *cfg_logical_dev, int count);
+void launch_cfg_out(Handle *hd, int *cfg_logical_dev);
+
+inline int64_t ceil_div(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+}  // namespace fem
+
+namespace fem {
+// typed views of the live state arrays
+template <typename T> struct StateOf;
+template <> struct StateOf<float> {
+    static float *h(Handle *d) { return d->h; }
+    static float *m1(Handle *d) { return d->m1; }
+    static float *m2(Handle *d) { return d->m2; }
+    static float *g(Handle *d, int k) { return d->g[k]; }
+    static float *field(Handle *d) { return d->field; }
+};
+template <> struct StateOf<double> {
+    static double *h(Handle *d) { return d->hW; }
+    static double *m1(Handle *d) { return d->m1W; }
+    static double *m2(Handle *d) { return d->m2W; }
+    static double *g(Handle *d, int k) { return d->gW[k]; }
+    static double *field(Handle *d) { return reinterpret_cast<double *>(d->field); }
+};
+}  // namespace fem

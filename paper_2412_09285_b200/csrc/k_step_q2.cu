@@ -1,0 +1,262 @@
+// Fused annealing step for the two-state kinds (MaxCut, sparse/dense Ising, Max-SAT).
+//
+// One thread owns VEC consecutive replicas of one variable and does, in registers, rows a1-a4 of
+// the coupling contraction over the variable's CSR row (a coalesced VEC-wide
+// gather of m_j = tanh(h_j/2) per neighbour, S30 PAPER.md:671) or the clause leave-one-out products
+// (S28 PAPER.md:650, from the same m_j: the literal-false probabilities are (1 -+ m_j)/2), the entropy
+// gradient h/beta and chain rule (S29 PAPER.md:667), Adam, and the next step's gathered
+// quantity.  No gradient ever reaches HBM.  The step is synchronous (Jacobi): gathers read g_in (from
+// h(t)), results go to g_out.  T is both the arithmetic and the storage type: float for the bulk of the
+// anneal, double for the wide phase of the first precise_steps steps.
+#include "device_math.cuh"
+
+namespace fem {
+
+template <typename T>
+struct Q2Params {
+    BlockArrays<T> a;
+    DevProblem dp;
+    StepScalars sc;
+    const T *field;  // dense Ising: precomputed J*m, same layout as h
+    int rv;          // Rb / VEC
+    int64_t total;   // n * rv
+};
+
+enum { MODE_MAXCUT = 0, MODE_ISING = 1, MODE_SAT = 3, MODE_FIELD = 4 };
+
+template <typename T, int VEC, int MODE, int DEG>
+__global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) {
+    using R = Row<T, VEC>;
+    const int64_t idx = (int64_t)blockIdx.x * kThreads + threadIdx.x;
+    if (idx >= p.total) return;
+    const int i = (int)(idx / p.rv);
+    const int c = (int)(idx - (int64_t)i * p.rv) * VEC;
+    const int64_t blk = (int64_t)blockIdx.y * p.a.blk_stride;
+    const int Rb = p.a.Rb;
+    const int64_t off = blk + (int64_t)i * Rb + c;
+    const T *__restrict__ gin = p.a.g_in + blk + c;
+
+    // issue the streaming loads first so they overlap the dependent gather chain
+    const R h4 = R::ld_stream(p.a.h + off);
+    R m1 = R::ld_stream(p.a.m1 + off);
+    R m2 = R::ld_stream(p.a.m2 + off);
+
+    T dU[VEC];
+#pragma unroll
+    for (int v = 0; v < VEC; ++v) dU[v] = (T)0;
+
+    if (MODE == MODE_MAXCUT || MODE == MODE_ISING) {
+        const int *__restrict__ col = p.dp.col;
+        const float *__restrict__ w = p.dp.w;
+        if (DEG > 0) {
+            const int e0 = i * DEG;
+            R nb[DEG > 0 ? DEG : 1];
+            float wj[DEG > 0 ? DEG : 1];
+#pragma unroll
+            for (int k = 0; k < DEG; ++k) {
+                const int j = __ldg(col + e0 + k);
+                wj[k] = w ? __ldg(w + e0 + k) : 1.0f;
+                nb[k] = R::ld(gin + (int64_t)j * Rb);
+            }
+#pragma unroll
+            for (int k = 0; k < DEG; ++k)
+#pragma unroll
+                for (int v = 0; v < VEC; ++v) dU[v] += (T)wj[k] * nb[k].v[v];
+        } else {
+            const int e0 = __ldg(p.dp.row_ptr + i), e1 = __ldg(p.dp.row_ptr + i + 1);
+#pragma unroll 4
+            for (int e = e0; e < e1; ++e) {
+                const int j = __ldg(col + e);
+                const float wj = w ? __ldg(w + e) : 1.0f;
+                const R nb = R::ld(gin + (int64_t)j * Rb);
+#pragma unroll
+                for (int v = 0; v < VEC; ++v) dU[v] += (T)wj * nb.v[v];
+            }
+        }
+        if (MODE == MODE_ISING) {
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) dU[v] = (T)-2 * dU[v];  // dU/dp = 2 dU/dm = -2 sum_j J_ij m_j
+        }
+    } else if (MODE == MODE_FIELD) {
+        const R f = R::ld_stream(p.field + off);
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) dU[v] = (T)-2 * f.v[v];
+    } else {  // MODE_SAT: dU/dp_i = sum_{m ni i} s_mi prod_{k != i} u_mk
+        const int o0 = __ldg(p.dp.occ_ptr + i), o1 = __ldg(p.dp.occ_ptr + i + 1);
+        const int ks = p.dp.kstride;
+        for (int o = o0; o < o1; ++o) {
+            const int *__restrict__ ent = p.dp.occ + (int64_t)o * ks;
+            T prod[VEC];
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) prod[v] = (T)1;
+            int first = 0;
+            for (int x = 0; x < ks; ++x) {
+                int pk = __ldg(ent + x);
+                if (x == 0) first = pk;
+                pk &= 0x7fffffff;
+                const R mr = R::ld(gin + (int64_t)(pk >> 1) * Rb);
+                // probability the literal is false: 1-p = (1-m)/2 (positive literal), p = (1+m)/2 (negated)
+                const T sg = (pk & 1) ? (T)0.5 : (T)-0.5;
+#pragma unroll
+                for (int v = 0; v < VEC; ++v) prod[v] *= (T)0.5 + sg * mr.v[v];
+            }
+            const bool positive = first < 0;  // bit 31
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) dU[v] += positive ? -prod[v] : prod[v];
+        }
+    }
+
+    const Sc<T> sc(p.sc);
+    R hn, gn;
+#pragma unroll
+    for (int v = 0; v < VEC; ++v) {
+        const T h = h4.v[v];
+        const T g = (dU[v] + h * sc.inv_beta) * p1mp_of(h);  // S29 with ln(p/(1-p)) = h
+        hn.v[v] = adam_update(h, g, m1.v[v], m2.v[v], sc);
+        gn.v[v] = mag_of(hn.v[v]);
+    }
+    hn.st_stream(p.a.h + off);
+    m1.st_stream(p.a.m1 + off);
+    m2.st_stream(p.a.m2 + off);
+    gn.st(p.a.g_out + off);
+}
+
+// Gathered quantity m = tanh(h/2) from the fields (used at t = 0 and after fem_set_fields); also writes
+// the constant-1 row that pads short clauses, in both gather buffers.
+template <typename T>
+__global__ void __launch_bounds__(kThreads) q2_prepare_kernel(const T *h, T *g, T *g_other, int64_t blk_stride, int Rb,
+                                                              int n, int nblocks) {
+    const int64_t per = (int64_t)n * Rb;
+    const int64_t idx = (int64_t)blockIdx.x * kThreads + threadIdx.x;
+    if (idx >= per * nblocks) return;
+    const int64_t b = idx / per, r = idx - b * per;
+    const int64_t off = b * blk_stride + r;
+    g[off] = (T)mag_of((double)h[off]);
+    if (r < Rb) {
+        g[b * blk_stride + per + r] = (T)1;
+        g_other[b * blk_stride + per + r] = (T)1;
+    }
+}
+
+// ---- dense Ising: field = J * m on CUDA cores (placeholder GEMM; the tcgen05 path replaces it) ----
+// C[n x Rb] = J[n x n] * M[n x Rb], all row-major.  64x64 tile, 16x16 threads, 4x4 micro-tile.
+template <typename T>
+__global__ void __launch_bounds__(256) dense_field_kernel(const float *__restrict__ J, const T *__restrict__ M,
+                                                          T *__restrict__ C, int n, int Rb) {
+    __shared__ T As[16][64 + 1];
+    __shared__ T Bs[16][64];
+    const int tx = threadIdx.x % 16, ty = threadIdx.x / 16;
+    const int row0 = blockIdx.y * 64, col0 = blockIdx.x * 64;
+    T acc[4][4] = {};
+    for (int k0 = 0; k0 < n; k0 += 16) {
+        for (int t = threadIdx.x; t < 64 * 16; t += 256) {
+            const int r = t / 16, k = t % 16;
+            const int gr = row0 + r, gk = k0 + k;
+            As[k][r] = (gr < n && gk < n) ? (T)J[(int64_t)gr * n + gk] : (T)0;
+        }
+        for (int t = threadIdx.x; t < 16 * 64; t += 256) {
+            const int k = t / 64, cc = t % 64;
+            const int gk = k0 + k, gc = col0 + cc;
+            Bs[k][cc] = (gk < n && gc < Rb) ? M[(int64_t)gk * Rb + gc] : (T)0;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            T a[4], b[4];
+#pragma unroll
+            for (int x = 0; x < 4; ++x) a[x] = As[k][ty * 4 + x];
+#pragma unroll
+            for (int x = 0; x < 4; ++x) b[x] = Bs[k][tx * 4 + x];
+#pragma unroll
+            for (int x = 0; x < 4; ++x)
+#pragma unroll
+                for (int y = 0; y < 4; ++y) acc[x][y] += a[x] * b[y];
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int x = 0; x < 4; ++x)
+#pragma unroll
+        for (int y = 0; y < 4; ++y) {
+            const int gr = row0 + ty * 4 + x, gc = col0 + tx * 4 + y;
+            if (gr < n && gc < Rb) C[(int64_t)gr * Rb + gc] = acc[x][y];
+        }
+}
+
+template <typename T, int VEC, int MODE>
+static void launch_q2_deg(Handle *hd, const Q2Params<T> &p, dim3 grid) {
+    const int d = (MODE == MODE_MAXCUT || MODE == MODE_ISING) ? hd->dp.uniform_deg : 0;
+    if (d == 3)
+        step_q2_kernel<T, VEC, MODE, 3><<<grid, kThreads, 0, hd->stream>>>(p);
+    else if (d == 4)
+        step_q2_kernel<T, VEC, MODE, 4><<<grid, kThreads, 0, hd->stream>>>(p);
+    else
+        step_q2_kernel<T, VEC, MODE, 0><<<grid, kThreads, 0, hd->stream>>>(p);
+}
+
+template <typename T, int VEC>
+static void launch_q2_mode(Handle *hd, const Q2Params<T> &p, dim3 grid, int mode) {
+    switch (mode) {
+        case MODE_MAXCUT: launch_q2_deg<T, VEC, MODE_MAXCUT>(hd, p, grid); break;
+        case MODE_ISING: launch_q2_deg<T, VEC, MODE_ISING>(hd, p, grid); break;
+        case MODE_SAT: launch_q2_deg<T, VEC, MODE_SAT>(hd, p, grid); break;
+        default: launch_q2_deg<T, VEC, MODE_FIELD>(hd, p, grid); break;
+    }
+}
+
+template <typename T>
+static void launch_step_q2_t(Handle *hd, const StepScalars &sc, int blk_begin, int blk_count) {
+    using S = StateOf<T>;
+    const int Rb = hd->Rb;
+    const int64_t base = (int64_t)blk_begin * hd->rows * Rb;
+    Q2Params<T> p;
+    p.a.h = S::h(hd) + base;
+    p.a.m1 = S::m1(hd) + base;
+    p.a.m2 = S::m2(hd) + base;
+    p.a.g_in = S::g(hd, hd->cur) + base;
+    p.a.g_out = S::g(hd, hd->cur ^ 1) + base;
+    p.a.blk_stride = hd->rows * Rb;
+    p.a.Rb = Rb;
+    p.dp = hd->dp;
+    p.sc = sc;
+    p.field = nullptr;
+    int mode = hd->dp.kind == FEM_MAXCUT ? MODE_MAXCUT : hd->dp.kind == FEM_MAXSAT ? MODE_SAT : MODE_ISING;
+    if (hd->dp.kind == FEM_ISING && hd->dp.J) {
+        mode = MODE_FIELD;
+        p.field = S::field(hd) + base;
+        const int n = hd->dp.n;
+        dim3 g((unsigned)ceil_div(Rb, 64), (unsigned)ceil_div(n, 64));
+        for (int b = 0; b < blk_count; ++b) {
+            const int64_t o = (int64_t)b * p.a.blk_stride;
+            dense_field_kernel<T><<<g, 256, 0, hd->stream>>>(hd->dp.J, p.a.g_in + o, S::field(hd) + base + o, n, Rb);
+            hd->launches++;
+        }
+    }
+    const int VEC = (Rb % 4 == 0) ? 4 : 1;
+    p.rv = Rb / VEC;
+    p.total = (int64_t)hd->dp.n * p.rv;
+    dim3 grid((unsigned)ceil_div(p.total, kThreads), (unsigned)blk_count);
+    if (VEC == 4) launch_q2_mode<T, 4>(hd, p, grid, mode);
+    else launch_q2_mode<T, 1>(hd, p, grid, mode);
+    hd->launches++;
+}
+
+void launch_step_q2(Handle *hd, const StepScalars &sc, bool wide, int blk_begin, int blk_count) {
+    if (wide) launch_step_q2_t<double>(hd, sc, blk_begin, blk_count);
+    else launch_step_q2_t<float>(hd, sc, blk_begin, blk_count);
+}
+
+void launch_prepare_q2(Handle *hd, bool wide) {
+    const int nb = hd->R / hd->Rb;
+    const int64_t total = (int64_t)hd->dp.n * hd->Rb * nb;
+    const unsigned grid = (unsigned)ceil_div(total, kThreads);
+    if (wide)
+        q2_prepare_kernel<double><<<grid, kThreads, 0, hd->stream>>>(hd->hW, hd->gW[hd->cur], hd->gW[hd->cur ^ 1],
+                                                                     hd->rows * hd->Rb, hd->Rb, hd->dp.n, nb);
+    else
+        q2_prepare_kernel<float><<<grid, kThreads, 0, hd->stream>>>(hd->h, hd->g[hd->cur], hd->g[hd->cur ^ 1],
+                                                                    hd->rows * hd->Rb, hd->Rb, hd->dp.n, nb);
+    hd->launches++;
+}
+
+}  // namespace fem

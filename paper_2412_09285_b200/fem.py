@@ -1,0 +1,264 @@
+"""Python binding of include/fem.h: argument marshalling only.
+
+Every step of the path (init, fused annealing steps, rounding, energies, argmin) runs in the CUDA
+kernels of csrc/libfem_b200.so.  PyTorch provides the device workspace and the stream, nothing else.
+If the library is missing or there is no CUDA device this module raises; there is no CPU fallback.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+
+from . import workloads as wl
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "csrc", "libfem_b200.so")
+
+FEM_OK, FEM_EINVAL, FEM_ENOMEM, FEM_ECUDA, FEM_ESTATE = range(5)
+STATUS_NAMES = {0: "FEM_OK", 1: "FEM_EINVAL", 2: "FEM_ENOMEM", 3: "FEM_ECUDA", 4: "FEM_ESTATE"}
+
+EXPORTS = [
+    "fem_abi_version", "fem_workspace_bytes", "fem_create", "fem_anneal", "fem_reset", "fem_readout", "fem_result",
+    "fem_set_fields", "fem_get_fields", "fem_get_moments", "fem_get_marginals", "fem_get_configs", "fem_energy_of",
+    "fem_set_option", "fem_get_info", "fem_last_error", "fem_destroy",
+]
+
+
+class FemError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"{STATUS_NAMES.get(status, status)}: {message}")
+        self.status = status
+
+
+class CProblem(C.Structure):
+    _fields_ = [
+        ("kind", C.c_int32), ("n", C.c_int32), ("q", C.c_int32),
+        ("row_ptr", C.c_void_p), ("col_idx", C.c_void_p), ("weight", C.c_void_p), ("dense_J", C.c_void_p),
+        ("m", C.c_int32), ("clause_ptr", C.c_void_p), ("lits", C.c_void_p), ("lambda_", C.c_double),
+    ]
+
+
+class CSchedule(C.Structure):
+    _fields_ = [
+        ("steps", C.c_int32), ("beta", C.c_void_p), ("lambda_", C.c_void_p),
+        ("lr", C.c_double), ("beta1", C.c_double), ("beta2", C.c_double), ("eps", C.c_double),
+        ("weight_decay", C.c_double), ("init_scale", C.c_double), ("precise_steps", C.c_int32),
+    ]
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen csrc/libfem_b200.so (built by paper_2412_09285_b200.build); loud failure if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2412_09285_b200.build` "
+                          "(there is no CPU fallback for the FEM path)")
+    lib = C.CDLL(LIB_PATH)
+    lib.fem_abi_version.restype = C.c_int32
+    lib.fem_workspace_bytes.restype = C.c_size_t
+    lib.fem_workspace_bytes.argtypes = [C.POINTER(CProblem), C.c_int32]
+    lib.fem_create.argtypes = [C.POINTER(CProblem), C.c_int32, C.c_void_p, C.c_size_t, C.c_void_p,
+                               C.POINTER(C.c_void_p)]
+    lib.fem_anneal.argtypes = [C.c_void_p, C.POINTER(CSchedule), C.c_int32, C.c_uint64, C.c_int32]
+    lib.fem_reset.argtypes = [C.c_void_p]
+    lib.fem_readout.argtypes = [C.c_void_p]
+    lib.fem_result.argtypes = [C.c_void_p] + [C.c_void_p] * 5
+    lib.fem_set_fields.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
+    lib.fem_get_fields.argtypes = [C.c_void_p, C.c_void_p]
+    lib.fem_get_moments.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.fem_get_marginals.argtypes = [C.c_void_p, C.c_void_p]
+    lib.fem_get_configs.argtypes = [C.c_void_p, C.c_void_p]
+    lib.fem_energy_of.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.fem_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_int64]
+    lib.fem_get_info.restype = C.c_int64
+    lib.fem_get_info.argtypes = [C.c_void_p, C.c_char_p]
+    lib.fem_last_error.restype = C.c_char_p
+    lib.fem_last_error.argtypes = [C.c_void_p]
+    lib.fem_destroy.argtypes = [C.c_void_p]
+    _lib = lib
+    return lib
+
+
+def _ptr(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+@dataclass
+class Schedule:
+    """Host-side schedule: beta[t] (and optional lambda[t]) plus Adam settings."""
+    beta: np.ndarray
+    lr: float = 0.1
+    beta1: float = 0.9
+    beta2: float = 0.999
+    eps: float = 1e-8
+    weight_decay: float = 0.0
+    init_scale: float = 1e-3
+    precise_steps: int = 8
+    lam: Optional[np.ndarray] = None
+
+    def c(self) -> CSchedule:
+        self.beta = np.ascontiguousarray(self.beta, dtype=np.float64)
+        if self.lam is not None:
+            self.lam = np.ascontiguousarray(self.lam, dtype=np.float64)
+        return CSchedule(int(self.beta.size), _ptr(self.beta), _ptr(self.lam), self.lr, self.beta1, self.beta2, self.eps,
+                         self.weight_decay, self.init_scale, self.precise_steps)
+
+
+def linear_temperature_schedule(T_max: float, T_min: float, steps: int) -> np.ndarray:
+    """Inverse-proportional schedule: T linear from T_max to T_min; returns beta[t] = 1/T(t)."""
+    t = np.arange(steps, dtype=np.float64)
+    T = T_max + (T_min - T_max) * t / max(steps - 1, 1)
+    return 1.0 / T
+
+
+def exponential_schedule(beta_min: float, beta_max: float, steps: int) -> np.ndarray:
+    """Exponential schedule."""
+    t = np.arange(steps, dtype=np.float64) / max(steps - 1, 1)
+    return np.exp((np.log(beta_max) - np.log(beta_min)) * t + np.log(beta_min))
+
+
+class Fem:
+    """One problem instance resident on a CUDA device (fem_create .. fem_destroy)."""
+
+    def __init__(self, inst: wl.Instance, R_cap: int, device: str = "cuda:0", stream=None):
+        import torch  # device memory and streams only
+
+        self._lib = load_library()
+        if not torch.cuda.is_available():
+            raise FemError(FEM_ECUDA, "no CUDA device: the FEM path has no CPU fallback")
+        self.inst = inst
+        self.R_cap = int(R_cap)
+        self.device = torch.device(device)
+        self._keep = []
+
+        def host(a, dt):
+            if a is None:
+                return None
+            a = np.ascontiguousarray(a, dtype=dt)
+            self._keep.append(a)
+            return a
+
+        self._cp = CProblem(inst.kind, inst.n, inst.q, _ptr(host(inst.row_ptr, np.int64)),
+                            _ptr(host(inst.col_idx, np.int32)), _ptr(host(inst.weight, np.float32)),
+                            _ptr(host(inst.dense_J, np.float32)), inst.m, _ptr(host(inst.clause_ptr, np.int64)),
+                            _ptr(host(inst.lits, np.int32)), float(inst.lam))
+        nbytes = self._lib.fem_workspace_bytes(C.byref(self._cp), self.R_cap)
+        if nbytes == 0:
+            raise FemError(FEM_EINVAL, "fem_workspace_bytes rejected the problem")
+        self.workspace_bytes = int(nbytes)
+        with torch.cuda.device(self.device):
+            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = self._ws.data_ptr()
+            self._ws_ptr = (base + 255) & ~255
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            h = C.c_void_p()
+            st = self._lib.fem_create(C.byref(self._cp), self.R_cap, C.c_void_p(self._ws_ptr), C.c_size_t(nbytes),
+                                      C.c_void_p(self.stream.cuda_stream), C.byref(h))
+        if st != FEM_OK:
+            raise FemError(st, (self._lib.fem_last_error(None) or b"").decode())
+        self._h = h
+        self.R = 0
+
+    # -- plumbing
+    def _check(self, st: int):
+        if st != FEM_OK:
+            raise FemError(st, (self._lib.fem_last_error(self._h) or b"").decode())
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.fem_destroy(self._h)
+            self._h = None
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def F(self) -> int:
+        return self.inst.fields_per_var
+
+    def _shape(self, R: int):
+        return (R, self.inst.n, self.F) if self.F > 1 else (R, self.inst.n)
+
+    # -- the three calls of the path
+    def anneal(self, schedule: Schedule, R: int, seed: int = 0, stop_after: Optional[int] = None) -> None:
+        cs = schedule.c()
+        stop = cs.steps if stop_after is None else int(stop_after)
+        self._check(self._lib.fem_anneal(self._h, C.byref(cs), int(R), C.c_uint64(seed), stop))
+        self.R = int(R)
+
+    def readout(self) -> None:
+        self._check(self._lib.fem_readout(self._h))
+
+    def result(self):
+        """-> dict(best_replica, best_config[n], energy_int[R], energy[R], part_sizes[R,q])"""
+        R, n, q = self.R, self.inst.n, self.inst.q
+        best = np.zeros(1, dtype=np.int32)
+        cfg = np.empty(n, dtype=np.int32)
+        e_int = np.empty(R, dtype=np.int64)
+        e = np.empty(R, dtype=np.float64)
+        part = np.empty((R, q), dtype=np.int32)
+        self._check(self._lib.fem_result(self._h, _ptr(best), _ptr(cfg), _ptr(e_int), _ptr(e), _ptr(part)))
+        return {"best_replica": int(best[0]), "best_config": cfg, "energy_int": e_int, "energy": e, "part_sizes": part}
+
+    def reset(self) -> None:
+        self._check(self._lib.fem_reset(self._h))
+
+    # -- parity hooks
+    def set_fields(self, h0: np.ndarray) -> None:
+        h0 = np.ascontiguousarray(h0, dtype=np.float32)
+        R = h0.size // (self.inst.n * self.F)
+        self._check(self._lib.fem_set_fields(self._h, R, _ptr(h0)))
+        self.R = R
+
+    def get_fields(self) -> np.ndarray:
+        out = np.empty(self._shape(self.R), dtype=np.float32)
+        self._check(self._lib.fem_get_fields(self._h, _ptr(out)))
+        return out
+
+    def get_moments(self):
+        m1 = np.empty(self._shape(self.R), dtype=np.float32)
+        m2 = np.empty(self._shape(self.R), dtype=np.float32)
+        self._check(self._lib.fem_get_moments(self._h, _ptr(m1), _ptr(m2)))
+        return m1, m2
+
+    def get_marginals(self) -> np.ndarray:
+        out = np.empty(self._shape(self.R), dtype=np.float32)
+        self._check(self._lib.fem_get_marginals(self._h, _ptr(out)))
+        return out
+
+    def get_configs(self) -> np.ndarray:
+        out = np.empty((self.R, self.inst.n), dtype=np.int32)
+        self._check(self._lib.fem_get_configs(self._h, _ptr(out)))
+        return out
+
+    def energy_of(self, cfg: np.ndarray):
+        cfg = np.ascontiguousarray(cfg, dtype=np.int32).reshape(-1, self.inst.n)
+        count = cfg.shape[0]
+        e_int = np.empty(count, dtype=np.int64)
+        e = np.empty(count, dtype=np.float64)
+        part = np.empty((count, self.inst.q), dtype=np.int32)
+        self._check(self._lib.fem_energy_of(self._h, _ptr(cfg), count, _ptr(e_int), _ptr(e), _ptr(part)))
+        return e_int, e, part
+
+    def set_option(self, key: str, value: int) -> None:
+        self._check(self._lib.fem_set_option(self._h, key.encode(), int(value)))
+
+    def info(self, key: str) -> int:
+        return int(self._lib.fem_get_info(self._h, key.encode()))
+
+
+def schedule_for(cfg: wl.Config, precise_steps: int = 8) -> Schedule:
+    return Schedule(beta=linear_temperature_schedule(cfg.T_max, cfg.T_min, cfg.steps), lr=cfg.lr, beta1=cfg.beta1,
+                    beta2=cfg.beta2, eps=cfg.eps, init_scale=cfg.init_scale, precise_steps=precise_steps)

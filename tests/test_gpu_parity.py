@@ -1,0 +1,238 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element on the
+same seeded inputs.  Bars (north_star): integer energies bit-exact; marginals within 1e-4 absolute
+after the first 50 steps from identical initial fields; mean final energy within 0.5%."""
+import numpy as np
+import pytest
+
+from oracle import fem_oracle as fo
+from paper_2412_09285_b200 import workloads as wl
+from test_oracle_gradient import as_problem
+
+pytestmark = pytest.mark.gpu
+
+MARGINAL_TOL = 1e-4       # north_star: absolute, after 50 steps
+WIDE_TOL = 2e-7          # fp64 state on both sides; the marginals come back as fp32
+
+
+@pytest.fixture(scope="module")
+def fem():
+    from paper_2412_09285_b200 import fem as femlib
+    return femlib
+
+
+def small_instances():
+    reg = wl.random_regular(1500, 10, 2002, wl.BMINCUT, 8, lam=0.05 / 1500)
+    reg3 = wl.random_regular(999, 6, 2003, wl.BMINCUT, 3, lam=0.01)
+    er = wl.erdos_renyi_maxcut(300, 0.1, 2004, pm1=False)
+    potts_w = wl.Instance(wl.BMINCUT, er.n, 5, er.row_ptr, er.col_idx,
+                          (np.random.default_rng(1).integers(1, 4, er.nnz // 2).astype(np.float32))[
+                              edge_ids(er)], lam=0.02)
+    return {
+        "cfg0_maxcut_er800": (wl.CONFIGS["cfg0"].make(), 32),
+        "maxcut_torus_30x34": (wl.torus_maxcut(30, 2001, W=34), 24),
+        "maxcut_reg3_pm1": (wl.random_regular(5000, 3, 2005, wl.MAXCUT, pm1=True), 32),
+        "maxcut_er_odd_R": (wl.erdos_renyi_maxcut(257, 0.08, 2006, pm1=True), 7),
+        "ising_sparse": (wl.sparse_ising_from(wl.torus_maxcut(20, 2007), -0.5), 16),
+        "ising_dense_sk": (wl.sk_dense(200, 2008), 40),
+        "bmincut_q8_reg10": (reg, 16),
+        "bmincut_q3_reg6_odd_R": (reg3, 10),
+        "bmincut_q5_weighted": (potts_w, 12),
+        "maxsat_k4": (wl.random_ksat(600, 6000, 4, 2009), 16),
+        "maxsat_k3_odd_R": (wl.random_ksat(301, 1300, 3, 2010), 9),
+    }
+
+
+def edge_ids(inst):
+    """Index of the undirected edge of every CSR entry (so both directions get the same weight)."""
+    rows = np.repeat(np.arange(inst.n), np.diff(inst.row_ptr))
+    a, b = np.minimum(rows, inst.col_idx), np.maximum(rows, inst.col_idx)
+    _, inv = np.unique(a.astype(np.int64) * inst.n + b, return_inverse=True)
+    return inv
+
+
+INST = None
+
+
+def get(name):
+    global INST
+    if INST is None:
+        INST = small_instances()
+    return INST[name]
+
+
+NAMES = ["cfg0_maxcut_er800", "maxcut_torus_30x34", "maxcut_reg3_pm1", "maxcut_er_odd_R", "ising_sparse",
+         "ising_dense_sk", "bmincut_q8_reg10", "bmincut_q3_reg6_odd_R", "bmincut_q5_weighted", "maxsat_k4",
+         "maxsat_k3_odd_R"]
+
+
+def oracle_run(inst, h0, beta, steps, lam):
+    pb = as_problem(inst)
+    st = fo.State(pb, h0.astype(np.float64))
+    fo.anneal(st, beta, fo.Adam(), lam, t_end=steps)
+    return pb, st
+
+
+@pytest.mark.parametrize("name", NAMES)
+def test_marginals_after_50_steps(fem, name):
+    inst, R = get(name)
+    steps = 500
+    beta = fem.linear_temperature_schedule(1.0, 0.01, steps)
+    assert np.array_equal(beta, fo.schedule_inverse_proportional(1.0, 0.01, steps))
+    h0 = fo.init_fields(0, R, inst.n, inst.fields_per_var).astype(np.float32)
+    pb, st = oracle_run(inst, h0, beta, 50, inst.lam)
+    P_ref = fo.marginals(pb, st.h)
+    eng = fem.Fem(inst, R)
+    eng.set_fields(h0)
+    assert np.array_equal(eng.get_fields(), h0)                      # layout round trip is exact
+    # default launch configuration: wide (fp64) phase for the first 8 steps, fp32 afterwards
+    eng.anneal(fem.Schedule(beta=beta, precise_steps=8), R, stop_after=50)
+    P = eng.get_marginals().astype(np.float64)
+    err = np.max(np.abs(P - P_ref.reshape(P.shape)))
+    assert err < MARGINAL_TOL, err
+    assert np.max(np.abs(eng.get_fields() - st.h.reshape(P.shape))) < 1e-3
+    # wide phase over all 50 steps: the state is fp64 like the oracle's, only libm separates them
+    eng.set_fields(h0)
+    eng.anneal(fem.Schedule(beta=beta, precise_steps=50), R, stop_after=50)
+    err64 = np.max(np.abs(eng.get_marginals().astype(np.float64) - P_ref.reshape(P.shape)))
+    assert err64 < WIDE_TOL, err64
+    # ... and the fp32 bulk kernel on its own: ten more steps from that state
+    fo.anneal(st, beta, fo.Adam(), inst.lam, t_end=60)
+    eng.anneal(fem.Schedule(beta=beta, precise_steps=50), R, stop_after=60)
+    err60 = np.max(np.abs(eng.get_marginals().astype(np.float64) - fo.marginals(pb, st.h).reshape(P.shape)))
+    assert err60 < 2e-5, err60
+    eng.close()
+
+
+@pytest.mark.parametrize("name", NAMES)
+def test_first_steps_one_by_one(fem, name):
+    """Steps 1, 2, 5, 10, 20 against the oracle (the first Adam steps normalise tiny gradients and are the
+    sensitive ones), and resumability of fem_anneal."""
+    inst, R = get(name)
+    beta = fem.linear_temperature_schedule(1.0, 0.01, 500)
+    h0 = fo.init_fields(3, R, inst.n, inst.fields_per_var).astype(np.float32)
+    pb = as_problem(inst)
+    st = fo.State(pb, h0.astype(np.float64))
+    eng = fem.Fem(inst, R)
+    eng.set_fields(h0)
+    sch = fem.Schedule(beta=beta, precise_steps=8)
+    for stop in (1, 2, 5, 10, 20):
+        fo.anneal(st, beta, fo.Adam(), inst.lam, t_end=stop)
+        eng.anneal(sch, R, stop_after=stop)
+        P = eng.get_marginals().astype(np.float64)
+        err = np.max(np.abs(P - fo.marginals(pb, st.h).reshape(P.shape)))
+        assert err < MARGINAL_TOL, (stop, err)
+    m1, m2 = eng.get_moments()
+    assert np.max(np.abs(m1 - st.m1.reshape(m1.shape))) < 1e-4 * max(1.0, np.max(np.abs(st.m1)))
+    eng.close()
+
+
+@pytest.mark.parametrize("name", NAMES)
+def test_energies_bit_exact_on_random_configurations(fem, name):
+    inst, R = get(name)
+    pb = as_problem(inst)
+    rng = np.random.default_rng(11)
+    cfg = rng.integers(0, inst.q, size=(R, inst.n)).astype(np.int32)
+    cfg[0] = 0                                                      # degenerate: everything in one state
+    if R > 1:
+        cfg[1] = np.arange(inst.n) % inst.q
+    eng = fem.Fem(inst, R)
+    e_int, e, part = eng.energy_of(cfg)
+    r_int, r, rpart = fo.energies(pb, cfg, inst.lam)
+    if inst.kind == wl.ISING:
+        assert np.max(np.abs(e - r)) <= 1e-9 * max(1.0, np.max(np.abs(r)))
+    else:
+        assert np.array_equal(e_int, r_int)
+        assert np.array_equal(e, r)                                 # fp64 energy bit-exact (integral weights)
+    if inst.kind == wl.BMINCUT:
+        assert np.array_equal(part, rpart)
+    # fewer configurations than R_cap
+    e1 = eng.energy_of(cfg[:1])
+    assert e1[0][0] == e_int[0] and e1[1][0] == e[0]
+    eng.close()
+
+
+@pytest.mark.parametrize("name", ["cfg0_maxcut_er800", "bmincut_q8_reg10", "maxsat_k4", "ising_dense_sk"])
+def test_readout_is_consistent_and_deterministic(fem, name):
+    inst, R = get(name)
+    pb = as_problem(inst)
+    steps = 200
+    sch = fem.Schedule(beta=fem.linear_temperature_schedule(1.0, 0.01, steps))
+    outs = []
+    for _ in range(2):
+        eng = fem.Fem(inst, R)
+        eng.anneal(sch, R, seed=5)
+        res = eng.result()
+        cfg = eng.get_configs()
+        h = eng.get_fields()
+        outs.append((res, cfg, h))
+        eng.close()
+    (res, cfg, h), (res2, cfg2, h2) = outs
+    assert np.array_equal(h, h2) and np.array_equal(cfg, cfg2)       # bit-identical run to run
+    assert np.array_equal(res["energy"], res2["energy"])
+    # rounding rule on the final fields (reading R3) and energies of exactly those configurations
+    assert np.array_equal(cfg, fo.round_configs(pb, h.astype(np.float64)))
+    r_int, r, rpart = fo.energies(pb, cfg, inst.lam)
+    if inst.kind == wl.ISING:
+        assert np.max(np.abs(res["energy"] - r)) <= 1e-9 * np.max(np.abs(r))
+    else:
+        assert np.array_equal(res["energy_int"], r_int) and np.array_equal(res["energy"], r)
+    assert res["best_replica"] == int(np.argmin(res["energy"]))     # first minimum = lowest index on ties
+    assert np.array_equal(res["best_config"], cfg[res["best_replica"]])
+
+
+def test_seeded_initial_fields_match_oracle_generator(fem):
+    inst, R = get("maxcut_torus_30x34")
+    eng = fem.Fem(inst, R)
+    sch = fem.Schedule(beta=fem.linear_temperature_schedule(1.0, 0.01, 10))
+    eng.anneal(sch, R, seed=42, stop_after=0)
+    h = eng.get_fields()
+    ref = fo.init_fields(42, R, inst.n, 1).astype(np.float32)
+    ulp = np.abs(h.view(np.int32).astype(np.int64) - ref.view(np.int32).astype(np.int64))
+    assert ulp.max() <= 1 and np.mean(ulp == 0) > 0.999
+    # Potts layout and a replica subset: replica a does not depend on R
+    pinst, _ = get("bmincut_q3_reg6_odd_R")
+    e2 = fem.Fem(pinst, 10)
+    e2.anneal(sch, 4, seed=7, stop_after=0)
+    ref = fo.init_fields(7, 10, pinst.n, 3).astype(np.float32)[:4]
+    ulp = np.abs(e2.get_fields().view(np.int32).astype(np.int64) - ref.view(np.int32).astype(np.int64))
+    assert ulp.max() <= 1
+    eng.close(); e2.close()
+
+
+@pytest.mark.parametrize("name", ["maxcut_torus_30x34", "bmincut_q8_reg10", "maxsat_k4"])
+def test_replica_blocking_changes_nothing(fem, name):
+    """Replicas are independent, so running them in L2-sized blocks (any order of blocks and steps) must give
+    bit-identical fields."""
+    inst, R = get(name)
+    sch = fem.Schedule(beta=fem.linear_temperature_schedule(1.0, 0.01, 60))
+    ref = None
+    for blk, spb in ((0, 0), (R // 2, 1), (R // 2, 0), (R // 4, 7)):
+        eng = fem.Fem(inst, R)
+        eng.set_option("replica_block", blk)
+        eng.set_option("steps_per_block", spb)
+        eng.anneal(sch, R, seed=9)
+        h = eng.get_fields()
+        res = eng.result()
+        if ref is None:
+            ref = (h, res)
+        else:
+            assert np.array_equal(h, ref[0])
+            assert np.array_equal(res["energy"], ref[1]["energy"]) and res["best_replica"] == ref[1]["best_replica"]
+        eng.close()
+
+
+def test_full_anneal_energy_distribution_cfg0(fem):
+    """Config 0 in full: R=32, 500 steps; mean final energy over replicas within 0.5% of the oracle's."""
+    c = wl.CONFIGS["cfg0"]
+    inst = c.make()
+    pb = as_problem(inst)
+    beta = fem.linear_temperature_schedule(c.T_max, c.T_min, c.steps)
+    h0 = fo.init_fields(0, c.R, inst.n, 1).astype(np.float32)
+    st = fo.anneal(fo.State(pb, h0.astype(np.float64)), beta, fo.Adam())
+    ref = fo.energies(pb, fo.round_configs(pb, st.h))[0]
+    eng = fem.Fem(inst, c.R)
+    eng.anneal(fem.schedule_for(c), c.R, seed=0)
+    res = eng.result()
+    assert abs(res["energy_int"].mean() - ref.mean()) <= 0.005 * abs(ref.mean())
+    assert res["energy_int"].min() <= 0.995 * ref.min()              # energies are negative cuts
+    eng.close()
