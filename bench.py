@@ -1,0 +1,334 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the FEM annealing hot path on B200 (contract: see DESIGN.md section 9).
+
+One "step" of this benchmark is one pass of the WHOLE hot path over one batch of synthetic input:
+seeded initial fields, all annealing steps of the schedule (fused step kernel per step), rounding,
+per-replica energies and the best-replica argmin, for BASELINE.json configs[1] by default
+(MaxCut, 200x200 torus, +-1 weights, R = 256 replicas, 2000 annealing steps).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1] [--impl ours|reference]
+
+`value`  : variable-replica updates/s with the problem already resident in HBM (CUDA events).
+`e2e`    : the same metric through the public API from HOST buffers: fem_create (uploads the problem
+           from pinned host memory) + fem_anneal + fem_result (downloads energies and the best config).
+`roofline`: the fused fp32 step kernel, algorithmic bytes per launch / its mean launch duration measured
+           with CUDA events inside the timed region, against the measured HBM copy bandwidth.
+`cpu_baseline`: the oracle (oracle/fem_oracle.c, as it stands) on this box's host cores, bounded sample.
+N > 1: replicas are independent, so every rank anneals its own R replicas (weak scaling, no data-path
+collective); one tiny exchange at the end picks the best replica over all ranks (Eq.5).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "variable-replica updates/s"
+UNIT = "updates/s"
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md, 6.65 TB/s)"
+
+
+def load_traffic(workload: str):
+    """dram bytes per launch of the fused step kernel from the committed ncu capture, or None."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f).get(workload)
+    return None
+
+
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f:
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        os.unlink(self.f.name)
+        # under load = the upper half of the samples (idle samples before/after the region drop out)
+        sm_sorted = sorted(sm)
+        load = sm_sorted[len(sm_sorted) // 2:] if sm_sorted else []
+        return {"sm_mhz": float(np.median(load)) if load else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_sample(cfg, inst, seconds_target: float = 12.0):
+    """Time the oracle on a bounded sample of the workload: a few annealing steps at full n and R."""
+    from oracle import fem_oracle as fo
+    pb = fo.Problem(kind=inst.kind, n=inst.n, q=inst.q, row_ptr=inst.row_ptr, col_idx=inst.col_idx, weight=inst.weight,
+                    dense_J=inst.dense_J, m=inst.m, clause_ptr=inst.clause_ptr, lits=inst.lits)
+    beta = fo.schedule_inverse_proportional(cfg.T_max, cfg.T_min, cfg.steps)
+    h0 = fo.init_fields(cfg.field_seed, cfg.R, inst.n, inst.fields_per_var, cfg.init_scale)
+    adam = fo.Adam(cfg.lr, cfg.beta1, cfg.beta2, cfg.eps)
+    out = {}
+    for openmp in (False, True):
+        st = fo.State(pb, h0)
+        t0 = time.perf_counter()
+        fo.anneal(st, beta, adam, inst.lam, t_end=1, openmp=openmp)
+        one = time.perf_counter() - t0
+        nsteps = int(max(2, min(cfg.steps - 1, seconds_target / 2 / max(one, 1e-6))))
+        t0 = time.perf_counter()
+        fo.anneal(st, beta, adam, inst.lam, t_end=1 + nsteps, openmp=openmp)
+        dt = time.perf_counter() - t0
+        out[openmp] = (inst.n * cfg.R * nsteps / dt, nsteps, fo.num_threads(openmp))
+    return out
+
+
+def run_reference(args, cfg, inst):
+    """--impl reference: the oracle, as it stands, on the host cores; each step = a bounded sample."""
+    from oracle import fem_oracle as fo
+    pb = fo.Problem(kind=inst.kind, n=inst.n, q=inst.q, row_ptr=inst.row_ptr, col_idx=inst.col_idx, weight=inst.weight,
+                    dense_J=inst.dense_J, m=inst.m, clause_ptr=inst.clause_ptr, lits=inst.lits)
+    beta = fo.schedule_inverse_proportional(cfg.T_max, cfg.T_min, cfg.steps)
+    h0 = fo.init_fields(cfg.field_seed, cfg.R, inst.n, inst.fields_per_var, cfg.init_scale)
+    adam = fo.Adam(cfg.lr, cfg.beta1, cfg.beta2, cfg.eps)
+    st = fo.State(pb, h0)
+    t0 = time.perf_counter()
+    fo.anneal(st, beta, adam, inst.lam, t_end=1, openmp=True)
+    one = time.perf_counter() - t0
+    total = args.steps + args.warmup
+    per = int(max(1, min((cfg.steps - 1) // max(total, 1), 120.0 / total / max(one, 1e-6))))
+    t = 1
+    for _ in range(args.warmup):
+        fo.anneal(st, beta, adam, inst.lam, t_end=t + per, openmp=True)
+        t += per
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        fo.anneal(st, beta, adam, inst.lam, t_end=t + per, openmp=True)
+        t += per
+    dt = time.perf_counter() - t0
+    value = inst.n * cfg.R * per * args.steps / dt
+    cores = fo.num_threads(True)
+    sample = f"{per} annealing steps at full n={inst.n}, R={cfg.R} per bench step (of {cfg.steps})"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg.name, "note": "oracle/fem_oracle.c on host cores (OpenMP over replicas)"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cfg1")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--replica-block", type=int, default=None, help="override the replica_block option")
+    ap.add_argument("--steps-per-block", type=int, default=None)
+    ap.add_argument("--precise-steps", type=int, default=8)
+    ap.add_argument("--anneal-steps", type=int, default=None,
+                    help="shorten the schedule (profiling under ncu only; such a run is not a bench value)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+
+    from paper_2412_09285_b200 import workloads as wl
+    cfg = wl.CONFIGS[args.workload]
+    if args.anneal_steps is not None:
+        import dataclasses
+        cfg = dataclasses.replace(cfg, steps=args.anneal_steps, name=cfg.name + f" [schedule cut to {args.anneal_steps} steps]")
+
+    if args.impl == "reference":
+        if rank != 0:
+            return
+        run_reference(args, cfg, cfg.make())
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2412_09285_b200 import fem
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the FEM path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    inst = cfg.make()
+    R, N, n = cfg.R, cfg.steps, inst.n
+    sched = fem.schedule_for(cfg, precise_steps=args.precise_steps)
+    K = min(args.precise_steps, N)
+
+    def apply_options(eng):
+        if args.replica_block is not None:
+            eng.set_option("replica_block", args.replica_block)
+        if args.steps_per_block is not None:
+            eng.set_option("steps_per_block", args.steps_per_block)
+
+    eng = fem.Fem(inst, R, device=f"cuda:{local_rank}")
+    apply_options(eng)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > L2 (126 MB)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def one_pass(seed, ev=None):
+        """The whole hot path on resident inputs; `ev` collects (start, end) events around the fp32 bulk."""
+        flush.zero_()
+        eng.reset()
+        eng.anneal(sched, R, seed=seed, stop_after=K)          # init + wide phase
+        if ev is not None:
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            l0 = eng.info("launches")
+            a.record()
+        eng.anneal(sched, R, seed=seed, stop_after=N)          # launches of the fused fp32 step kernel (+1 narrowing)
+        if ev is not None:
+            b.record()
+            ev.append((a, b, eng.info("launches") - l0 - (1 if K > 0 else 0)))
+        eng.readout()                                          # rounding + energies + argmin
+
+    for w in range(args.warmup):
+        one_pass(1000 + rank * 131 + w)
+    barrier()
+    launches0 = eng.info("launches")
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    bulk_events = []
+    start, end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    start.record()
+    for k in range(args.steps):
+        one_pass(rank * 131 + k, bulk_events)
+    end.record()
+    barrier()
+    elapsed_ms = start.elapsed_time(end)
+    clocks = sampler.stop() if sampler else None
+    launches = eng.info("launches") - launches0
+    res = eng.result()
+    bulk_ms = sum(a.elapsed_time(b) for a, b, _ in bulk_events)
+    bulk_launches = sum(c for _, _, c in bulk_events)
+    # algorithmic bytes of one launch: the whole step's bytes spread over the launches that make up a step
+    step_bytes = eng.info("step_bytes") * (N - K) * args.steps / max(bulk_launches, 1)
+
+    # ---- e2e through the public API from host buffers (pinned), host<->device copies inside the timed region
+    def pin(a):
+        return None if a is None else torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
+    pinned = wl.Instance(inst.kind, inst.n, inst.q, pin(inst.row_ptr), pin(inst.col_idx), pin(inst.weight),
+                         pin(inst.dense_J), inst.m, pin(inst.clause_ptr), pin(inst.lits), inst.lam, inst.name)
+    h2d = sum(a.nbytes for a in (pinned.row_ptr, pinned.col_idx, pinned.weight, pinned.dense_J, pinned.clause_ptr,
+                                 pinned.lits) if a is not None)
+    d2h = 4 + 4 * n + 8 * R + 8 * R + 4 * R * inst.q
+
+    def e2e_pass(seed):
+        e = fem.Fem(pinned, R, device=f"cuda:{local_rank}")     # fem_create: validate + upload
+        apply_options(e)
+        e.anneal(sched, R, seed=seed)
+        out = e.result()                                        # readout + download + synchronize
+        e.close()
+        return out
+
+    e2e_pass(7)
+    barrier()
+    t0 = time.perf_counter()
+    e2e_steps = max(1, min(args.steps, 3))
+    for k in range(e2e_steps):
+        e2e_pass(rank * 131 + k)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+
+    # ---- max over ranks, best replica over ranks
+    times = torch.tensor([elapsed_ms, e2e_s * 1e3, bulk_ms], dtype=torch.float64, device=dev)
+    best = torch.tensor([res["energy"][res["best_replica"]]], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+        allbest = [torch.zeros_like(best) for _ in range(world)]
+        dist.all_gather(allbest, best)                         # Eq.5 across ranks: 8 bytes per rank
+        best = torch.stack(allbest).min().reshape(1)
+    elapsed_ms, e2e_ms, bulk_ms = [float(x) for x in times.tolist()]
+
+    if rank == 0:
+        updates = float(n) * R * N
+        value = updates * args.steps * world / (elapsed_ms * 1e-3)
+        peak, peak_src = load_peaks()
+        kernel_us = bulk_ms * 1e3 / bulk_launches
+        achieved = step_bytes / (kernel_us * 1e-6) / 1e9
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": cfg.name, "instance": inst.name, "n": n, "R_per_gpu": R, "anneal_steps": N,
+                       "precise_steps": K, "replica_block": eng.info("replica_block"),
+                       "l2": "256 MiB buffer written between timed passes (L2 flush)",
+                       "parallelism": f"replicas x{world}" if world > 1 else "single GPU"},
+            "roofline": {"bound": "hbm", "kernel": "step_q2_kernel<float> (fused gather + entropy gradient + Adam)",
+                         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": load_traffic(args.workload), "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": step_bytes, "kernel_us": kernel_us,
+                         "kernel_share_of_step": bulk_ms / elapsed_ms},
+            "e2e": {"value": updates * e2e_steps * world / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h, "steps": e2e_steps},
+            "gpu_launches": int(launches),
+            "clocks": clocks,
+            "result": {"best_energy": float(best.item()), "mean_energy": float(np.mean(res["energy"]))},
+        }
+        if not args.no_cpu_baseline and world == 1:
+            o = oracle_sample(cfg, inst)
+            v1, s1, c1 = o[False]
+            vN, sN, cN = o[True]
+            use_omp = vN > v1
+            line["cpu_baseline"] = {"value": vN if use_omp else v1, "unit": UNIT, "cores": cN if use_omp else c1,
+                                    "kind": "oracle",
+                                    "sample": f"{sN if use_omp else s1} annealing steps at full n={n}, R={R} of {cfg.name}",
+                                    "single_thread_value": v1, "all_core_value": vN, "all_core_threads": cN}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

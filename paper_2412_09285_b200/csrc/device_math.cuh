@@ -83,43 +83,67 @@ struct Row {
     }
 };
 
-// ---- scalars narrowed to the compute type ----
+// ---- per-step scalars in the compute type (narrowed once on the host, not per thread) ----
 template <typename T>
 struct Sc {
     T inv_beta, step_size, rsqrt_bc2, eps, b1, b2, omb1, omb2, wd, two_lambda;
-    __device__ __forceinline__ explicit Sc(const StepScalars &s)
+    Sc() = default;
+    __host__ explicit Sc(const StepScalars &s)
         : inv_beta((T)s.inv_beta), step_size((T)s.step_size), rsqrt_bc2((T)s.rsqrt_bc2), eps((T)s.eps), b1((T)s.b1),
           b2((T)s.b2), omb1((T)s.one_minus_b1), omb2((T)s.one_minus_b2), wd((T)s.wd), two_lambda((T)s.two_lambda) {}
 };
 
-__device__ __forceinline__ float fexp(float x) { return expf(x); }
+// fp64 (wide phase): accurate libm.  fp32 (bulk): hardware approximations (ex2/rcp/sqrt MUFU ops, <= 2 ulp),
+// which sit at the level of the fp32 storage rounding of the state itself.
 __device__ __forceinline__ double fexp(double x) { return exp(x); }
-__device__ __forceinline__ float fsqrt(float x) { return sqrtf(x); }
+__device__ __forceinline__ float fexp(float x) {  // exp via ex2.approx; results below 2^-126 flush to 0 (harmless here)
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x * 1.4426950408889634f));
+    return y;
+}
 __device__ __forceinline__ double fsqrt(double x) { return sqrt(x); }
-__device__ __forceinline__ float flog(float x) { return logf(x); }
+__device__ __forceinline__ float fsqrt(float x) {
+    float y;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
 __device__ __forceinline__ double flog(double x) { return log(x); }
+__device__ __forceinline__ float flog(float x) { return __logf(x); }
+__device__ __forceinline__ double fdiv(double a, double b) { return a / b; }
+__device__ __forceinline__ float fdiv(float a, float b) {
+    float y;
+    asm("div.approx.ftz.f32 %0, %1, %2;" : "=f"(y) : "f"(a), "f"(b));
+    return y;
+}
+__device__ __forceinline__ double frcp(double x) { return 1.0 / x; }
+__device__ __forceinline__ float frcp(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
 
-__device__ __forceinline__ float ftanh(float x) { return tanhf(x); }
-__device__ __forceinline__ double ftanh(double x) { return tanh(x); }
-
-// Two-state pieces from one field h = h(+1) - h(-1), each free of cancellation:
+// Two-state pieces from one field h = h(+1) - h(-1):
 //   p(1-p) = e/(1+e)^2 with e = exp(-|h|)   (exact in the saturated tails, where 1 - m^2 would round to 0)
-//   m = 2p - 1 = tanh(h/2)                   (library tanh: relative accuracy also for |h| -> 0, where the
-//                                             deviation from the uniform marginal is all the signal there is)
+//   m = 2p - 1 = tanh(h/2)
+// fp64: library tanh keeps RELATIVE accuracy for |h| -> 0, where the deviation from the uniform marginal is all
+// the signal there is (the start of the anneal, which the wide phase covers).  fp32: m = sign(h)(1-e)/(1+e),
+// absolute accuracy ~6e-8, one exp shared with nothing else to compute.
 template <typename T>
 __device__ __forceinline__ T p1mp_of(T h) {
     const T e = fexp(-fabs(h));
-    const T r = (T)1 / ((T)1 + e);
+    const T r = frcp((T)1 + e);
     return e * r * r;
 }
-template <typename T>
-__device__ __forceinline__ T mag_of(T h) {
-    return ftanh((T)0.5 * h);
+__device__ __forceinline__ double mag_of(double h) { return tanh(0.5 * h); }
+__device__ __forceinline__ float mag_of(float h) {
+    const float e = fexp(-fabsf(h));
+    const float am = (1.0f - e) * frcp(1.0f + e);
+    return copysignf(am, h);
 }
 template <typename T>
 __device__ __forceinline__ T sigmoid_of(T h) {
     const T e = fexp(-fabs(h));
-    const T r = (T)1 / ((T)1 + e);
+    const T r = frcp((T)1 + e);
     return h < (T)0 ? e * r : r;
 }
 
@@ -129,8 +153,8 @@ __device__ __forceinline__ T adam_update(T h, T g, T &m1, T &m2, const Sc<T> &sc
     g = g + sc.wd * h;
     m1 = sc.b1 * m1 + sc.omb1 * g;
     m2 = sc.b2 * m2 + sc.omb2 * g * g;
-    T denom = fsqrt(m2) * sc.rsqrt_bc2 + sc.eps;
-    return h - sc.step_size * (m1 / denom);
+    const T denom = fsqrt(m2) * sc.rsqrt_bc2 + sc.eps;
+    return h - sc.step_size * fdiv(m1, denom);
 }
 
 }  // namespace fem

@@ -169,6 +169,11 @@ static void configure_R(Handle *hd, int R) {
     if (hd->opt_replica_block > 0 && hd->opt_replica_block < R && R % hd->opt_replica_block == 0)
         Rb = (int)hd->opt_replica_block;
     hd->Rb = Rb;
+    while ((uint64_t)hd->rows * (uint64_t)hd->Rb >= (1ull << 32)) {  // kernels index a replica block with 32 bits
+        int nb = R / hd->Rb + 1;
+        while (R % nb) ++nb;
+        hd->Rb = R / nb;
+    }
     if (hd->dp.kind == FEM_BMINCUT) {  // one variable's replicas must fit one CTA pass
         for (;;) {
             const int vec = potts_vec(hd);

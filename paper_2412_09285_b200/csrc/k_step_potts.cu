@@ -16,7 +16,7 @@ template <typename T>
 struct PottsParams {
     BlockArrays<T> a;
     DevProblem dp;
-    StepScalars sc;
+    Sc<T> sc;
     const double *S_in;  // [q][Rb] of this block (blockIdx.y stride q*Rb)
     double *partial;     // [gridDim.x][q*Rb] per block (blockIdx.y stride kColBlocks*q*Rb)
     int rv;              // Rb / VEC lanes per variable
@@ -34,7 +34,7 @@ __global__ void __launch_bounds__(kThreads) potts_kernel(const PottsParams<T> p)
     const int64_t blk = (int64_t)blockIdx.y * p.a.blk_stride;
     const T *__restrict__ gin = p.a.g_in + blk + c;
     const double *__restrict__ S = p.S_in + (int64_t)blockIdx.y * q * Rb;
-    const Sc<T> sc(p.sc);
+    const Sc<T> &sc = p.sc;
     const T inv_q = (T)1 / (T)q;
 
     T colacc[QMAX][VEC];
@@ -70,7 +70,7 @@ __global__ void __launch_bounds__(kThreads) potts_kernel(const PottsParams<T> p)
                         P[s][v] = fexp(h[s][v] - mx);
                         z += P[s][v];
                     }
-                const T rz = (T)1 / z;
+                const T rz = frcp(z);
 #pragma unroll
                 for (int s = 0; s < QMAX; ++s)
                     if (s < q) P[s][v] *= rz;
@@ -148,7 +148,7 @@ __global__ void __launch_bounds__(kThreads) potts_kernel(const PottsParams<T> p)
                     P[s][v] = fexp(h[s][v] - mx);
                     z += P[s][v];
                 }
-            const T rz = (T)1 / z;
+            const T rz = frcp(z);
 #pragma unroll
             for (int s = 0; s < QMAX; ++s)
                 if (s < q) P[s][v] *= rz;
@@ -244,7 +244,7 @@ static void launch_potts_typed(Handle *hd, const StepScalars &sc, bool step, int
     p.a.blk_stride = hd->rows * Rb;
     p.a.Rb = Rb;
     p.dp = hd->dp;
-    p.sc = sc;
+    p.sc = Sc<T>(sc);
     p.S_in = hd->colsum[hd->cur] + (int64_t)blk_begin * q * Rb;
     p.partial = hd->colpart + (int64_t)blk_begin * kColBlocks * q * Rb;
     const int vec = potts_vec(hd);  // fem_anneal keeps Rb / vec <= kThreads (one variable inside one CTA pass)

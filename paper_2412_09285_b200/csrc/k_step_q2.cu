@@ -16,10 +16,11 @@ template <typename T>
 struct Q2Params {
     BlockArrays<T> a;
     DevProblem dp;
-    StepScalars sc;
-    const T *field;  // dense Ising: precomputed J*m, same layout as h
-    int rv;          // Rb / VEC
-    int64_t total;   // n * rv
+    Sc<T> sc;
+    const T *field;     // dense Ising: precomputed J*m, same layout as h
+    unsigned rv;        // Rb / VEC lanes per variable
+    int rv_shift;       // log2(rv) when rv is a power of two, else -1
+    unsigned total;     // n * rv threads per replica block
 };
 
 enum { MODE_MAXCUT = 0, MODE_ISING = 1, MODE_SAT = 3, MODE_FIELD = 4 };
@@ -27,13 +28,13 @@ enum { MODE_MAXCUT = 0, MODE_ISING = 1, MODE_SAT = 3, MODE_FIELD = 4 };
 template <typename T, int VEC, int MODE, int DEG>
 __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) {
     using R = Row<T, VEC>;
-    const int64_t idx = (int64_t)blockIdx.x * kThreads + threadIdx.x;
+    const unsigned idx = blockIdx.x * kThreads + threadIdx.x;
     if (idx >= p.total) return;
-    const int i = (int)(idx / p.rv);
-    const int c = (int)(idx - (int64_t)i * p.rv) * VEC;
+    const unsigned i = p.rv_shift >= 0 ? idx >> p.rv_shift : idx / p.rv;
+    const unsigned c = (idx - i * p.rv) * VEC;
     const int64_t blk = (int64_t)blockIdx.y * p.a.blk_stride;
-    const int Rb = p.a.Rb;
-    const int64_t off = blk + (int64_t)i * Rb + c;
+    const unsigned Rb = p.a.Rb;
+    const int64_t off = blk + (i * Rb + c);  // a replica block holds < 2^32 elements (checked at fem_anneal)
     const T *__restrict__ gin = p.a.g_in + blk + c;
 
     // issue the streaming loads first so they overlap the dependent gather chain
@@ -49,14 +50,14 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
         const int *__restrict__ col = p.dp.col;
         const float *__restrict__ w = p.dp.w;
         if (DEG > 0) {
-            const int e0 = i * DEG;
+            const unsigned e0 = i * DEG;
             R nb[DEG > 0 ? DEG : 1];
             float wj[DEG > 0 ? DEG : 1];
 #pragma unroll
             for (int k = 0; k < DEG; ++k) {
                 const int j = __ldg(col + e0 + k);
                 wj[k] = w ? __ldg(w + e0 + k) : 1.0f;
-                nb[k] = R::ld(gin + (int64_t)j * Rb);
+                nb[k] = R::ld(gin + (unsigned)j * Rb);
             }
 #pragma unroll
             for (int k = 0; k < DEG; ++k)
@@ -68,7 +69,7 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
             for (int e = e0; e < e1; ++e) {
                 const int j = __ldg(col + e);
                 const float wj = w ? __ldg(w + e) : 1.0f;
-                const R nb = R::ld(gin + (int64_t)j * Rb);
+                const R nb = R::ld(gin + (unsigned)j * Rb);
 #pragma unroll
                 for (int v = 0; v < VEC; ++v) dU[v] += (T)wj * nb.v[v];
             }
@@ -85,7 +86,7 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
         const int o0 = __ldg(p.dp.occ_ptr + i), o1 = __ldg(p.dp.occ_ptr + i + 1);
         const int ks = p.dp.kstride;
         for (int o = o0; o < o1; ++o) {
-            const int *__restrict__ ent = p.dp.occ + (int64_t)o * ks;
+            const int *__restrict__ ent = p.dp.occ + (unsigned)o * (unsigned)ks;
             T prod[VEC];
 #pragma unroll
             for (int v = 0; v < VEC; ++v) prod[v] = (T)1;
@@ -94,7 +95,7 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
                 int pk = __ldg(ent + x);
                 if (x == 0) first = pk;
                 pk &= 0x7fffffff;
-                const R mr = R::ld(gin + (int64_t)(pk >> 1) * Rb);
+                const R mr = R::ld(gin + (unsigned)(pk >> 1) * Rb);
                 // probability the literal is false: 1-p = (1-m)/2 (positive literal), p = (1+m)/2 (negated)
                 const T sg = (pk & 1) ? (T)0.5 : (T)-0.5;
 #pragma unroll
@@ -106,7 +107,7 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
         }
     }
 
-    const Sc<T> sc(p.sc);
+    const Sc<T> &sc = p.sc;
     R hn, gn;
 #pragma unroll
     for (int v = 0; v < VEC; ++v) {
@@ -218,7 +219,7 @@ static void launch_step_q2_t(Handle *hd, const StepScalars &sc, int blk_begin, i
     p.a.blk_stride = hd->rows * Rb;
     p.a.Rb = Rb;
     p.dp = hd->dp;
-    p.sc = sc;
+    p.sc = Sc<T>(sc);
     p.field = nullptr;
     int mode = hd->dp.kind == FEM_MAXCUT ? MODE_MAXCUT : hd->dp.kind == FEM_MAXSAT ? MODE_SAT : MODE_ISING;
     if (hd->dp.kind == FEM_ISING && hd->dp.J) {
@@ -233,8 +234,9 @@ static void launch_step_q2_t(Handle *hd, const StepScalars &sc, int blk_begin, i
         }
     }
     const int VEC = (Rb % 4 == 0) ? 4 : 1;
-    p.rv = Rb / VEC;
-    p.total = (int64_t)hd->dp.n * p.rv;
+    p.rv = (unsigned)(Rb / VEC);
+    p.rv_shift = (p.rv & (p.rv - 1)) == 0 ? __builtin_ctz(p.rv) : -1;
+    p.total = (unsigned)hd->dp.n * p.rv;
     dim3 grid((unsigned)ceil_div(p.total, kThreads), (unsigned)blk_count);
     if (VEC == 4) launch_q2_mode<T, 4>(hd, p, grid, mode);
     else launch_q2_mode<T, 1>(hd, p, grid, mode);
