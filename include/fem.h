@@ -81,7 +81,8 @@ typedef struct {
     const double *lambda; /* HOST [steps] per-step balance weight, or NULL */
     double lr, beta1, beta2, eps, weight_decay; /* Adam, PyTorch semantics */
     double init_scale;     /* h(0) = init_scale * N(0,1); used when fields were not injected */
-    int32_t precise_steps; /* the first K steps do their arithmetic in fp64 registers (storage stays fp32) */
+    int32_t precise_steps; /* wide phase: the first K steps keep state AND arithmetic in fp64, then the state is
+                            * rounded to fp32 once and the rest of the anneal is fp32 */
 } fem_schedule;
 
 /* Bytes of device workspace fem_create needs for this problem with up to R_cap replicas
@@ -134,9 +135,10 @@ fem_status fem_get_configs(fem_handle *h, int32_t *cfg /* [R][n] */);
 fem_status fem_energy_of(fem_handle *h, const int32_t *cfg /* [count][n] */, int32_t count, int64_t *energy_int,
                          double *energy, int32_t *part_sizes /* [count][q] or NULL */);
 
-/* Tuning knobs (all optional): "replica_block" (replicas per L2-resident block, 0 = all),
- * "steps_per_block" (steps run on one replica block before moving to the next, 0 = whole anneal
- * per block when blocking is on, 1 = step-major).  Unknown key: FEM_EINVAL. */
+/* Tuning knobs (all optional): "replica_block" (replicas per L2-resident block; 0 = chosen from the
+ * device's L2 size, the default; >= R = no blocking), "steps_per_block" (steps run on one replica
+ * block before moving to the next; 0 = the whole anneal per block, the default; 1 = step-major).
+ * Results do not depend on either (replicas are independent).  Unknown key: FEM_EINVAL. */
 fem_status fem_set_option(fem_handle *h, const char *key, int64_t value);
 /* Introspection for benchmarks: "launches" (kernels enqueued so far), "t_done", "R", "nnz",
  * "step_bytes" (algorithmic HBM bytes of one fused step). */

@@ -83,6 +83,28 @@ struct Row {
     }
 };
 
+// ---- programmatic dependent launch (PDL): consecutive step kernels overlap launch latency and tail ----
+// pdl_trigger lets the NEXT kernel in the stream start being scheduled once every CTA of this grid has
+// started; pdl_wait blocks until the PREVIOUS grid has completed and its writes are visible.  Only loads
+// of the static problem structure may precede pdl_wait.
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStream_t stream, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, args...);
+}
+
 // ---- per-step scalars in the compute type (narrowed once on the host, not per thread) ----
 template <typename T>
 struct Sc {

@@ -163,11 +163,25 @@ static bool validate_graph(const fem_problem *pb, int64_t nnz, bool *integral, i
     return true;
 }
 
+// Replica block size.  Replicas are independent, so a block whose five fp32 state arrays (h, m1, m2 and the
+// two gather buffers: 20 B per field) fit in L2 can run its whole anneal out of L2 before the next block
+// starts.  opt_replica_block: 0 = choose automatically, >= R = off, else that size.
 static void configure_R(Handle *hd, int R) {
     hd->R = R;
     int Rb = R;
-    if (hd->opt_replica_block > 0 && hd->opt_replica_block < R && R % hd->opt_replica_block == 0)
-        Rb = (int)hd->opt_replica_block;
+    if (hd->opt_replica_block > 0) {
+        if (hd->opt_replica_block < R && R % hd->opt_replica_block == 0) Rb = (int)hd->opt_replica_block;
+    } else {
+        const double per_replica = 20.0 * (double)hd->dp.n * hd->dp.F;
+        const double budget = 0.45 * (double)hd->l2_bytes;
+        if (per_replica * R > budget) {
+            const int vec = (R % 4 == 0) ? 4 : 1;
+            int best = 0;
+            for (int d = vec; d < R; d += vec)
+                if (R % d == 0 && per_replica * d <= budget && (double)hd->dp.n * hd->dp.F * d >= 1.0e6) best = d;
+            if (best > 0) Rb = best;
+        }
+    }
     hd->Rb = Rb;
     while ((uint64_t)hd->rows * (uint64_t)hd->Rb >= (1ull << 32)) {  // kernels index a replica block with 32 bits
         int nb = R / hd->Rb + 1;
@@ -343,6 +357,11 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
         hd->structure_bytes = (dp.uniform_deg > 0 ? 0 : 4 * ((int64_t)pb->n + 1)) + (s.weighted ? 8 : 4) * s.nnz;
     }
     hd->lambda_last = pb->lambda;
+    {
+        int dev = 0, l2 = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev) == cudaSuccess)
+            hd->l2_bytes = l2;
+    }
     hd->h = reinterpret_cast<float *>(at(L.h));
     hd->m1 = reinterpret_cast<float *>(at(L.m1));
     hd->m2 = reinterpret_cast<float *>(at(L.m2));

@@ -90,6 +90,7 @@ struct Handle {
     bool injected = false, readout_valid = false, gather_valid = false;
     int64_t opt_replica_block = 0, opt_steps_per_block = 0;
     int64_t launches = 0;
+    int64_t l2_bytes = 0;  // device L2 size (0 when unknown: no automatic replica blocking)
     int64_t structure_bytes = 0;  // problem-structure bytes one step reads (indices, weights, clause entries)
     double lambda_last = 0.0;     // balance weight of the last executed step (readout uses it)
     std::string err;

@@ -28,6 +28,7 @@ enum { MODE_MAXCUT = 0, MODE_ISING = 1, MODE_SAT = 3, MODE_FIELD = 4 };
 template <typename T, int VEC, int MODE, int DEG>
 __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) {
     using R = Row<T, VEC>;
+    pdl_trigger();
     const unsigned idx = blockIdx.x * kThreads + threadIdx.x;
     if (idx >= p.total) return;
     const unsigned i = p.rv_shift >= 0 ? idx >> p.rv_shift : idx / p.rv;
@@ -37,7 +38,17 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
     const int64_t off = blk + (i * Rb + c);  // a replica block holds < 2^32 elements (checked at fem_anneal)
     const T *__restrict__ gin = p.a.g_in + blk + c;
 
-    // issue the streaming loads first so they overlap the dependent gather chain
+    // static structure first (legal before pdl_wait), then everything the previous step wrote
+    int jj[DEG > 0 ? DEG : 1];
+    float wj[DEG > 0 ? DEG : 1];
+    if ((MODE == MODE_MAXCUT || MODE == MODE_ISING) && DEG > 0) {
+#pragma unroll
+        for (int k = 0; k < DEG; ++k) {
+            jj[k] = __ldg(p.dp.col + i * DEG + k);
+            wj[k] = p.dp.w ? __ldg(p.dp.w + i * DEG + k) : 1.0f;
+        }
+    }
+    pdl_wait();
     const R h4 = R::ld_stream(p.a.h + off);
     R m1 = R::ld_stream(p.a.m1 + off);
     R m2 = R::ld_stream(p.a.m2 + off);
@@ -50,15 +61,9 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
         const int *__restrict__ col = p.dp.col;
         const float *__restrict__ w = p.dp.w;
         if (DEG > 0) {
-            const unsigned e0 = i * DEG;
             R nb[DEG > 0 ? DEG : 1];
-            float wj[DEG > 0 ? DEG : 1];
 #pragma unroll
-            for (int k = 0; k < DEG; ++k) {
-                const int j = __ldg(col + e0 + k);
-                wj[k] = w ? __ldg(w + e0 + k) : 1.0f;
-                nb[k] = R::ld(gin + (unsigned)j * Rb);
-            }
+            for (int k = 0; k < DEG; ++k) nb[k] = R::ld(gin + (unsigned)jj[k] * Rb);
 #pragma unroll
             for (int k = 0; k < DEG; ++k)
 #pragma unroll
@@ -188,11 +193,11 @@ template <typename T, int VEC, int MODE>
 static void launch_q2_deg(Handle *hd, const Q2Params<T> &p, dim3 grid) {
     const int d = (MODE == MODE_MAXCUT || MODE == MODE_ISING) ? hd->dp.uniform_deg : 0;
     if (d == 3)
-        step_q2_kernel<T, VEC, MODE, 3><<<grid, kThreads, 0, hd->stream>>>(p);
+        launch_pdl(step_q2_kernel<T, VEC, MODE, 3>, grid, dim3(kThreads), hd->stream, p);
     else if (d == 4)
-        step_q2_kernel<T, VEC, MODE, 4><<<grid, kThreads, 0, hd->stream>>>(p);
+        launch_pdl(step_q2_kernel<T, VEC, MODE, 4>, grid, dim3(kThreads), hd->stream, p);
     else
-        step_q2_kernel<T, VEC, MODE, 0><<<grid, kThreads, 0, hd->stream>>>(p);
+        launch_pdl(step_q2_kernel<T, VEC, MODE, 0>, grid, dim3(kThreads), hd->stream, p);
 }
 
 template <typename T, int VEC>
