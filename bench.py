@@ -190,7 +190,7 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_2412_09285_b200 import fem
+    from paper_2412_09285_b200 import fem, multigpu
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the FEM path has no CPU fallback")
@@ -235,7 +235,7 @@ def main():
         eng.readout()                                          # rounding + energies + argmin
 
     for w in range(args.warmup):
-        one_pass(1000 + rank * 131 + w)
+        one_pass(multigpu.replica_seed(1000 + w, rank))
     barrier()
     launches0 = eng.info("launches")
     sampler = ClockSampler(local_rank) if rank == 0 else None
@@ -243,7 +243,7 @@ def main():
     start, end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     start.record()
     for k in range(args.steps):
-        one_pass(rank * 131 + k, bulk_events)
+        one_pass(multigpu.replica_seed(k, rank), bulk_events)
     end.record()
     barrier()
     elapsed_ms = start.elapsed_time(end)
@@ -277,18 +277,17 @@ def main():
     t0 = time.perf_counter()
     e2e_steps = max(1, min(args.steps, 3))
     for k in range(e2e_steps):
-        e2e_pass(rank * 131 + k)
+        e2e_pass(multigpu.replica_seed(k, rank))
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
 
     # ---- max over ranks, best replica over ranks
     times = torch.tensor([elapsed_ms, e2e_s * 1e3, bulk_ms], dtype=torch.float64, device=dev)
-    best = torch.tensor([res["energy"][res["best_replica"]]], dtype=torch.float64, device=dev)
     if world > 1:
         dist.all_reduce(times, op=dist.ReduceOp.MAX)
-        allbest = [torch.zeros_like(best) for _ in range(world)]
-        dist.all_gather(allbest, best)                         # Eq.5 across ranks: 8 bytes per rank
-        best = torch.stack(allbest).min().reshape(1)
+    # Eq.5 across ranks: 8 bytes per rank, then the owner's configuration
+    best_energy, best_owner, _ = multigpu.best_over_ranks(float(res["energy"][res["best_replica"]]),
+                                                          res["best_config"], dev)
     elapsed_ms, e2e_ms, bulk_ms = [float(x) for x in times.tolist()]
 
     if rank == 0:
@@ -314,7 +313,7 @@ def main():
                     "d2h_bytes_per_step": d2h, "steps": e2e_steps},
             "gpu_launches": int(launches),
             "clocks": clocks,
-            "result": {"best_energy": float(best.item()), "mean_energy": float(np.mean(res["energy"]))},
+            "result": {"best_energy": best_energy, "best_rank": best_owner, "mean_energy": float(np.mean(res["energy"]))},
         }
         if not args.no_cpu_baseline and world == 1:
             o = oracle_sample(cfg, inst)

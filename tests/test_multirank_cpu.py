@@ -1,0 +1,57 @@
+"""world_size-2 gloo test of the N > 1 host logic: replica sharding and the Eq.5 exchange across ranks."""
+import os
+import socket
+
+import numpy as np
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+from paper_2412_09285_b200 import multigpu
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, out):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        # every rank "anneals" its own replicas: stand-in energies, rank 1 holds the better one
+        rng = np.random.default_rng(multigpu.replica_seed(0, rank))
+        energies = np.array([-10.0, -12.0]) if rank == 0 else np.array([-15.0, -11.0])
+        cfgs = rng.integers(0, 2, size=(2, 9)).astype(np.int32)
+        a = int(np.argmin(energies))
+        e, owner, cfg = multigpu.best_over_ranks(float(energies[a]), cfgs[a], torch.device("cpu"))
+        assert e == -15.0 and owner == 1
+        # a tie goes to the lowest rank
+        e2, owner2, _ = multigpu.best_over_ranks(-7.0, cfgs[0], torch.device("cpu"))
+        assert e2 == -7.0 and owner2 == 0
+        out.put((rank, cfg.tolist(), cfgs[a].tolist()))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_best_replica_over_two_ranks():
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, out)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = [out.get(timeout=120) for _ in procs]
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    got.sort()
+    assert got[0][1] == got[1][1] == got[1][2]        # both ranks hold rank 1's configuration
+
+
+def test_replica_seeds_are_distinct():
+    seeds = {multigpu.replica_seed(0, r) for r in range(64)} | {multigpu.replica_seed(1, r) for r in range(64)}
+    assert len(seeds) == 128
