@@ -1,0 +1,104 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (seeded device-side
+initial fields, default precise_steps, automatic replica blocking).  The oracle cannot run every replica at
+these sizes, so it runs a replica SUBSET: the field generator is keyed on (seed, replica, variable, state),
+so replica a's trajectory does not depend on R (R4)."""
+import numpy as np
+import pytest
+
+from oracle import fem_oracle as fo
+from paper_2412_09285_b200 import workloads as wl
+from test_oracle_gradient import as_problem
+
+pytestmark = pytest.mark.gpu
+
+# config -> replicas the oracle follows for 50 steps
+SUBSET = {"cfg0": 32, "cfg1": 4, "cfg2": 2, "cfg3": 4, "cfg4a": 2, "cfg4b": 2}
+
+
+@pytest.fixture(scope="module")
+def fem():
+    from paper_2412_09285_b200 import fem as femlib
+    return femlib
+
+
+_cache = {}
+
+
+def instance(name):
+    if name not in _cache:
+        _cache.clear()                       # one full-size instance alive at a time
+        _cache[name] = wl.CONFIGS[name].make()
+    return _cache[name]
+
+
+@pytest.mark.parametrize("name", ["cfg0", "cfg1", "cfg2", "cfg3", "cfg4a", "cfg4b"])
+def test_marginals_after_50_steps_full_size(fem, name):
+    c = wl.CONFIGS[name]
+    inst = instance(name)
+    k = SUBSET[name]
+    F = inst.fields_per_var
+    pb = as_problem(inst)
+    beta = fo.schedule_inverse_proportional(c.T_max, c.T_min, c.steps)
+    h0 = fo.init_fields(c.field_seed, k, inst.n, F, c.init_scale)
+    st = fo.State(pb, h0)
+    fo.anneal(st, beta, fo.Adam(c.lr, c.beta1, c.beta2, c.eps), inst.lam, t_end=50, openmp=True)
+    P_ref = fo.marginals(pb, st.h).reshape(h0.shape)
+
+    eng = fem.Fem(inst, c.R)
+    sch = fem.schedule_for(c)                # the schedule and precise_steps bench.py uses
+    eng.anneal(sch, c.R, seed=c.field_seed, stop_after=0)
+    hg = eng.get_fields()[:k]
+    ulp = np.abs(hg.view(np.int32).astype(np.int64) - h0.astype(np.float32).view(np.int32).astype(np.int64))
+    assert ulp.max() <= 1                    # device generator == oracle generator
+    eng.anneal(sch, c.R, seed=c.field_seed, stop_after=50)
+    P = eng.get_marginals()[:k].astype(np.float64)
+    err = np.max(np.abs(P - P_ref))
+    assert err < 1e-4, (name, err)
+    eng.close()
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3", "cfg4a", "cfg4b"])
+def test_full_anneal_readout_properties(fem, name):
+    """Properties that hold at any size: the reported energies are the oracle's energies of the reported
+    configurations (bit-exact for the integer kinds), the rounding rule, the argmin and its tie-break."""
+    c = wl.CONFIGS[name]
+    inst = instance(name)
+    pb = as_problem(inst)
+    eng = fem.Fem(inst, c.R)
+    eng.anneal(fem.schedule_for(c), c.R, seed=c.field_seed)
+    res = eng.result()
+    rng = np.random.default_rng(0)
+    sample = np.unique(np.concatenate([[0, c.R - 1, res["best_replica"]], rng.integers(0, c.R, 3)]))
+    cfg = eng.get_configs()
+    h = eng.get_fields()
+    assert np.array_equal(cfg[sample], fo.round_configs(pb, h[sample].astype(np.float64)))
+    e_int, e_real, part = fo.energies(pb, cfg[sample], inst.lam)
+    if inst.kind == wl.ISING:
+        assert np.max(np.abs(res["energy"][sample] - e_real)) <= 1e-9 * np.max(np.abs(e_real))
+    else:
+        assert np.array_equal(res["energy_int"][sample], e_int)
+        assert np.array_equal(res["energy"][sample], e_real)
+    if inst.kind == wl.BMINCUT:
+        assert np.array_equal(res["part_sizes"][sample], part)
+        assert np.all(res["part_sizes"].sum(axis=1) == inst.n)
+    assert res["best_replica"] == int(np.argmin(res["energy"]))
+    assert np.array_equal(res["best_config"], cfg[res["best_replica"]])
+    eng.close()
+
+
+def test_full_anneal_energy_distribution_cfg1(fem):
+    """cfg 1 in full on the GPU (R = 256, 2000 steps) against the oracle's full anneal of replicas 0..7: the mean
+    final energy over those replicas, and over all 256, within 0.5% of the oracle's mean."""
+    c = wl.CONFIGS["cfg1"]
+    inst = instance("cfg1")
+    pb = as_problem(inst)
+    beta = fo.schedule_inverse_proportional(c.T_max, c.T_min, c.steps)
+    st = fo.State(pb, fo.init_fields(c.field_seed, 8, inst.n, 1, c.init_scale))
+    fo.anneal(st, beta, fo.Adam(c.lr, c.beta1, c.beta2, c.eps), openmp=True)
+    ref = fo.energies(pb, fo.round_configs(pb, st.h))[0].astype(np.float64)
+    eng = fem.Fem(inst, c.R)
+    eng.anneal(fem.schedule_for(c), c.R, seed=c.field_seed)
+    e = eng.result()["energy_int"].astype(np.float64)
+    assert abs(e[:8].mean() - ref.mean()) <= 0.005 * abs(ref.mean())
+    assert abs(e.mean() - ref.mean()) <= 0.005 * abs(ref.mean())
+    eng.close()
