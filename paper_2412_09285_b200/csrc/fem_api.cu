@@ -17,11 +17,13 @@ void launch_potts(Handle *hd, const StepScalars &sc, bool wide, bool step, int b
 void launch_sigmoid(Handle *hd, float *out);
 int potts_vec(const Handle *hd);
 void launch_potts_softmax(Handle *hd, float *out);
+void launch_tc_split(Handle *hd);
+int tc_tile_n(int n, int Rb);
 
 static std::string g_create_error;
 
 struct Layout {
-    size_t row_ptr, col, w, J, field, occ_ptr, occ, clause_ptr, lits;
+    size_t row_ptr, col, w, J, Jlo, glo0, glo1, field, occ_ptr, occ, clause_ptr, lits;
     size_t h, m1, m2, g0, g1, stage, hW, m1W, m2W, gW0, gW1, colsum0, colsum1, colpart, cfg, e_part_i, e_part_d, part_part, e_int, e_real, part,
         best, total;
 };
@@ -85,6 +87,9 @@ static Layout make_layout(const fem_problem *pb, const ProblemShape &s, int R_ca
     L.col = take((size_t)s.nnz * 4);
     L.w = take(s.weighted ? (size_t)s.nnz * 4 : 0);
     L.J = take(s.dense ? (size_t)pb->n * pb->n * 4 : 0);
+    L.Jlo = take(s.dense ? (size_t)pb->n * pb->n * 4 : 0);
+    L.glo0 = take(s.dense ? state : 0);
+    L.glo1 = take(s.dense ? state : 0);
     L.field = take(s.dense ? 2 * state : 0);  // fp64 in the wide phase
     L.occ_ptr = take(pb->kind == FEM_MAXSAT ? ((size_t)pb->n + 1) * 4 : 0);
     L.occ = take((size_t)s.nocc * std::max(1, s.kmax - 1) * 4);
@@ -171,7 +176,7 @@ static void configure_R(Handle *hd, int R) {
     int Rb = R;
     if (hd->opt_replica_block > 0) {
         if (hd->opt_replica_block < R && R % hd->opt_replica_block == 0) Rb = (int)hd->opt_replica_block;
-    } else {
+    } else if (!hd->dp.J) {  // (the dense kind runs as one block: its tensor maps cover all R replicas)
         const double per_replica = 20.0 * (double)hd->dp.n * hd->dp.F;
         const double budget = 0.45 * (double)hd->l2_bytes;
         if (per_replica * R > budget) {
@@ -338,6 +343,10 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
         up(at(L.J), pb->dense_J, (size_t)n * n * 4, "upload J");
         dp.J = reinterpret_cast<float *>(at(L.J));
         hd->field = reinterpret_cast<float *>(at(L.field));
+        hd->Jlo = reinterpret_cast<float *>(at(L.Jlo));
+        hd->glo[0] = reinterpret_cast<float *>(at(L.glo0));
+        hd->glo[1] = reinterpret_cast<float *>(at(L.glo1));
+        if (ok) launch_tc_split(hd);  // J_lo = J - tf32(J) for the 3xTF32 tensor-core path
         hd->integral_weights = false;
         hd->structure_bytes = 4 * (int64_t)n * n;
     } else {
@@ -405,6 +414,7 @@ fem_status fem_reset(fem_handle *h) {
     hd->gather_valid = false;
     hd->readout_valid = false;
     hd->wide_live = false;
+    hd->tc_ready = false;
     return FEM_OK;
 }
 
@@ -418,6 +428,9 @@ fem_status fem_set_option(fem_handle *h, const char *key, int64_t value) {
     } else if (!strcmp(key, "steps_per_block")) {
         if (value < 0) return fail(hd, FEM_EINVAL, "steps_per_block must be >= 0");
         hd->opt_steps_per_block = value;
+    } else if (!strcmp(key, "tensor_cores")) {
+        if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "tensor_cores must be 0 or 1");
+        hd->opt_tensor_cores = value;
     } else {
         return fail(hd, FEM_EINVAL, "unknown option");
     }
@@ -458,6 +471,7 @@ fem_status fem_set_fields(fem_handle *h, int32_t R, const float *fields) {
     hd->gather_valid = false;
     hd->readout_valid = false;
     hd->wide_live = false;
+    hd->tc_ready = false;
     return FEM_OK;
 }
 
@@ -531,6 +545,7 @@ fem_status fem_anneal(fem_handle *h, const fem_schedule *sch, int32_t R, uint64_
             hd->wide_live = false;
         }
         hd->gather_valid = false;
+        hd->tc_ready = false;
     }
     ensure_gather(hd);
     const int nb = hd->R / hd->Rb;
@@ -561,6 +576,7 @@ fem_status fem_anneal(fem_handle *h, const fem_schedule *sch, int32_t R, uint64_
     if (hd->wide_live && t < stop_after) {  // leave the wide phase only when fp32 steps follow
         launch_narrow(hd, false);
         hd->wide_live = false;
+        hd->tc_ready = false;
     }
     if (nb == 1 || hd->opt_steps_per_block == 1) {
         for (; t < stop_after; ++t) {

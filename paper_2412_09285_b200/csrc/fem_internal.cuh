@@ -75,6 +75,11 @@ struct Handle {
     double *hW = nullptr, *m1W = nullptr, *m2W = nullptr, *gW[2] = {nullptr, nullptr};
     bool wide_live = false;                  // the fp64 arrays hold the current state
     float *field = nullptr;                  // dense Ising: J*m scratch [rows*R_cap] (fp64 in the wide phase: 2x)
+    // dense Ising on the tensor cores (k_dense_tc.cu): low parts of J and of the transposed gather buffers
+    float *Jlo = nullptr, *glo[2] = {nullptr, nullptr};
+    alignas(64) unsigned char tc_maps[6 * 128];  // CUtensorMap x6: J, Jlo, GT[0], GTlo[0], GT[1], GTlo[1]
+    int tc_maps_R = -1;
+    bool tc_ready = false;                   // g[cur]/glo[cur] hold GT / GT_lo of the current fields
     double *colsum[2] = {nullptr, nullptr};  // Potts S[q][R]
     double *colpart = nullptr;               // [kColBlocks][q*R]
     int8_t *cfg = nullptr;                   // [rows*R_cap]
@@ -88,7 +93,7 @@ struct Handle {
     int cur = 0;          // g[cur] holds the gathered quantity of the current fields
     int t_done = 0;
     bool injected = false, readout_valid = false, gather_valid = false;
-    int64_t opt_replica_block = 0, opt_steps_per_block = 0;
+    int64_t opt_replica_block = 0, opt_steps_per_block = 0, opt_tensor_cores = 0;
     int64_t launches = 0;
     int64_t l2_bytes = 0;  // device L2 size (0 when unknown: no automatic replica blocking)
     int64_t structure_bytes = 0;  // problem-structure bytes one step reads (indices, weights, clause entries)

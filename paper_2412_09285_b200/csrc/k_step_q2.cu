@@ -210,9 +210,14 @@ static void launch_q2_mode(Handle *hd, const Q2Params<T> &p, dim3 grid, int mode
     }
 }
 
+bool launch_step_dense_tc(Handle *hd, const StepScalars &sc);  // k_dense_tc.cu
+
 template <typename T>
 static void launch_step_q2_t(Handle *hd, const StepScalars &sc, int blk_begin, int blk_count) {
     using S = StateOf<T>;
+    if (std::is_same<T, float>::value && hd->dp.kind == FEM_ISING && hd->dp.J && blk_begin == 0 && blk_count == 1 &&
+        launch_step_dense_tc(hd, sc))
+        return;  // dense couplings: tcgen05 GEMM with the update fused in its epilogue
     const int Rb = hd->Rb;
     const int64_t base = (int64_t)blk_begin * hd->rows * Rb;
     Q2Params<T> p;
