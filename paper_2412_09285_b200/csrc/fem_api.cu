@@ -15,7 +15,7 @@ void launch_step_q2(Handle *hd, const StepScalars &sc, bool wide, int blk_begin,
 void launch_prepare_q2(Handle *hd, bool wide);
 void launch_potts(Handle *hd, const StepScalars &sc, bool wide, bool step, int blk_begin, int blk_count);
 void launch_sigmoid(Handle *hd, float *out);
-int potts_vec(const Handle *hd);
+bool potts_block_ok(int q, int Rb);
 void launch_potts_softmax(Handle *hd, float *out);
 void launch_tc_split(Handle *hd);
 int tc_tile_n(int n, int Rb);
@@ -24,7 +24,7 @@ static std::string g_create_error;
 
 struct Layout {
     size_t row_ptr, col, w, J, Jlo, glo0, glo1, field, occ_ptr, occ, clause_ptr, lits;
-    size_t h, m1, m2, g0, g1, stage, hW, m1W, m2W, gW0, gW1, colsum0, colsum1, colpart, cfg, e_part_i, e_part_d, part_part, e_int, e_real, part,
+    size_t h, m1, m2, g0, g1, stage, hW, m1W, m2W, gW0, gW1, colsum0, colsum1, colsum2, cfg, e_part_i, e_part_d, part_part, e_int, e_real, part,
         best, total;
 };
 
@@ -110,7 +110,7 @@ static Layout make_layout(const fem_problem *pb, const ProblemShape &s, int R_ca
     const bool potts = pb->kind == FEM_BMINCUT;
     L.colsum0 = take(potts ? qR * 8 : 0);
     L.colsum1 = take(potts ? qR * 8 : 0);
-    L.colpart = take(potts ? (size_t)kColBlocks * qR * 8 : 0);
+    L.colsum2 = take(potts ? qR * 8 : 0);
     L.cfg = take((size_t)pb->n * R_cap);
     L.e_part_i = take((size_t)kEnergyChunks * R_cap * 8);
     L.e_part_d = take((size_t)kEnergyChunks * R_cap * 8);
@@ -174,11 +174,29 @@ static bool validate_graph(const fem_problem *pb, int64_t nnz, bool *integral, i
 static void configure_R(Handle *hd, int R) {
     hd->R = R;
     int Rb = R;
-    if (hd->opt_replica_block > 0) {
+    const double per_replica = 20.0 * (double)hd->dp.n * hd->dp.F;
+    const double budget = 0.45 * (double)hd->l2_bytes;
+    if (hd->dp.kind == FEM_BMINCUT) {
+        // a block must fit the team mapping of the Potts kernel (one variable's lanes inside a warp); among the
+        // divisors of R that do, take the requested one, else the largest that is L2-resident, else the smallest
+        const int q = hd->dp.q;
+        int largest = 1, resident = 0, smallest_vec = 0;
+        for (int d = 1; d <= R; ++d) {
+            if (R % d || !potts_block_ok(q, d)) continue;
+            largest = d;
+            if (per_replica * d <= budget) resident = d;
+            if (!smallest_vec && d % 2 == 0) smallest_vec = d;
+        }
+        if (hd->opt_replica_block > 0 && hd->opt_replica_block <= R && R % hd->opt_replica_block == 0 &&
+            potts_block_ok(q, (int)hd->opt_replica_block))
+            Rb = (int)hd->opt_replica_block;
+        else if (per_replica * R <= budget || hd->l2_bytes == 0)
+            Rb = largest;
+        else
+            Rb = resident > 1 ? resident : (smallest_vec ? smallest_vec : largest);
+    } else if (hd->opt_replica_block > 0) {
         if (hd->opt_replica_block < R && R % hd->opt_replica_block == 0) Rb = (int)hd->opt_replica_block;
     } else if (!hd->dp.J) {  // (the dense kind runs as one block: its tensor maps cover all R replicas)
-        const double per_replica = 20.0 * (double)hd->dp.n * hd->dp.F;
-        const double budget = 0.45 * (double)hd->l2_bytes;
         if (per_replica * R > budget) {
             const int vec = (R % 4 == 0) ? 4 : 1;
             int best = 0;
@@ -190,17 +208,8 @@ static void configure_R(Handle *hd, int R) {
     hd->Rb = Rb;
     while ((uint64_t)hd->rows * (uint64_t)hd->Rb >= (1ull << 32)) {  // kernels index a replica block with 32 bits
         int nb = R / hd->Rb + 1;
-        while (R % nb) ++nb;
+        while (R % nb || (hd->dp.kind == FEM_BMINCUT && !potts_block_ok(hd->dp.q, R / nb))) ++nb;
         hd->Rb = R / nb;
-    }
-    if (hd->dp.kind == FEM_BMINCUT) {  // one variable's replicas must fit one CTA pass
-        for (;;) {
-            const int vec = potts_vec(hd);
-            if (hd->Rb / vec <= kThreads) break;
-            int nb = R / hd->Rb + 1;
-            while (R % nb) ++nb;
-            hd->Rb = R / nb;
-        }
     }
 }
 
@@ -382,9 +391,14 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
     hd->m2W = reinterpret_cast<double *>(at(L.m2W));
     hd->gW[0] = reinterpret_cast<double *>(at(L.gW0));
     hd->gW[1] = reinterpret_cast<double *>(at(L.gW1));
-    hd->colsum[0] = reinterpret_cast<double *>(at(L.colsum0));
-    hd->colsum[1] = reinterpret_cast<double *>(at(L.colsum1));
-    hd->colpart = reinterpret_cast<double *>(at(L.colpart));
+    hd->colsum[0] = reinterpret_cast<long long *>(at(L.colsum0));
+    hd->colsum[1] = reinterpret_cast<long long *>(at(L.colsum1));
+    hd->colsum[2] = reinterpret_cast<long long *>(at(L.colsum2));
+    {   // |sum_i D_i(s)| < n: the largest power of two (up to 2^44) that keeps n * scale below 2^62
+        int bits = 0;
+        while (((int64_t)1 << bits) <= pb->n) ++bits;
+        hd->colsum_scale = std::ldexp(1.0, std::min(44, 62 - bits));
+    }
     hd->cfg = reinterpret_cast<int8_t *>(at(L.cfg));
     hd->e_part_i = reinterpret_cast<long long *>(at(L.e_part_i));
     hd->e_part_d = reinterpret_cast<double *>(at(L.e_part_d));
@@ -504,6 +518,7 @@ fem_status fem_get_moments(fem_handle *h, float *m1, float *m2) {
 static void ensure_gather(Handle *hd) {
     if (hd->gather_valid) return;
     StepScalars sc{};
+    sc.t = hd->t_done;
     if (hd->dp.kind == FEM_BMINCUT) launch_potts(hd, sc, hd->wide_live, /*step=*/false, 0, hd->R / hd->Rb);
     else launch_prepare_q2(hd, hd->wide_live);
     hd->gather_valid = true;
@@ -561,6 +576,7 @@ fem_status fem_anneal(fem_handle *h, const fem_schedule *sch, int32_t R, uint64_
         sc.one_minus_b2 = 1.0 - sch->beta2;
         sc.wd = sch->weight_decay;
         sc.two_lambda = 2.0 * (sch->lambda ? sch->lambda[t] : hd->pb.lambda);
+        sc.t = t;
         return sc;
     };
     auto one_step = [&](int t, int b0, int bc) {

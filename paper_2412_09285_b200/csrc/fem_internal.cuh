@@ -29,6 +29,7 @@ struct StepScalars {
     double rsqrt_bc2;  // 1 / sqrt(1 - beta2^(t+1))
     double eps, b1, b2, one_minus_b1, one_minus_b2, wd;
     double two_lambda;  // Potts balance term 2*lambda_t
+    int t;              // step number (the Potts column-sum buffers rotate with it)
 };
 
 // Device view of the problem (pointers into the workspace).
@@ -80,8 +81,8 @@ struct Handle {
     alignas(64) unsigned char tc_maps[6 * 128];  // CUtensorMap x6: J, Jlo, GT[0], GTlo[0], GT[1], GTlo[1]
     int tc_maps_R = -1;
     bool tc_ready = false;                   // g[cur]/glo[cur] hold GT / GT_lo of the current fields
-    double *colsum[2] = {nullptr, nullptr};  // Potts S[q][R]
-    double *colpart = nullptr;               // [kColBlocks][q*R]
+    long long *colsum[3] = {nullptr, nullptr, nullptr};  // Potts column sums S[q][R] in fixed point, rotating
+    double colsum_scale = 1.0;                            // fixed-point scale (a power of two)
     int8_t *cfg = nullptr;                   // [rows*R_cap]
     long long *e_part_i = nullptr;
     double *e_part_d = nullptr;
@@ -101,7 +102,7 @@ struct Handle {
     std::string err;
 };
 
-constexpr int kColBlocks = 592;     // Potts column-sum partial blocks (4 per SM)
+constexpr int kColBlocks = 592;     // CTAs of a Potts step launch (4 per SM, grid-stride over the variables)
 constexpr int kEnergyChunks = 1184;  // readout partials per replica (8 node slots x 148 blocks)
 
 // ---- launchers implemented in the .cu files (all asynchronous on hd->stream) ----

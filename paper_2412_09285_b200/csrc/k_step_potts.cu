@@ -1,13 +1,16 @@
 // Fused annealing step for the q-state Potts kind (balanced minimum cut).
 //
-// One thread owns VEC consecutive replicas of one variable and all q of its states: softmax of the
-// fields, the gather f_i(s) = sum_j W_ij D_j(s) of the centred marginals D = P - 1/q over the CSR row -- each neighbour is a
-// row of q*Rb contiguous floats --, g^p from S26 (edge-once reading R1) with the balance
-// term 2*lambda*[S_s - P_i(s)] (balance()) and the entropy term (h - lse)/beta, the chain
-// rule S20, Adam, and the next marginals.  The column sums S_s = sum_i P_i(s) of the NEXT
-// step are produced here as a by-product: per-thread partial sums over a fixed set of variables, a fixed
-// shared-memory tree per block, fp64 partials per block, and a tiny second kernel that adds the blocks
-// in order -- deterministic, no float atomics.
+// A TEAM of lanes owns one variable: the variable's row is q*Rb contiguous values [state][replica], lane l
+// of the team holds VEC consecutive replicas of state s = l / (Rb/VEC), so every access of the team -- the
+// streamed h / m1 / m2 rows and each CSR neighbour gather of the centred marginals D_j = P_j - 1/q -- is one
+// contiguous, vectorised segment (north_star subsystem 1).  Sums over the states (softmax normaliser, the
+// mean <g^p>_P of the chain rule S20) are butterfly shuffles across the team.  Per step and
+// lane: softmax of the fields, f_i(s) = sum_j W_ij D_j(s) over the CSR row, g^p from S26
+// (edge-once reading R1) with the balance term 2*lambda*[S_s - P_i(s)] (balance(),
+// PAPER.md:536) and the entropy term h_i(s)/beta (ln P = h - lse; lse is constant in s and cancels in
+// S20, like the "+1"), the chain rule, Adam, and the next marginals.  The column sums S_s of the NEXT step
+// are a by-product: every lane adds its new D' in 64-bit fixed point, so the sum is exact, independent of
+// the order and of the replica blocking, and integer atomics keep it deterministic (no float atomics).
 #include "device_math.cuh"
 
 namespace fem {
@@ -17,218 +20,202 @@ struct PottsParams {
     BlockArrays<T> a;
     DevProblem dp;
     Sc<T> sc;
-    const double *S_in;  // [q][Rb] of this block (blockIdx.y stride q*Rb)
-    double *partial;     // [gridDim.x][q*Rb] per block (blockIdx.y stride kColBlocks*q*Rb)
-    int rv;              // Rb / VEC lanes per variable
-    int npb;             // variables per CTA pass = kThreads / rv
+    const long long *S_in;  // fixed-point column sums of D(t), [q*Rb] per replica block
+    long long *S_out;       // accumulated by this launch: column sums of D(t+1)
+    long long *S_zero;      // cleared by this launch (the buffer the launch after next accumulates into)
+    double fx_scale, fx_inv;
+    int lps;             // lanes per state = Rb / VEC
+    int team;            // QPAD * lps lanes per variable (<= 32)
+    int teams_per_warp;  // 32 / team
+    unsigned row_len;    // q * Rb
 };
 
-template <typename T, int QMAX, int VEC, bool STEP>
-__global__ void __launch_bounds__(kThreads) potts_kernel(const PottsParams<T> p) {
+__device__ __forceinline__ float shfl_any(float v, int src) { return __shfl_sync(0xffffffffu, v, src); }
+__device__ __forceinline__ double shfl_any(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
+
+constexpr int kGatherChunk = 5;  // neighbour rows in flight per lane
+
+template <typename T, int QPAD, int VEC, bool STEP>
+__global__ void __launch_bounds__(kThreads) potts_team_kernel(const PottsParams<T> p) {
     using R = Row<T, VEC>;
-    __shared__ double red[kThreads];
-    const int q = p.dp.q, n = p.dp.n, Rb = p.a.Rb;
-    const int nl = threadIdx.x / p.rv;
-    const int c = (threadIdx.x - nl * p.rv) * VEC;
-    const bool lane_ok = nl < p.npb;
+    constexpr int kStages = QPAD == 32 ? 5 : QPAD == 16 ? 4 : QPAD == 8 ? 3 : QPAD == 4 ? 2 : 1;
+    __shared__ unsigned long long cta_sum[32 * VEC];
+    pdl_trigger();
+    const int q = p.dp.q, n = p.dp.n;
+    const int lane = threadIdx.x & 31;
+    const int tw = lane / p.team;       // team within the warp
+    const int l = lane - tw * p.team;   // lane within the team
+    const int s = l / p.lps;            // state of this lane
+    const int rl = l - s * p.lps;       // replica group of this lane
+    const bool lane_ok = tw < p.teams_per_warp && s < q;
+    int partner[kStages];               // butterfly partners across the states of the same replica group
+#pragma unroll
+    for (int k = 0; k < kStages; ++k)
+        partner[k] = tw < p.teams_per_warp ? tw * p.team + ((s ^ (1 << k)) * p.lps + rl) : lane;
+
     const int64_t blk = (int64_t)blockIdx.y * p.a.blk_stride;
-    const T *__restrict__ gin = p.a.g_in + blk + c;
-    const double *__restrict__ S = p.S_in + (int64_t)blockIdx.y * q * Rb;
+    const unsigned lo = (unsigned)(s * p.lps + rl) * VEC;  // offset inside a row
+    const T *__restrict__ gin = p.a.g_in + blk + lo;
     const Sc<T> &sc = p.sc;
     const T inv_q = (T)1 / (T)q;
+    const T neg_big = (T)-3.0e38;
+    const int warps_total = gridDim.x * (kThreads / 32);
+    const int warp_id = blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5);
+    const int stride = warps_total * p.teams_per_warp;
 
-    T colacc[QMAX][VEC];
-#pragma unroll
-    for (int s = 0; s < QMAX; ++s)
-#pragma unroll
-        for (int v = 0; v < VEC; ++v) colacc[s][v] = (T)0;
+    if (threadIdx.x < 32 * VEC) cta_sum[threadIdx.x] = 0ull;
+    pdl_wait();  // everything below reads or overwrites what the previous launch wrote
 
-    for (int i = blockIdx.x * p.npb + nl; lane_ok && i < n; i += gridDim.x * p.npb) {
-        const int64_t off = blk + (int64_t)i * q * Rb + c;
-        T h[QMAX][VEC], P[QMAX][VEC];
+    T Ss[VEC];
 #pragma unroll
-        for (int s = 0; s < QMAX; ++s) {
-            if (s < q) {
-                const R r = R::ld_stream(p.a.h + off + (int64_t)s * Rb);
+    for (int v = 0; v < VEC; ++v) Ss[v] = (T)0;
+    if (STEP && lane_ok) {
+        const long long *Sp = p.S_in + (int64_t)blockIdx.y * p.row_len + lo;
 #pragma unroll
-                for (int v = 0; v < VEC; ++v) h[s][v] = r.v[v];
-            }
+        for (int v = 0; v < VEC; ++v) Ss[v] = (T)((double)Sp[v] * p.fx_inv);
+    }
+    if (blockIdx.x == 0)
+        for (unsigned k = threadIdx.x; k < p.row_len; k += kThreads) p.S_zero[(int64_t)blockIdx.y * p.row_len + k] = 0ll;
+
+    long long colacc[VEC];
+#pragma unroll
+    for (int v = 0; v < VEC; ++v) colacc[v] = 0ll;
+
+    for (int base = warp_id * p.teams_per_warp; base < n; base += stride) {  // warp-uniform trip count
+        const int i = base + tw;
+        const bool ok = lane_ok && i < n;
+        const int64_t off = blk + (int64_t)(ok ? i : 0) * p.row_len + lo;
+        T h[VEC];
+        {
+            R r;
+            if (ok) r = R::ld_stream(p.a.h + off);
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) h[v] = ok ? r.v[v] : neg_big;
         }
         if (STEP) {
-            // softmax and log-sum-exp of h(t)
-            T lse[VEC];
+            // softmax of h(t) across the team's states
+            T P[VEC];
 #pragma unroll
             for (int v = 0; v < VEC; ++v) {
-                T mx = h[0][v];
+                T mx = h[v];
 #pragma unroll
-                for (int s = 1; s < QMAX; ++s)
-                    if (s < q) mx = fmax(mx, h[s][v]);
-                T z = (T)0;
+                for (int k = 0; k < kStages; ++k) mx = fmax(mx, shfl_any(mx, partner[k]));
+                const T e = ok ? fexp(h[v] - mx) : (T)0;
+                T z = e;
 #pragma unroll
-                for (int s = 0; s < QMAX; ++s)
-                    if (s < q) {
-                        P[s][v] = fexp(h[s][v] - mx);
-                        z += P[s][v];
-                    }
-                const T rz = frcp(z);
-#pragma unroll
-                for (int s = 0; s < QMAX; ++s)
-                    if (s < q) P[s][v] *= rz;
-                lse[v] = mx + flog(z);
+                for (int k = 0; k < kStages; ++k) z += shfl_any(z, partner[k]);
+                P[v] = e * frcp(z);
             }
-            // coupling contraction f(s) = sum_j W_ij P_j(s)
-            T f[QMAX][VEC];
+            // coupling contraction f(s) = sum_j W_ij D_j(s): kGatherChunk neighbour rows in flight
+            T f[VEC];
 #pragma unroll
-            for (int s = 0; s < QMAX; ++s)
-#pragma unroll
-                for (int v = 0; v < VEC; ++v) f[s][v] = (T)0;
-            int e0, e1;
-            if (p.dp.uniform_deg > 0) {
-                e0 = i * p.dp.uniform_deg;
-                e1 = e0 + p.dp.uniform_deg;
-            } else {
-                e0 = __ldg(p.dp.row_ptr + i);
-                e1 = __ldg(p.dp.row_ptr + i + 1);
-            }
-            for (int e = e0; e < e1; ++e) {
-                const int j = __ldg(p.dp.col + e);
-                const T wj = p.dp.w ? (T)__ldg(p.dp.w + e) : (T)1;
-                const T *row = gin + (int64_t)j * q * Rb;
-#pragma unroll
-                for (int s = 0; s < QMAX; ++s)
-                    if (s < q) {
-                        const R r = R::ld(row + (int64_t)s * Rb);
-#pragma unroll
-                        for (int v = 0; v < VEC; ++v) f[s][v] += wj * r.v[v];
-                    }
-            }
-            // g^p (S26, the "+1" of the entropy term cancels in S20), then g^h = P (g^p - <g^p>_P)
-            T gbar[VEC];
-#pragma unroll
-            for (int v = 0; v < VEC; ++v) gbar[v] = (T)0;
-#pragma unroll
-            for (int s = 0; s < QMAX; ++s)
-                if (s < q) {
-#pragma unroll
-                    for (int v = 0; v < VEC; ++v) {
-                        const T Ss = (T)S[s * Rb + c + v];
-                        f[s][v] = -f[s][v] + sc.two_lambda * (Ss - P[s][v]) + (h[s][v] - lse[v]) * sc.inv_beta;
-                        gbar[v] += P[s][v] * f[s][v];
-                    }
+            for (int v = 0; v < VEC; ++v) f[v] = (T)0;
+            if (ok) {
+                int e0, e1;
+                if (p.dp.uniform_deg > 0) {
+                    e0 = i * p.dp.uniform_deg;
+                    e1 = e0 + p.dp.uniform_deg;
+                } else {
+                    e0 = __ldg(p.dp.row_ptr + i);
+                    e1 = __ldg(p.dp.row_ptr + i + 1);
                 }
-            // Adam per state; h[s] becomes the new (fp32-rounded) field
+                for (int e = e0; e < e1; e += kGatherChunk) {
+                    unsigned jj[kGatherChunk];
+                    T ww[kGatherChunk];
+                    R nb[kGatherChunk];
 #pragma unroll
-            for (int s = 0; s < QMAX; ++s)
-                if (s < q) {
-                    R m1 = R::ld_stream(p.a.m1 + off + (int64_t)s * Rb);
-                    R m2 = R::ld_stream(p.a.m2 + off + (int64_t)s * Rb);
-                    R hn;
-#pragma unroll
-                    for (int v = 0; v < VEC; ++v) {
-                        const T g = P[s][v] * (f[s][v] - gbar[v]);
-                        hn.v[v] = adam_update(h[s][v], g, m1.v[v], m2.v[v], sc);
-                        h[s][v] = hn.v[v];
+                    for (int k = 0; k < kGatherChunk; ++k) {
+                        const bool in = e + k < e1;
+                        jj[k] = in ? (unsigned)__ldg(p.dp.col + e + k) : (unsigned)i;
+                        ww[k] = in ? (p.dp.w ? (T)__ldg(p.dp.w + e + k) : (T)1) : (T)0;
                     }
-                    hn.st_stream(p.a.h + off + (int64_t)s * Rb);
-                    m1.st_stream(p.a.m1 + off + (int64_t)s * Rb);
-                    m2.st_stream(p.a.m2 + off + (int64_t)s * Rb);
+#pragma unroll
+                    for (int k = 0; k < kGatherChunk; ++k) nb[k] = R::ld(gin + jj[k] * p.row_len);
+#pragma unroll
+                    for (int k = 0; k < kGatherChunk; ++k)
+#pragma unroll
+                        for (int v = 0; v < VEC; ++v) f[v] += ww[k] * nb[k].v[v];
                 }
+            }
+            // g^p (S26), then g^h = P (g^p - <g^p>_P) (S20), Adam
+            R m1, m2, hn;
+            if (ok) {
+                m1 = R::ld_stream(p.a.m1 + off);
+                m2 = R::ld_stream(p.a.m2 + off);
+            }
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) {
+                const T gp = ok ? -f[v] + sc.two_lambda * (Ss[v] - P[v]) + h[v] * sc.inv_beta : (T)0;
+                T gbar = P[v] * gp;
+#pragma unroll
+                for (int k = 0; k < kStages; ++k) gbar += shfl_any(gbar, partner[k]);
+                if (ok) {
+                    const T g = P[v] * (gp - gbar);
+                    hn.v[v] = adam_update(h[v], g, m1.v[v], m2.v[v], sc);
+                    h[v] = hn.v[v];
+                }
+            }
+            if (ok) {
+                hn.st_stream(p.a.h + off);
+                m1.st_stream(p.a.m1 + off);
+                m2.st_stream(p.a.m2 + off);
+            }
         }
-        // marginals of the (new) fields -> g_out, and their column sums
+        // centred marginals D = P - 1/q of the (new) fields -> g_out, and their column sums.  Constants in s
+        // cancel in S20, and near the uniform start the deviation from 1/q is all the signal there is, so it
+        // is what gets stored and gathered.
+        R po;
 #pragma unroll
         for (int v = 0; v < VEC; ++v) {
-            T mx = h[0][v];
+            T mx = h[v];
 #pragma unroll
-            for (int s = 1; s < QMAX; ++s)
-                if (s < q) mx = fmax(mx, h[s][v]);
-            T z = (T)0;
+            for (int k = 0; k < kStages; ++k) mx = fmax(mx, shfl_any(mx, partner[k]));
+            const T e = ok ? fexp(h[v] - mx) : (T)0;
+            T z = e;
 #pragma unroll
-            for (int s = 0; s < QMAX; ++s)
-                if (s < q) {
-                    P[s][v] = fexp(h[s][v] - mx);
-                    z += P[s][v];
-                }
-            const T rz = frcp(z);
-#pragma unroll
-            for (int s = 0; s < QMAX; ++s)
-                if (s < q) P[s][v] *= rz;
+            for (int k = 0; k < kStages; ++k) z += shfl_any(z, partner[k]);
+            po.v[v] = e * frcp(z) - inv_q;
+            if (ok) colacc[v] += __double2ll_rn((double)po.v[v] * p.fx_scale);
         }
-#pragma unroll
-        for (int s = 0; s < QMAX; ++s)
-            if (s < q) {
-                R po;
-#pragma unroll
-                for (int v = 0; v < VEC; ++v) {
-                    // centred marginal D = P - 1/q: constants in s cancel in S20, and near the uniform start
-                    // the deviation is all the signal, so it is what gets stored and gathered
-                    po.v[v] = P[s][v] - inv_q;
-                    colacc[s][v] += po.v[v];  // sum what the next step will gather
-                }
-                po.st(p.a.g_out + off + (int64_t)s * Rb);
-            }
+        if (ok) po.st(p.a.g_out + off);
     }
 
-    // block reduction over the npb variable slots, fixed order, fp64; one partial row per CTA
-    double *part = p.partial + ((int64_t)blockIdx.y * gridDim.x + blockIdx.x) * q * Rb;
+    // column sums: exact integer adds -- lanes -> CTA (shared atomics) -> grid (global atomics)
+    __syncthreads();
+    if (lane_ok) {
 #pragma unroll
-    for (int s = 0; s < QMAX; ++s) {
-        if (s < q) {  // q is uniform over the CTA, so the barriers below are too
-#pragma unroll
-            for (int v = 0; v < VEC; ++v) {
-                __syncthreads();
-                red[threadIdx.x] = lane_ok ? (double)colacc[s][v] : 0.0;
-                __syncthreads();
-                if (nl == 0 && lane_ok) {
-                    double acc = 0.0;
-                    for (int k = 0; k < p.npb; ++k) acc += red[k * p.rv + threadIdx.x];
-                    part[s * Rb + c + v] = acc;
-                }
-            }
-        }
+        for (int v = 0; v < VEC; ++v)
+            if (colacc[v] != 0ll) atomicAdd(&cta_sum[l * VEC + v], (unsigned long long)colacc[v]);
+    }
+    __syncthreads();
+    if (threadIdx.x < p.row_len) {  // row_len = q * Rb <= 32 * VEC; team lane l covers row offsets l*VEC ..
+        const unsigned long long v = cta_sum[threadIdx.x];
+        if (v != 0ull)
+            atomicAdd(reinterpret_cast<unsigned long long *>(p.S_out) + (int64_t)blockIdx.y * p.row_len + threadIdx.x, v);
     }
 }
 
-// S[s][a] = sum over CTAs of the partial rows, in CTA order (deterministic), fp64.
-__global__ void __launch_bounds__(kThreads) potts_colsum_kernel(const double *partial, double *S, int nparts, int qR) {
-    const int k = blockIdx.x * kThreads + threadIdx.x;
-    if (k >= qR) return;
-    const double *pp = partial + (int64_t)blockIdx.y * nparts * qR;
-    double acc = 0.0;
-    for (int b = 0; b < nparts; ++b) acc += pp[(int64_t)b * qR + k];
-    S[(int64_t)blockIdx.y * qR + k] = acc;
-}
-
-template <typename T, int QMAX, int VEC>
+template <typename T, int QPAD, int VEC>
 static void launch_potts_t(Handle *hd, const PottsParams<T> &p, dim3 grid, bool step) {
-    if (step)
-        potts_kernel<T, QMAX, VEC, true><<<grid, kThreads, 0, hd->stream>>>(p);
-    else
-        potts_kernel<T, QMAX, VEC, false><<<grid, kThreads, 0, hd->stream>>>(p);
+    if (step) launch_pdl(potts_team_kernel<T, QPAD, VEC, true>, grid, dim3(kThreads), hd->stream, p);
+    else launch_pdl(potts_team_kernel<T, QPAD, VEC, false>, grid, dim3(kThreads), hd->stream, p);
 }
 
-template <typename T>
-static void launch_potts_q(Handle *hd, PottsParams<T> &p, dim3 grid, bool step, int vec) {
-    const int q = hd->dp.q;
-    if (q <= 4) {
-        if (vec == 4) launch_potts_t<T, 4, 4>(hd, p, grid, step);
-        else if (vec == 2) launch_potts_t<T, 4, 2>(hd, p, grid, step);
-        else launch_potts_t<T, 4, 1>(hd, p, grid, step);
-    } else if (q <= 8) {
-        if (vec >= 2) launch_potts_t<T, 8, 2>(hd, p, grid, step);
-        else launch_potts_t<T, 8, 1>(hd, p, grid, step);
-    } else if (q <= 16) {
-        launch_potts_t<T, 16, 1>(hd, p, grid, step);
-    } else {
-        launch_potts_t<T, 32, 1>(hd, p, grid, step);
-    }
+template <typename T, int QPAD>
+static void launch_potts_v(Handle *hd, const PottsParams<T> &p, dim3 grid, bool step, int vec) {
+    if (vec == 4) launch_potts_t<T, QPAD, 4>(hd, p, grid, step);
+    else if (vec == 2) launch_potts_t<T, QPAD, 2>(hd, p, grid, step);
+    else launch_potts_t<T, QPAD, 1>(hd, p, grid, step);
 }
 
-int potts_vec(const Handle *hd) {
-    const int q = hd->dp.q, Rb = hd->Rb;
-    if (q <= 4) return Rb % 4 == 0 ? 4 : (Rb % 2 == 0 ? 2 : 1);
-    if (q <= 8) return Rb % 2 == 0 ? 2 : 1;
-    return 1;
+int potts_qpad(int q) {
+    int qp = 2;
+    while (qp < q) qp <<= 1;
+    return qp;
 }
+int potts_vec(int Rb) { return Rb % 4 == 0 ? 4 : (Rb % 2 == 0 ? 2 : 1); }
+// a replica block fits the team mapping when one variable's lanes fit a warp
+bool potts_block_ok(int q, int Rb) { return potts_qpad(q) * (Rb / potts_vec(Rb)) <= 32; }
 
 template <typename T>
 static void launch_potts_typed(Handle *hd, const StepScalars &sc, bool step, int blk_begin, int blk_count) {
@@ -245,22 +232,40 @@ static void launch_potts_typed(Handle *hd, const StepScalars &sc, bool step, int
     p.a.Rb = Rb;
     p.dp = hd->dp;
     p.sc = Sc<T>(sc);
-    p.S_in = hd->colsum[hd->cur] + (int64_t)blk_begin * q * Rb;
-    p.partial = hd->colpart + (int64_t)blk_begin * kColBlocks * q * Rb;
-    const int vec = potts_vec(hd);  // fem_anneal keeps Rb / vec <= kThreads (one variable inside one CTA pass)
-    p.rv = Rb / vec;
-    p.npb = kThreads / p.rv;
-    const int nblk = (int)std::min<int64_t>(kColBlocks, ceil_div(hd->dp.n, p.npb));
+    // column-sum buffers rotate with the step number: step t reads [t%3], accumulates [(t+1)%3], clears [(t+2)%3];
+    // the preparation at step t accumulates [t%3] (cleared by the caller) and clears [(t+1)%3]
+    const int64_t so = (int64_t)blk_begin * q * Rb;
+    const int t = sc.t;
+    p.S_in = hd->colsum[t % 3] + so;
+    p.S_out = hd->colsum[(step ? t + 1 : t) % 3] + so;
+    p.S_zero = hd->colsum[(step ? t + 2 : t + 1) % 3] + so;
+    p.fx_scale = hd->colsum_scale;
+    p.fx_inv = 1.0 / hd->colsum_scale;
+    const int vec = potts_vec(Rb);
+    const int qpad = potts_qpad(q);
+    p.lps = Rb / vec;
+    p.team = qpad * p.lps;
+    p.teams_per_warp = 32 / p.team;
+    p.row_len = (unsigned)(q * Rb);
+    const int64_t warps_needed = ceil_div(hd->dp.n, p.teams_per_warp);
+    const int nblk = (int)std::min<int64_t>(kColBlocks, ceil_div(warps_needed, kThreads / 32));
     dim3 grid((unsigned)nblk, (unsigned)blk_count);
-    launch_potts_q<T>(hd, p, grid, step, vec);
-    double *S_out = (step ? hd->colsum[hd->cur ^ 1] : hd->colsum[hd->cur]) + (int64_t)blk_begin * q * Rb;
-    dim3 g2((unsigned)ceil_div((int64_t)q * Rb, kThreads), (unsigned)blk_count);
-    potts_colsum_kernel<<<g2, kThreads, 0, hd->stream>>>(p.partial, S_out, nblk, q * Rb);
-    hd->launches += 2;
+    switch (qpad) {
+        case 2: launch_potts_v<T, 2>(hd, p, grid, step, vec); break;
+        case 4: launch_potts_v<T, 4>(hd, p, grid, step, vec); break;
+        case 8: launch_potts_v<T, 8>(hd, p, grid, step, vec); break;
+        case 16: launch_potts_v<T, 16>(hd, p, grid, step, vec); break;
+        default: launch_potts_v<T, 32>(hd, p, grid, step, vec); break;
+    }
+    hd->launches++;
 }
 
-// step == false: centred marginals + column sums of the current fields into g[cur] / colsum[cur] (t = 0).
+// step == false: centred marginals + column sums of the current fields into g[cur] / colsum[t % 3].
 void launch_potts(Handle *hd, const StepScalars &sc, bool wide, bool step, int blk_begin, int blk_count) {
+    if (!step) {
+        const size_t bytes = (size_t)hd->dp.q * hd->Rb * blk_count * sizeof(long long);
+        cudaMemsetAsync(hd->colsum[sc.t % 3] + (int64_t)blk_begin * hd->dp.q * hd->Rb, 0, bytes, hd->stream);
+    }
     if (wide) launch_potts_typed<double>(hd, sc, step, blk_begin, blk_count);
     else launch_potts_typed<float>(hd, sc, step, blk_begin, blk_count);
 }
