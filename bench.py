@@ -167,6 +167,8 @@ def main():
     ap.add_argument("--replica-block", type=int, default=None, help="override the replica_block option")
     ap.add_argument("--steps-per-block", type=int, default=None)
     ap.add_argument("--precise-steps", type=int, default=8)
+    ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
+                    help="library option passed to fem_set_option (e.g. tensor_cores=0); repeatable")
     ap.add_argument("--anneal-steps", type=int, default=None,
                     help="shorten the schedule (profiling under ncu only; such a run is not a bench value)")
     args = ap.parse_args()
@@ -209,6 +211,9 @@ def main():
             eng.set_option("replica_block", args.replica_block)
         if args.steps_per_block is not None:
             eng.set_option("steps_per_block", args.steps_per_block)
+        for kv in args.opt:
+            key, _, val = kv.partition("=")
+            eng.set_option(key, int(val))
 
     eng = fem.Fem(inst, R, device=f"cuda:{local_rank}")
     apply_options(eng)

@@ -138,9 +138,13 @@ fem_status fem_energy_of(fem_handle *h, const int32_t *cfg /* [count][n] */, int
 /* Tuning knobs (all optional): "replica_block" (replicas per L2-resident block; 0 = chosen from the
  * device's L2 size, the default; >= R = no blocking), "steps_per_block" (steps run on one replica
  * block before moving to the next; 0 = the whole anneal per block, the default; 1 = step-major).
- * Results do not depend on either (replicas are independent).  Unknown key: FEM_EINVAL. */
+ * Results do not depend on either (replicas are independent).  Dense ISING only: "tensor_cores"
+ * (1 = tcgen05 3xTF32 step, the default where it applies: n % 4 == 0 and R % 32 == 0; 0 = CUDA-core
+ * GEMM) and "tc_tile_n" (replica columns per tensor-core tile: 0 = default, 32/64/128/256).
+ * Unknown key: FEM_EINVAL. */
 fem_status fem_set_option(fem_handle *h, const char *key, int64_t value);
-/* Introspection for benchmarks: "launches" (kernels enqueued so far), "t_done", "R", "nnz",
+/* Introspection for benchmarks: "launches" (kernels enqueued so far), "tc_launches" (of which tcgen05
+ * dense steps), "t_done", "R", "nnz",
  * "step_bytes" (algorithmic HBM bytes of one fused step). */
 int64_t fem_get_info(const fem_handle *h, const char *key);
 

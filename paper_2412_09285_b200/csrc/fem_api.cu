@@ -18,7 +18,6 @@ void launch_sigmoid(Handle *hd, float *out);
 bool potts_block_ok(int q, int Rb);
 void launch_potts_softmax(Handle *hd, float *out);
 void launch_tc_split(Handle *hd);
-int tc_tile_n(int n, int Rb);
 
 static std::string g_create_error;
 
@@ -442,6 +441,10 @@ fem_status fem_set_option(fem_handle *h, const char *key, int64_t value) {
     } else if (!strcmp(key, "steps_per_block")) {
         if (value < 0) return fail(hd, FEM_EINVAL, "steps_per_block must be >= 0");
         hd->opt_steps_per_block = value;
+    } else if (!strcmp(key, "tc_tile_n")) {
+        if (value != 0 && value != 32 && value != 64 && value != 128 && value != 256)
+            return fail(hd, FEM_EINVAL, "tc_tile_n must be 0, 32, 64, 128 or 256");
+        hd->opt_tc_tile_n = value;
     } else if (!strcmp(key, "tensor_cores")) {
         if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "tensor_cores must be 0 or 1");
         hd->opt_tensor_cores = value;
@@ -455,6 +458,7 @@ int64_t fem_get_info(const fem_handle *h, const char *key) {
     const Handle *hd = reinterpret_cast<const Handle *>(h);
     if (!hd || !key) return -1;
     if (!strcmp(key, "launches")) return hd->launches;
+    if (!strcmp(key, "tc_launches")) return hd->tc_launches;
     if (!strcmp(key, "t_done")) return hd->t_done;
     if (!strcmp(key, "R")) return hd->R;
     if (!strcmp(key, "replica_block")) return hd->Rb;

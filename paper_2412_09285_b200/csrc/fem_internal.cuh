@@ -94,8 +94,9 @@ struct Handle {
     int cur = 0;          // g[cur] holds the gathered quantity of the current fields
     int t_done = 0;
     bool injected = false, readout_valid = false, gather_valid = false;
-    int64_t opt_replica_block = 0, opt_steps_per_block = 0, opt_tensor_cores = 0;
+    int64_t opt_replica_block = 0, opt_steps_per_block = 0, opt_tensor_cores = 1, opt_tc_tile_n = 0;
     int64_t launches = 0;
+    int64_t tc_launches = 0;  // launches of the tcgen05 dense step (k_dense_tc.cu)
     int64_t l2_bytes = 0;  // device L2 size (0 when unknown: no automatic replica blocking)
     int64_t structure_bytes = 0;  // problem-structure bytes one step reads (indices, weights, clause entries)
     double lambda_last = 0.0;     // balance weight of the last executed step (readout uses it)

@@ -27,12 +27,18 @@ constexpr int TC_BK = 32;       // floats per k-block = one 128-byte swizzle ato
 constexpr int TC_UMMA_K = 8;    // tf32 elements per tcgen05.mma
 constexpr int TC_THREADS = 192;
 
+// The tensor core adds each MMA's result into the fp32 accumulator with truncation, so a long accumulation
+// chain carries a bias towards zero that grows with the number of adds and the size of the running sum
+// (measured: one 1536-add chain per output leaves 1.6e-4 on the marginals at step 50 of cfg 4b).  The k range
+// is therefore cut into chunks that accumulate in SEPARATE TMEM accumulators, and the two small 3xTF32 terms
+// get an accumulator of their own; the epilogue adds the kAcc partial sums in fp32, round to nearest.
 template <int BN>
 struct TcShape {
     static constexpr int kStageBytes = 2 * TC_BM * 128 + 2 * BN * 128;  // A_hi, A_lo, B_hi, B_lo
     static constexpr int kStages = BN >= 256 ? 2 : (BN >= 128 ? 3 : 4);
     static constexpr int kSmem = kStages * kStageBytes + 1024;  // + alignment slack
-    static constexpr int kTmemCols = BN < 32 ? 32 : BN;
+    static constexpr int kAcc = 512 / BN > 8 ? 8 : 512 / BN;    // accumulators: [0] small terms, [1..] chunks of k
+    static constexpr int kTmemCols = kAcc * BN;                 // 256 or 512 columns (a power of two >= 32)
 };
 
 struct TcParams {
@@ -124,6 +130,7 @@ dense_tc_step_kernel(const __grid_constant__ CUtensorMap tmJ, const __grid_const
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int m0 = blockIdx.x * TC_BM, n0 = blockIdx.y * BN;
     const int nkb = (p.n + TC_BK - 1) / TC_BK;
+    const int nchunks = nkb < S::kAcc - 1 ? nkb : S::kAcc - 1;  // chunks of k the main term is cut into
 
     if (warp == 0 && lane == 0) {
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmJ));
@@ -165,7 +172,10 @@ dense_tc_step_kernel(const __grid_constant__ CUtensorMap tmJ, const __grid_const
     } else if (warp == 1 && lane == 0) {
         // ===== MMA issuer =====
         constexpr uint32_t idesc = umma_idesc_tf32(TC_BM, BN);
+        uint32_t started = 0;  // bit c: accumulator c holds something
         for (int kb = 0; kb < nkb; ++kb) {
+            const int c = 1 + (kb * nchunks) / nkb;  // accumulator of this k-block's main term
+            const uint32_t d_main = tmem_d + (uint32_t)(c * BN);
             const int s = kb % S::kStages;
             const uint32_t ph = (kb / S::kStages) & 1;
             mbar_wait(&full_bar[s], ph);
@@ -179,9 +189,10 @@ dense_tc_step_kernel(const __grid_constant__ CUtensorMap tmJ, const __grid_const
                 const uint32_t ko = k * TC_UMMA_K * 4;  // bytes inside the 128-byte swizzle atom
                 const uint64_t dAh = umma_desc_sw128(a_hi + ko), dAl = umma_desc_sw128(a_lo + ko);
                 const uint64_t dBh = umma_desc_sw128(b_hi + ko), dBl = umma_desc_sw128(b_lo + ko);
-                umma_tf32(tmem_d, dAl, dBh, idesc, (kb | k) != 0);  // small terms first
+                umma_tf32(tmem_d, dAl, dBh, idesc, started & 1u);
                 umma_tf32(tmem_d, dAh, dBl, idesc, 1);
-                umma_tf32(tmem_d, dAh, dBh, idesc, 1);
+                umma_tf32(d_main, dAh, dBh, idesc, (started >> c) & 1u);
+                started |= 1u | (1u << c);
             }
             umma_commit(&empty_bar[s]);  // frees the smem stage when these MMAs have read it
         }
@@ -198,7 +209,16 @@ dense_tc_step_kernel(const __grid_constant__ CUtensorMap tmJ, const __grid_const
 #pragma unroll 1
         for (int c0 = 0; c0 < BN; c0 += 16) {
             float f[16];
-            tmem_ld16(tmem_d + ((uint32_t)(quad * 32) << 16) + (uint32_t)c0, f);  // warp-collective: no divergence here
+            const uint32_t lane_base = tmem_d + ((uint32_t)(quad * 32) << 16) + (uint32_t)c0;
+            tmem_ld16(lane_base + (uint32_t)BN, f);  // warp-collective: no divergence here
+#pragma unroll
+            for (int c = 2; c <= S::kAcc; ++c) {    // chunks of the main term in k order, the small terms last
+                if (c < S::kAcc && c > nchunks) continue;  // (warp-uniform)
+                float part[16];
+                tmem_ld16(lane_base + (uint32_t)((c % S::kAcc) * BN), part);
+#pragma unroll
+                for (int k = 0; k < 16; ++k) f[k] += part[k];
+            }
             if (row_ok) {
                 float hv[16], a1[16], a2[16];
 #pragma unroll
@@ -296,10 +316,13 @@ static bool make_map(CUtensorMap *tm, const float *base, int rows, int cols, int
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-int tc_tile_n(int n, int Rb) {  // 0 = tensor-core path not applicable
+int tc_tile_n(int n, int Rb, int forced) {  // 0 = tensor-core path not applicable
     if (n % 4 != 0) return 0;   // TMA needs a 16-byte row pitch
-    for (int bn : {256, 128, 64, 32})
-        if (Rb % bn == 0) return bn;
+    // default 128: four accumulators (small terms + three chunks of k); 256 is ~7% faster per step but has room
+    // for two accumulators only (5e-5 instead of 2e-5 on the marginals at step 50 of cfg 4b)
+    for (int bn : {128, 64, 32})
+        if (Rb % bn == 0 && (forced == 0 || forced == bn)) return bn;
+    if (forced == 256 && Rb % 256 == 0) return 256;
     return 0;
 }
 
@@ -336,7 +359,7 @@ void launch_tc_split(Handle *hd) {
 // back to the CUDA-core GEMM).
 bool launch_step_dense_tc(Handle *hd, const StepScalars &sc) {
     const int n = hd->dp.n, Rb = hd->Rb;
-    const int bn = tc_tile_n(n, Rb);
+    const int bn = tc_tile_n(n, Rb, (int)hd->opt_tc_tile_n);
     if (bn == 0 || hd->R != Rb || !hd->Jlo || !hd->opt_tensor_cores) return false;
     if (hd->tc_maps_R != hd->R) {  // tensor maps depend on R (rows of GT) -- rebuild when it changes
         CUtensorMap *m = reinterpret_cast<CUtensorMap *>(hd->tc_maps);
@@ -370,7 +393,10 @@ bool launch_step_dense_tc(Handle *hd, const StepScalars &sc) {
         case 64: ok = launch_tc<64>(hd, p, maps); break;
         default: ok = launch_tc<32>(hd, p, maps); break;
     }
-    if (ok) hd->launches++;
+    if (ok) {
+        hd->launches++;
+        hd->tc_launches++;
+    }
     return ok;
 }
 

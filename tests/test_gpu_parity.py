@@ -33,7 +33,8 @@ def small_instances():
         "maxcut_reg3_pm1": (wl.random_regular(5000, 3, 2005, wl.MAXCUT, pm1=True), 32),
         "maxcut_er_odd_R": (wl.erdos_renyi_maxcut(257, 0.08, 2006, pm1=True), 7),
         "ising_sparse": (wl.sparse_ising_from(wl.torus_maxcut(20, 2007), -0.5), 16),
-        "ising_dense_sk": (wl.sk_dense(200, 2008), 40),
+        "ising_dense_sk": (wl.sk_dense(200, 2008), 40),            # R % 32 != 0: CUDA-core GEMM
+        "ising_dense_sk_tc": (wl.sk_dense(328, 2011), 96),         # tcgen05 path: ragged row tile and k block, 3 column tiles
         "bmincut_q8_reg10": (reg, 16),
         "bmincut_q3_reg6_odd_R": (reg3, 10),
         "bmincut_q5_weighted": (potts_w, 12),
@@ -61,7 +62,7 @@ def get(name):
 
 
 NAMES = ["cfg0_maxcut_er800", "maxcut_torus_30x34", "maxcut_reg3_pm1", "maxcut_er_odd_R", "ising_sparse",
-         "ising_dense_sk", "bmincut_q8_reg10", "bmincut_q3_reg6_odd_R", "bmincut_q5_weighted", "maxsat_k4",
+         "ising_dense_sk", "ising_dense_sk_tc", "bmincut_q8_reg10", "bmincut_q3_reg6_odd_R", "bmincut_q5_weighted", "maxsat_k4",
          "maxsat_k3_odd_R"]
 
 
@@ -236,3 +237,24 @@ def test_full_anneal_energy_distribution_cfg0(fem):
     assert abs(res["energy_int"].mean() - ref.mean()) <= 0.005 * abs(ref.mean())
     assert res["energy_int"].min() <= 0.995 * ref.min()              # energies are negative cuts
     eng.close()
+
+
+def test_dense_tensor_core_path_is_taken_and_agrees_with_cuda_cores(fem):
+    """Dense Ising: the tcgen05 3xTF32 step (default) against the CUDA-core GEMM step on the same fields, and
+    against the oracle; the info counter proves which kernel ran."""
+    inst, R = get("ising_dense_sk_tc")
+    beta = fem.linear_temperature_schedule(1.0, 0.01, 500)
+    h0 = fo.init_fields(5, R, inst.n, 1).astype(np.float32)
+    pb, st = oracle_run(inst, h0, beta, 30, inst.lam)
+    P_ref = fo.marginals(pb, st.h)
+    out = {}
+    for tc in (1, 0):
+        eng = fem.Fem(inst, R)
+        eng.set_option("tensor_cores", tc)
+        eng.set_fields(h0)
+        eng.anneal(fem.Schedule(beta=beta, precise_steps=8), R, stop_after=30)
+        out[tc] = eng.get_marginals().astype(np.float64)
+        assert (eng.info("tc_launches") == 22) == (tc == 1)         # 30 steps - 8 wide ones
+        assert np.max(np.abs(out[tc] - P_ref.reshape(out[tc].shape))) < MARGINAL_TOL
+        eng.close()
+    assert np.max(np.abs(out[1] - out[0])) < MARGINAL_TOL
