@@ -44,6 +44,14 @@ def load_peaks():
     return 6650.0, "fallback (B200_PROFILING.md, 6.65 TB/s)"
 
 
+def load_peak_file():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f)
+    return {}
+
+
 def load_traffic(workload: str):
     """dram bytes per launch of the fused step kernel from the committed ncu capture, or None."""
     path = os.path.join(ROOT, "profiles", "traffic.json")
@@ -300,7 +308,34 @@ def main():
         value = updates * args.steps * world / (elapsed_ms * 1e-3)
         peak, peak_src = load_peaks()
         kernel_us = bulk_ms * 1e3 / bulk_launches
-        achieved = step_bytes / (kernel_us * 1e-6) / 1e9
+        peaks = load_peak_file()
+        if inst.dense_J is not None and eng.info("tc_launches") > 0:
+            # dense couplings: J.M is a GEMM (2 n^2 R flop per step) on tcgen05 kind::tf32.  The 3xTF32 split issues
+            # three MMAs per algorithmic product; `achieved` counts the ALGORITHMIC flops only.
+            flops = 2.0 * n * n * R
+            achieved = flops / (kernel_us * 1e-6) / 1e12
+            tf32_peak = 0.5 * float(peaks.get("bf16_tflops_sustained", peaks.get("bf16_tflops", 1671.0)))
+            roofline = {"bound": "tensor",
+                        "kernel": "dense_tc_step_kernel (tcgen05 3xTF32 GEMM, FEM update fused in the TMEM epilogue)",
+                        "achieved": achieved, "peak": tf32_peak, "unit": "TFLOP/s", "frac": achieved / tf32_peak,
+                        "traffic": load_traffic(args.workload),
+                        "peak_source": "0.5 x measured sustained bf16 cuBLAS TFLOP/s (MEASURED_PEAKS.json; "
+                                       "tf32:bf16 nominal ratio 1:2)",
+                        "algorithmic_flops_per_launch": flops, "mma_tflops_issued": 3.0 * achieved,
+                        "kernel_us": kernel_us, "kernel_share_of_step": bulk_ms / elapsed_ms}
+        else:
+            achieved = step_bytes / (kernel_us * 1e-6) / 1e9
+            kname = ("potts_team_kernel<float> (fused softmax + gather + balance + chain rule + Adam)"
+                     if inst.kind == wl.BMINCUT else
+                     "step_q2_kernel<float> (fused gather + entropy gradient + Adam)")
+            roofline = {"bound": "hbm", "kernel": kname,
+                        "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                        "traffic": load_traffic(args.workload), "peak_source": peak_src,
+                        "algorithmic_bytes_per_launch": step_bytes, "kernel_us": kernel_us,
+                        "kernel_share_of_step": bulk_ms / elapsed_ms}
+            if inst.kind == wl.MAXSAT:
+                roofline["note"] = ("state is L2-resident; the binding roof is L2->SM gather bandwidth "
+                                    "((k-1) rows of R floats per literal occurrence), not HBM (DESIGN.md section 6)")
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": elapsed_ms / args.steps, "higher_is_better": True,
@@ -309,11 +344,7 @@ def main():
                        "precise_steps": K, "replica_block": eng.info("replica_block"),
                        "l2": "256 MiB buffer written between timed passes (L2 flush)",
                        "parallelism": f"replicas x{world}" if world > 1 else "single GPU"},
-            "roofline": {"bound": "hbm", "kernel": "step_q2_kernel<float> (fused gather + entropy gradient + Adam)",
-                         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": load_traffic(args.workload), "peak_source": peak_src,
-                         "algorithmic_bytes_per_launch": step_bytes, "kernel_us": kernel_us,
-                         "kernel_share_of_step": bulk_ms / elapsed_ms},
+            "roofline": roofline,
             "e2e": {"value": updates * e2e_steps * world / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "steps": e2e_steps},
             "gpu_launches": int(launches),

@@ -179,11 +179,14 @@ static void configure_R(Handle *hd, int R) {
         // a block must fit the team mapping of the Potts kernel (one variable's lanes inside a warp); among the
         // divisors of R that do, take the requested one, else the largest that is L2-resident, else the smallest
         const int q = hd->dp.q;
-        int largest = 1, resident = 0, smallest_vec = 0;
+        // gathers_fit: the two gather buffers (8 B per field) of the block fit in L2 even though the streamed
+        // arrays do not -- neighbour rows are then served from L2 while h, m1, m2 stream through (evict-first)
+        int largest = 1, resident = 0, gathers_fit = 0, smallest_vec = 0;
         for (int d = 1; d <= R; ++d) {
             if (R % d || !potts_block_ok(q, d)) continue;
             largest = d;
-            if (per_replica * d <= budget) resident = d;
+            if (per_replica * d <= budget && d % 4 == 0 && (double)hd->dp.n * hd->dp.F * d >= 1.0e6) resident = d;
+            if (8.0 * (double)hd->dp.n * hd->dp.F * d <= 0.85 * (double)hd->l2_bytes) gathers_fit = d;
             if (!smallest_vec && d % 2 == 0) smallest_vec = d;
         }
         if (hd->opt_replica_block > 0 && hd->opt_replica_block <= R && R % hd->opt_replica_block == 0 &&
@@ -192,7 +195,7 @@ static void configure_R(Handle *hd, int R) {
         else if (per_replica * R <= budget || hd->l2_bytes == 0)
             Rb = largest;
         else
-            Rb = resident > 1 ? resident : (smallest_vec ? smallest_vec : largest);
+            Rb = resident > 1 ? resident : (gathers_fit > 1 ? gathers_fit : (smallest_vec ? smallest_vec : largest));
     } else if (hd->opt_replica_block > 0) {
         if (hd->opt_replica_block < R && R % hd->opt_replica_block == 0) Rb = (int)hd->opt_replica_block;
     } else if (!hd->dp.J) {  // (the dense kind runs as one block: its tensor maps cover all R replicas)
