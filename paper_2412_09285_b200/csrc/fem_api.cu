@@ -18,6 +18,9 @@ void launch_sigmoid(Handle *hd, float *out);
 bool potts_block_ok(int q, int Rb);
 void launch_potts_softmax(Handle *hd, float *out);
 void launch_tc_split(Handle *hd);
+bool persist_eligible(const Handle *hd);
+void persist_prepare(Handle *hd, const int64_t *row_ptr);
+cudaError_t persist_run(Handle *hd, bool wide, int t_begin, int t_end, StepScalars (*scalars)(void *, int), void *ctx);
 
 static std::string g_create_error;
 
@@ -375,12 +378,15 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
         dp.w = s.weighted ? reinterpret_cast<float *>(at(L.w)) : nullptr;
         if (pb->kind == FEM_ISING) hd->integral_weights = false;
         hd->structure_bytes = (dp.uniform_deg > 0 ? 0 : 4 * ((int64_t)pb->n + 1)) + (s.weighted ? 8 : 4) * s.nnz;
+        if (pb->kind != FEM_BMINCUT) persist_prepare(hd, pb->row_ptr);
     }
     hd->lambda_last = pb->lambda;
     {
         int dev = 0, l2 = 0;
         if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev) == cudaSuccess)
             hd->l2_bytes = l2;
+        int sms = 0;
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0) hd->sm_count = sms;
     }
     hd->h = reinterpret_cast<float *>(at(L.h));
     hd->m1 = reinterpret_cast<float *>(at(L.m1));
@@ -448,6 +454,9 @@ fem_status fem_set_option(fem_handle *h, const char *key, int64_t value) {
         if (value != 0 && value != 32 && value != 64 && value != 128 && value != 256)
             return fail(hd, FEM_EINVAL, "tc_tile_n must be 0, 32, 64, 128 or 256");
         hd->opt_tc_tile_n = value;
+    } else if (!strcmp(key, "persistent")) {
+        if (value < 0 || value > 9) return fail(hd, FEM_EINVAL, "persistent must be 0, 1 or 1 + cluster size");
+        hd->opt_persistent = value;
     } else if (!strcmp(key, "tensor_cores")) {
         if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "tensor_cores must be 0 or 1");
         hd->opt_tensor_cores = value;
@@ -462,6 +471,8 @@ int64_t fem_get_info(const fem_handle *h, const char *key) {
     if (!hd || !key) return -1;
     if (!strcmp(key, "launches")) return hd->launches;
     if (!strcmp(key, "tc_launches")) return hd->tc_launches;
+    if (!strcmp(key, "persist_launches")) return hd->persist_launches;
+    if (!strcmp(key, "persist_cluster")) return hd->persist_cluster;
     if (!strcmp(key, "t_done")) return hd->t_done;
     if (!strcmp(key, "R")) return hd->R;
     if (!strcmp(key, "replica_block")) return hd->Rb;
@@ -592,6 +603,13 @@ fem_status fem_anneal(fem_handle *h, const fem_schedule *sch, int32_t R, uint64_
     };
     const int t0 = hd->t_done;
     int t = t0;
+    const bool persist = persist_eligible(hd);
+    auto scalars_thunk = [](void *ctx, int tt) { return (*static_cast<decltype(scalars) *>(ctx))(tt); };
+    if (persist && hd->wide_live && t < K && t < stop_after) {  // wide phase inside the replica-persistent kernel
+        const int te = std::min(stop_after, K);
+        if (!cuda_ok(hd, persist_run(hd, true, t, te, scalars_thunk, &scalars), "persistent launch")) return FEM_ECUDA;
+        t = te;
+    }
     for (; t < stop_after && hd->wide_live && t < K; ++t) {  // wide phase, step-major over all blocks
         one_step(t, 0, nb);
         hd->cur ^= 1;
@@ -601,7 +619,10 @@ fem_status fem_anneal(fem_handle *h, const fem_schedule *sch, int32_t R, uint64_
         hd->wide_live = false;
         hd->tc_ready = false;
     }
-    if (nb == 1 || hd->opt_steps_per_block == 1) {
+    if (persist && t < stop_after) {  // small sparse two-state problem: one CTA per replica, all steps in one launch
+        if (!cuda_ok(hd, persist_run(hd, false, t, stop_after, scalars_thunk, &scalars), "persistent launch")) return FEM_ECUDA;
+        t = stop_after;
+    } else if (nb == 1 || hd->opt_steps_per_block == 1) {
         for (; t < stop_after; ++t) {
             one_step(t, 0, nb);
             hd->cur ^= 1;

@@ -95,6 +95,12 @@ struct Handle {
     int t_done = 0;
     bool injected = false, readout_valid = false, gather_valid = false;
     int64_t opt_replica_block = 0, opt_steps_per_block = 0, opt_tensor_cores = 1, opt_tc_tile_n = 0;
+    // small sparse two-state problems: replica-persistent kernel (k_persist_q2.cu).  0 = off, 1 = automatic cluster
+    // size, 1 + CS = force clusters of CS CTAs per replica
+    int64_t opt_persistent = 1;
+    int64_t persist_launches = 0, persist_cluster = 0;
+    int64_t persist_ell[4] = {-1, -1, -1, -1};  // sliced-ELL entries per CTA for cluster sizes 1, 2, 4, 8
+    int sm_count = 148;
     int64_t launches = 0;
     int64_t tc_launches = 0;  // launches of the tcgen05 dense step (k_dense_tc.cu)
     int64_t l2_bytes = 0;  // device L2 size (0 when unknown: no automatic replica blocking)

@@ -258,3 +258,44 @@ def test_dense_tensor_core_path_is_taken_and_agrees_with_cuda_cores(fem):
         assert np.max(np.abs(out[tc] - P_ref.reshape(out[tc].shape))) < MARGINAL_TOL
         eng.close()
     assert np.max(np.abs(out[1] - out[0])) < MARGINAL_TOL
+
+
+def _persist_cases():
+    return {
+        "cfg0_maxcut_er800": lambda: get("cfg0_maxcut_er800"),                       # unit weights, 1 variable per thread
+        "maxcut_er_odd_R": lambda: get("maxcut_er_odd_R"),                           # +-1 weights, odd R (scalar rows)
+        "ising_sparse": lambda: get("ising_sparse"),                                 # real weights, Ising sign
+        "maxcut_er_n1500": lambda: (wl.erdos_renyi_maxcut(1500, 0.01, 2012, pm1=True), 12),   # 2 variables per thread
+        "maxcut_torus_61x50": lambda: (wl.torus_maxcut(61, 2013, W=50), 20),          # 3050 nodes: 4 variables per thread
+    }
+
+
+@pytest.mark.parametrize("name", list(_persist_cases()))
+def test_persistent_kernel_bit_identical_to_stepwise(fem, name):
+    """Small sparse two-state problems run in the replica-persistent kernel (one CTA per replica, state in
+    registers, gathers from shared memory).  Its arithmetic is the stepwise kernel's, so fields, moments and
+    energies must be bit-identical, including across a resume (stop_after) and the fp64 wide phase."""
+    inst, R = _persist_cases()[name]()
+    steps = 300                                                      # spans two parameter chunks of the fp32 kernel
+    sch = fem.Schedule(beta=fem.linear_temperature_schedule(1.0, 0.01, steps), precise_steps=8)
+    out = {}
+    for persistent in (0, 1, 2, 3, 5, 9):                             # off, automatic, clusters of 1, 2, 4, 8 CTAs per replica
+        eng = fem.Fem(inst, R)
+        eng.set_option("persistent", persistent)
+        eng.anneal(sch, R, seed=4, stop_after=5)                      # stops inside the wide phase
+        h5 = eng.get_fields()
+        eng.anneal(sch, R, seed=4, stop_after=37)
+        h37 = eng.get_fields()
+        eng.anneal(sch, R, seed=4, stop_after=steps)
+        out[persistent] = (h5, h37, eng.get_fields(), eng.get_moments(), eng.result())
+        if persistent <= 1:
+            assert (eng.info("persist_launches") > 0) == (persistent == 1)
+        elif eng.info("persist_launches") > 0:                        # a forced size that does not fit falls back to stepwise
+            assert eng.info("persist_cluster") == persistent - 1
+        eng.close()
+    b = out[0]
+    for persistent, a in out.items():
+        for k in range(3):
+            assert np.array_equal(a[k], b[k]), (persistent, k)
+        assert np.array_equal(a[3][0], b[3][0]) and np.array_equal(a[3][1], b[3][1])
+        assert np.array_equal(a[4]["energy"], b[4]["energy"]) and a[4]["best_replica"] == b[4]["best_replica"]
