@@ -87,28 +87,42 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
         const R f = R::ld_stream(p.field + off);
 #pragma unroll
         for (int v = 0; v < VEC; ++v) dU[v] = (T)-2 * f.v[v];
-    } else {  // MODE_SAT: dU/dp_i = sum_{m ni i} s_mi prod_{k != i} u_mk
+    } else {  // MODE_SAT: dU/dp_i = sum_{m ni i} s_mi prod_{k != i} u_mk; DEG = entries per occurrence (k_max - 1)
+        constexpr int KS = DEG > 0 ? DEG : 1;
+        constexpr int B = KS == 1 ? 8 : (KS == 2 ? 4 : (KS == 3 ? 4 : 2));  // occurrences in flight per thread
         const int o0 = __ldg(p.dp.occ_ptr + i), o1 = __ldg(p.dp.occ_ptr + i + 1);
-        const int ks = p.dp.kstride;
-        for (int o = o0; o < o1; ++o) {
-            const int *__restrict__ ent = p.dp.occ + (unsigned)o * (unsigned)ks;
-            T prod[VEC];
+        const unsigned pad = ((unsigned)p.dp.n << 1) | 1u;  // the constant-1 row, "negated": factor 0.5 + 0.5*1 = 1
+        for (int o = o0; o < o1; o += B) {
+            unsigned pk[B][KS];
 #pragma unroll
-            for (int v = 0; v < VEC; ++v) prod[v] = (T)1;
-            int first = 0;
-            for (int x = 0; x < ks; ++x) {
-                int pk = __ldg(ent + x);
-                if (x == 0) first = pk;
-                pk &= 0x7fffffff;
-                const R mr = R::ld(gin + (unsigned)(pk >> 1) * Rb);
-                // probability the literal is false: 1-p = (1-m)/2 (positive literal), p = (1+m)/2 (negated)
-                const T sg = (pk & 1) ? (T)0.5 : (T)-0.5;
+            for (int b = 0; b < B; ++b) {
+                const int *__restrict__ ent = p.dp.occ + (unsigned)(o + b) * (unsigned)KS;
 #pragma unroll
-                for (int v = 0; v < VEC; ++v) prod[v] *= (T)0.5 + sg * mr.v[v];
+                for (int x = 0; x < KS; ++x) pk[b][x] = (o + b < o1) ? (unsigned)__ldg(ent + x) : pad;
             }
-            const bool positive = first < 0;  // bit 31
+            R mr[B][KS];
 #pragma unroll
-            for (int v = 0; v < VEC; ++v) dU[v] += positive ? -prod[v] : prod[v];
+            for (int b = 0; b < B; ++b)
+#pragma unroll
+                for (int x = 0; x < KS; ++x) mr[b][x] = R::ld(gin + ((pk[b][x] & 0x7fffffffu) >> 1) * Rb);
+#pragma unroll
+            for (int b = 0; b < B; ++b) {
+                T prod[VEC];
+#pragma unroll
+                for (int v = 0; v < VEC; ++v) prod[v] = (T)1;
+#pragma unroll
+                for (int x = 0; x < KS; ++x) {
+                    // probability the literal is false: 1-p = (1-m)/2 (positive literal), p = (1+m)/2 (negated)
+                    const T sg = (pk[b][x] & 1u) ? (T)0.5 : (T)-0.5;
+#pragma unroll
+                    for (int v = 0; v < VEC; ++v) prod[v] *= (T)0.5 + sg * mr[b][x].v[v];
+                }
+                const bool positive = (pk[b][0] >> 31) != 0u;  // bit 31 of entry 0: own literal is positive
+                if (o + b < o1) {
+#pragma unroll
+                    for (int v = 0; v < VEC; ++v) dU[v] += positive ? -prod[v] : prod[v];
+                }
+            }
         }
     }
 
@@ -191,13 +205,25 @@ __global__ void __launch_bounds__(256) dense_field_kernel(const float *__restric
 
 template <typename T, int VEC, int MODE>
 static void launch_q2_deg(Handle *hd, const Q2Params<T> &p, dim3 grid) {
-    const int d = (MODE == MODE_MAXCUT || MODE == MODE_ISING) ? hd->dp.uniform_deg : 0;
-    if (d == 3)
-        launch_pdl(step_q2_kernel<T, VEC, MODE, 3>, grid, dim3(kThreads), hd->stream, p);
-    else if (d == 4)
-        launch_pdl(step_q2_kernel<T, VEC, MODE, 4>, grid, dim3(kThreads), hd->stream, p);
-    else
-        launch_pdl(step_q2_kernel<T, VEC, MODE, 0>, grid, dim3(kThreads), hd->stream, p);
+    if constexpr (MODE == MODE_SAT) {
+        switch (hd->dp.kstride) {
+            case 1: launch_pdl(step_q2_kernel<T, VEC, MODE, 1>, grid, dim3(kThreads), hd->stream, p); break;
+            case 2: launch_pdl(step_q2_kernel<T, VEC, MODE, 2>, grid, dim3(kThreads), hd->stream, p); break;
+            case 3: launch_pdl(step_q2_kernel<T, VEC, MODE, 3>, grid, dim3(kThreads), hd->stream, p); break;
+            case 4: launch_pdl(step_q2_kernel<T, VEC, MODE, 4>, grid, dim3(kThreads), hd->stream, p); break;
+            case 5: launch_pdl(step_q2_kernel<T, VEC, MODE, 5>, grid, dim3(kThreads), hd->stream, p); break;
+            case 6: launch_pdl(step_q2_kernel<T, VEC, MODE, 6>, grid, dim3(kThreads), hd->stream, p); break;
+            default: launch_pdl(step_q2_kernel<T, VEC, MODE, 7>, grid, dim3(kThreads), hd->stream, p); break;
+        }
+    } else {
+        const int d = (MODE == MODE_MAXCUT || MODE == MODE_ISING) ? hd->dp.uniform_deg : 0;
+        if (d == 3)
+            launch_pdl(step_q2_kernel<T, VEC, MODE, 3>, grid, dim3(kThreads), hd->stream, p);
+        else if (d == 4)
+            launch_pdl(step_q2_kernel<T, VEC, MODE, 4>, grid, dim3(kThreads), hd->stream, p);
+        else
+            launch_pdl(step_q2_kernel<T, VEC, MODE, 0>, grid, dim3(kThreads), hd->stream, p);
+    }
 }
 
 template <typename T, int VEC>
