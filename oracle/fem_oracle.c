@@ -33,6 +33,10 @@
  *   femo_schedule_*                : endpoints, 1/linspace
  *   femo_energy                    : brute-force enumeration, saturation U_MF == E
  *   femo_anneal                    : brute-force optima on n<=20
+ *   femo_rmsprop / femo_sgd        : torch.optim.RMSprop / torch.optim.SGD (float64, CPU)
+ *   femo_grad_h_manipulated        : the general-q S25 + S20 form written out in numpy (S29/S30 are its
+ *                                    two-state reduction); saturated fields reduce it to the exact
+ *                                    gradient on row-normalised weights; sum_s g^h_i(s) = 0; brute-force optima
  *   femo_init_fields               : moments / reproducibility only (a generator, not a
  *                                    formula of the paper)
  *   Solution quality against the paper's tables (G-set, K2000, Walshaw, MaxSAT-2016):
@@ -309,6 +313,129 @@ void femo_adam(const femo_adam_cfg *cfg, int32_t t, int64_t count, double *h, do
 }
 
 /* ------------------------------------------------------------------------------------------
+ * Manipulated gradients: what the paper benchmarks with.
+ * The marginals of the NEIGHBOURS are replaced by their one-hot vectors e_j ("discretization",
+ * PAPER.md:626), the coupling term is normalised per node, and gamma_grad scales the result.
+ *
+ * Two-state graph kinds, S29/S30:
+ *     g^h_i = gamma [ c_i sum_j W_ij sgn(m_j) + h_i/beta ] p_i (1 - p_i),   c_i = 1 / sum_j |W_ij|
+ *   (S30 writes gamma/4 (1 - m_i^2); p(1-p) = (1 - m^2)/4.)  sgn(m_j) = sgn(h_j), sgn(0) = 0.
+ *   Ising: the same with dU/dp_i = -2 sum_j J_ij m_j (see femo_grad_h), i.e. W_ij -> -2 J_ij, and
+ *   c_i = 1 / sum_j |2 J_ij| so that the normalised coupling term stays within [-1, 1] as PAPER.md:630 states.
+ * Potts kind, S27 taken literally (coefficient lambda, not 2 lambda, on the balance term):
+ *     ghat^p_i(s) = -c^f_i sum_j W_ij e_j(s) + lambda c^a_i [ sum_j e_j(s) - e_i(s) ] + (1/beta)[ln P_i(s) + 1]
+ *     c^f_i = q / sum_j W_ij,  c^a_i = q / sqrt(sum_j W_ij)
+ *   then S20:  g^h_i(s) = gamma P_i(s) [ ghat^p_i(s) - sum_s' P_i(s') ghat^p_i(s') ].
+ *   e_j = one-hot of argmax_s h_j(s), ties -> lowest state (the rounding rule R3).
+ * Max-SAT: the paper makes no modification: exact gradient times gamma.
+ * Nodes without neighbours have no coupling term; their c is taken as 0 (reading R13).
+ * ---------------------------------------------------------------------------------------- */
+void femo_grad_h_manipulated(const femo_problem *pb, const double *h, double beta, double lambda, double gamma,
+                             double *g) {
+    int n = pb->n;
+    if (pb->kind == FEMO_MAXSAT || (pb->kind == FEMO_ISING && pb->dense_J)) {
+        femo_grad_h(pb, h, beta, lambda, g);
+        for (int i = 0; i < n; ++i) g[i] *= gamma;
+        return;
+    }
+    if (pb->kind == FEMO_BMINCUT) {
+        int q = pb->q;
+        double *P = (double *)malloc(sizeof(double) * (size_t)n * q);
+        int *hot = (int *)malloc(sizeof(int) * (size_t)n);
+        double *cnt = (double *)calloc((size_t)q, sizeof(double));
+        double *gp = (double *)malloc(sizeof(double) * (size_t)q);
+        femo_marginals(pb, h, P);
+        for (int i = 0; i < n; ++i) {
+            int best = 0;
+            for (int s = 1; s < q; ++s)
+                if (h[(size_t)i * q + s] > h[(size_t)i * q + best]) best = s;
+            hot[i] = best;
+            cnt[best] += 1.0;
+        }
+        for (int i = 0; i < n; ++i) {
+            const double *hi = h + (size_t)i * q;
+            const double *Pi = P + (size_t)i * q;
+            double lse = logsumexp(hi, q);
+            double rowsum = 0.0;
+            for (int64_t e = pb->row_ptr[i]; e < pb->row_ptr[i + 1]; ++e) rowsum += wgt(pb, e);
+            double cf = rowsum > 0.0 ? (double)q / rowsum : 0.0;
+            double ca = rowsum > 0.0 ? (double)q / sqrt(rowsum) : 0.0;
+            for (int s = 0; s < q; ++s) {
+                double f = 0.0;
+                for (int64_t e = pb->row_ptr[i]; e < pb->row_ptr[i + 1]; ++e)
+                    if (hot[pb->col_idx[e]] == s) f += wgt(pb, e);
+                double ei = (hot[i] == s) ? 1.0 : 0.0;
+                gp[s] = -cf * f + lambda * ca * (cnt[s] - ei) + (hi[s] - lse + 1.0) / beta;
+            }
+            double gbar = 0.0;
+            for (int s = 0; s < q; ++s) gbar += Pi[s] * gp[s];
+            for (int s = 0; s < q; ++s) g[(size_t)i * q + s] = gamma * Pi[s] * (gp[s] - gbar);
+        }
+        free(P);
+        free(hot);
+        free(cnt);
+        free(gp);
+        return;
+    }
+    /* MaxCut / sparse Ising */
+    double scale = (pb->kind == FEMO_MAXCUT) ? 1.0 : -2.0;
+    for (int i = 0; i < n; ++i) {
+        double f = 0.0, l1 = 0.0;
+        for (int64_t e = pb->row_ptr[i]; e < pb->row_ptr[i + 1]; ++e) {
+            double hj = h[pb->col_idx[e]];
+            double sg = (hj > 0.0) ? 1.0 : (hj < 0.0 ? -1.0 : 0.0);
+            f += scale * wgt(pb, e) * sg;
+            l1 += fabs(scale * wgt(pb, e));
+        }
+        double c = l1 > 0.0 ? 1.0 / l1 : 0.0;
+        g[i] = gamma * (c * f + h[i] / beta) * sigmoid(h[i]) * sigmoid(-h[i]);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * RMSprop and SGD with momentum ("the Python
+ * implementations of these optimizers as provided by PyTorch", tuned: lr, weight decay, momentum,
+ * dampening (SGD); lr, weight decay, momentum, alpha (RMSprop); everything else PyTorch's default:
+ * RMSprop eps = 1e-8 added OUTSIDE the square root, not centered; SGD without Nesterov).
+ *   RMSprop:  g <- g + wd h;  v <- alpha v + (1-alpha) g^2;  d = g / (sqrt(v) + eps);
+ *             momentum > 0:  b <- momentum b + d;  h <- h - lr b      else  h <- h - lr d
+ *   SGD:      g <- g + wd h;  momentum > 0:  b <- g at the first step, b <- momentum b + (1-dampening) g after;
+ *             h <- h - lr b   (momentum = 0: h <- h - lr g)
+ * m1 holds the momentum buffer b, m2 the running square average v.  t is the 1-based step count.
+ * ---------------------------------------------------------------------------------------- */
+typedef struct {
+    int32_t kind; /* 0 Adam, 1 RMSprop, 2 SGD */
+    double lr, beta1, beta2, eps, weight_decay; /* Adam: beta1, beta2 */
+    double alpha, momentum, dampening;          /* RMSprop: alpha, momentum; SGD: momentum, dampening */
+} femo_opt_cfg;
+
+void femo_rmsprop(const femo_opt_cfg *cfg, int64_t count, double *h, double *m1, double *m2, const double *g) {
+    for (int64_t k = 0; k < count; ++k) {
+        double gk = g[k] + cfg->weight_decay * h[k];
+        m2[k] = cfg->alpha * m2[k] + (1.0 - cfg->alpha) * gk * gk;
+        double d = gk / (sqrt(m2[k]) + cfg->eps);
+        if (cfg->momentum > 0.0) {
+            m1[k] = cfg->momentum * m1[k] + d;
+            h[k] -= cfg->lr * m1[k];
+        } else {
+            h[k] -= cfg->lr * d;
+        }
+    }
+}
+
+void femo_sgd(const femo_opt_cfg *cfg, int32_t t, int64_t count, double *h, double *m1, const double *g) {
+    for (int64_t k = 0; k < count; ++k) {
+        double gk = g[k] + cfg->weight_decay * h[k];
+        if (cfg->momentum > 0.0) {
+            m1[k] = (t == 1) ? gk : cfg->momentum * m1[k] + (1.0 - cfg->dampening) * gk;
+            h[k] -= cfg->lr * m1[k];
+        } else {
+            h[k] -= cfg->lr * gk;
+        }
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
  * Annealing schedules, t = 0..N-1.
  *   inverse-proportional: T(t) = T_max + (T_min - T_max) t/(N-1), beta = 1/T
  *   exponential         : beta(t) = exp( (ln bmax - ln bmin) t/(N-1) + ln bmin )
@@ -382,6 +509,37 @@ void femo_anneal(const femo_problem *pb, int32_t R, double *h, double *m1, doubl
                  const double *lambda_t, double lambda, int32_t t_begin, int32_t t_end, const femo_adam_cfg *adam) {
     for (int t = t_begin; t < t_end; ++t)
         femo_step(pb, R, h, m1, m2, t, beta[t], lambda_t ? lambda_t[t] : lambda, adam);
+}
+
+/* The same synchronous step with the section 8(f) choices: optimiser kind and exact (manipulated = 0) or
+ * manipulated gradients (manipulated = 1, with gamma_grad).  manipulated = 0 ignores gamma (exact gradient). */
+void femo_step_ex(const femo_problem *pb, int32_t R, double *h, double *m1, double *m2, int32_t t, double beta,
+                  double lambda, const femo_opt_cfg *opt, int32_t manipulated, double gamma) {
+    int64_t per = (int64_t)pb->n * femo_fields_per_var(pb);
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+    for (int a = 0; a < R; ++a) {
+        double *g = (double *)malloc(sizeof(double) * (size_t)per);
+        if (manipulated) femo_grad_h_manipulated(pb, h + a * per, beta, lambda, gamma, g);
+        else femo_grad_h(pb, h + a * per, beta, lambda, g);
+        if (opt->kind == 0) {
+            femo_adam_cfg ac = {opt->lr, opt->beta1, opt->beta2, opt->eps, opt->weight_decay};
+            femo_adam(&ac, t + 1, per, h + a * per, m1 + a * per, m2 + a * per, g);
+        } else if (opt->kind == 1) {
+            femo_rmsprop(opt, per, h + a * per, m1 + a * per, m2 + a * per, g);
+        } else {
+            femo_sgd(opt, t + 1, per, h + a * per, m1 + a * per, g);
+        }
+        free(g);
+    }
+}
+
+void femo_anneal_ex(const femo_problem *pb, int32_t R, double *h, double *m1, double *m2, const double *beta,
+                    const double *lambda_t, double lambda, int32_t t_begin, int32_t t_end, const femo_opt_cfg *opt,
+                    int32_t manipulated, double gamma) {
+    for (int t = t_begin; t < t_end; ++t)
+        femo_step_ex(pb, R, h, m1, m2, t, beta[t], lambda_t ? lambda_t[t] : lambda, opt, manipulated, gamma);
 }
 
 /* ------------------------------------------------------------------------------------------

@@ -49,6 +49,14 @@ class _Adam(C.Structure):
                 ("eps", C.c_double), ("weight_decay", C.c_double)]
 
 
+class _Opt(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("lr", C.c_double), ("beta1", C.c_double), ("beta2", C.c_double),
+                ("eps", C.c_double), ("weight_decay", C.c_double), ("alpha", C.c_double), ("momentum", C.c_double),
+                ("dampening", C.c_double)]
+
+
+ADAM, RMSPROP, SGD = 0, 1, 2
+
 _libs: dict = {}
 
 
@@ -114,6 +122,24 @@ class Adam:
         return _Adam(self.lr, self.beta1, self.beta2, self.eps, self.weight_decay)
 
 
+@dataclass
+class Optimizer:
+    """Optimiser choice of SURVEY.md section 8(f) item 2 (PyTorch defaults for what the paper does not tune)."""
+    kind: int = ADAM
+    lr: float = 0.1
+    beta1: float = 0.9
+    beta2: float = 0.999
+    eps: float = 1e-8
+    weight_decay: float = 0.0
+    alpha: float = 0.99
+    momentum: float = 0.0
+    dampening: float = 0.0
+
+    def c(self) -> _Opt:
+        return _Opt(self.kind, self.lr, self.beta1, self.beta2, self.eps, self.weight_decay, self.alpha,
+                    self.momentum, self.dampening)
+
+
 def _f64(a) -> np.ndarray:
     return np.ascontiguousarray(a, dtype=np.float64)
 
@@ -155,6 +181,26 @@ def grad_h(pb: Problem, h: np.ndarray, beta: float, lam: float = 0.0) -> np.ndar
     cp = pb.c()
     _lib().femo_grad_h(C.byref(cp), _p(h), C.c_double(beta), C.c_double(lam), _p(g))
     return g
+
+
+def grad_h_manipulated(pb: Problem, h: np.ndarray, beta: float, lam: float = 0.0, gamma: float = 1.0) -> np.ndarray:
+    """One replica: manipulated gradient (S25/S27/S29/S30 with S20), h[n*F] -> g^h[n*F]."""
+    h = _f64(h)
+    g = np.empty_like(h)
+    cp = pb.c()
+    _lib().femo_grad_h_manipulated(C.byref(cp), _p(h), C.c_double(beta), C.c_double(lam), C.c_double(gamma), _p(g))
+    return g
+
+
+def rmsprop_update(opt: Optimizer, h: np.ndarray, m1: np.ndarray, m2: np.ndarray, g: np.ndarray) -> None:
+    co = opt.c()
+    _lib().femo_rmsprop(C.byref(co), C.c_int64(h.size), _p(h), _p(m1), _p(m2), _p(_f64(g)))
+
+
+def sgd_update(opt: Optimizer, t: int, h: np.ndarray, m1: np.ndarray, g: np.ndarray) -> None:
+    """t is the 1-based step count (the momentum buffer is initialised with the first gradient)."""
+    co = opt.c()
+    _lib().femo_sgd(C.byref(co), C.c_int32(t), C.c_int64(h.size), _p(h), _p(m1), _p(_f64(g)))
 
 
 def adam_update(adam: Adam, t: int, h: np.ndarray, m1: np.ndarray, m2: np.ndarray, g: np.ndarray) -> None:
@@ -202,6 +248,20 @@ def anneal(st: State, beta: np.ndarray, adam: Adam, lam: float = 0.0, lam_t: Opt
     cp, ca = st.pb.c(), adam.c()
     _lib(openmp).femo_anneal(C.byref(cp), C.c_int32(st.R), _p(st.h), _p(st.m1), _p(st.m2), _p(beta), _p(lam_t),
                              C.c_double(lam), C.c_int32(st.t), C.c_int32(t_end), C.byref(ca))
+    st.t = t_end
+    return st
+
+
+def anneal_ex(st: State, beta: np.ndarray, opt: Optimizer, lam: float = 0.0, lam_t: Optional[np.ndarray] = None,
+              t_end: Optional[int] = None, manipulated: bool = False, gamma: float = 1.0, openmp: bool = False) -> State:
+    """anneal() with the optimiser / gradient choices of SURVEY.md section 8(f)."""
+    beta = _f64(beta)
+    t_end = len(beta) if t_end is None else t_end
+    lam_t = None if lam_t is None else _f64(lam_t)
+    cp, co = st.pb.c(), opt.c()
+    _lib(openmp).femo_anneal_ex(C.byref(cp), C.c_int32(st.R), _p(st.h), _p(st.m1), _p(st.m2), _p(beta), _p(lam_t),
+                                C.c_double(lam), C.c_int32(st.t), C.c_int32(t_end), C.byref(co),
+                                C.c_int32(1 if manipulated else 0), C.c_double(gamma))
     st.t = t_end
     return st
 
