@@ -177,6 +177,10 @@ def main():
     ap.add_argument("--precise-steps", type=int, default=8)
     ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
                     help="library option passed to fem_set_option (e.g. tensor_cores=0); repeatable")
+    ap.add_argument("--optimizer", default="adam", choices=["adam", "rmsprop", "sgd"],
+                    help="SURVEY 8(f): adam is the BASELINE.json configuration; rmsprop (lr 0.05, alpha 0.9, momentum 0.5) and "
+                         "sgd (lr 0.5, momentum 0.8) are variants, named in config")
+    ap.add_argument("--manipulated", action="store_true", help="SURVEY 8(f): manipulated gradients S25/S27/S30 (variant)")
     ap.add_argument("--anneal-steps", type=int, default=None,
                     help="shorten the schedule (profiling under ncu only; such a run is not a bench value)")
     args = ap.parse_args()
@@ -213,6 +217,14 @@ def main():
     R, N, n = cfg.R, cfg.steps, inst.n
     sched = fem.schedule_for(cfg, precise_steps=args.precise_steps)
     K = min(args.precise_steps, N)
+    variant = None
+    if args.optimizer != "adam" or args.manipulated:
+        if args.optimizer == "rmsprop":
+            sched.optimizer, sched.lr, sched.alpha, sched.momentum = fem.RMSPROP, 0.05, 0.9, 0.5
+        elif args.optimizer == "sgd":
+            sched.optimizer, sched.lr, sched.momentum = fem.SGD, 0.5, 0.8
+        sched.manipulated = args.manipulated
+        variant = f"{args.optimizer}{'+manipulated gradients' if args.manipulated else ''} (not the BASELINE.json configuration)"
 
     def apply_options(eng):
         if args.replica_block is not None:
@@ -359,7 +371,8 @@ def main():
             "config": {"workload": cfg.name, "instance": inst.name, "n": n, "R_per_gpu": R, "anneal_steps": N,
                        "precise_steps": K, "replica_block": eng.info("replica_block"),
                        "l2": "256 MiB buffer written between timed passes (L2 flush)",
-                       "parallelism": f"replicas x{world}" if world > 1 else "single GPU"},
+                       "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+                       **({"variant": variant} if variant else {})},
             "roofline": roofline,
             "e2e": {"value": updates * e2e_steps * world / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "steps": e2e_steps},

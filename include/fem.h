@@ -83,7 +83,22 @@ typedef struct {
     double init_scale;     /* h(0) = init_scale * N(0,1); used when fields were not injected */
     int32_t precise_steps; /* wide phase: the first K steps keep state AND arithmetic in fp64, then the state is
                             * rounded to fp32 once and the rest of the anneal is fp32 */
+    /* ---- ABI version 2: the optimisers and gradient manipulations the paper benchmarks with ---- */
+    int32_t optimizer;     /* fem_optimizer; FEM_ADAM uses lr, beta1, beta2, eps, weight_decay above.
+                            * FEM_RMSPROP (torch.optim.RMSprop, not centered): lr, alpha, eps, weight_decay, momentum.
+                            * FEM_SGD (torch.optim.SGD, no Nesterov): lr, momentum, dampening, weight_decay */
+    double alpha;          /* RMSprop smoothing constant, in [0, 1) */
+    double momentum;       /* RMSprop / SGD momentum, >= 0 */
+    double dampening;      /* SGD dampening, in [0, 1] */
+    int32_t manipulated;   /* 0: exact gradient of F_MF (gamma_grad ignored).  1: manipulated gradients:
+                            * MAXCUT / sparse ISING S29-S30: neighbours enter as sgn(m_j), coupling term times
+                            * c_i = 1 / sum_j |W_ij| (Ising: |2 J_ij|); BMINCUT S27: one-hot neighbours e_j, c^f_i =
+                            * q / sum_j W_ij on the cut term and lambda * c^a_i, c^a_i = q / sqrt(sum_j W_ij), on the balance
+                            * term; MAXSAT and dense ISING: no modification; all kinds: g^h times gamma_grad (S20) */
+    double gamma_grad;     /* > 0; used when manipulated = 1 */
 } fem_schedule;
+
+typedef enum { FEM_ADAM = 0, FEM_RMSPROP = 1, FEM_SGD = 2 } fem_optimizer;
 
 /* Bytes of device workspace fem_create needs for this problem with up to R_cap replicas
  * (0 on invalid arguments).  Pure host arithmetic. */

@@ -106,13 +106,24 @@ inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, c
 }
 
 // ---- per-step scalars in the compute type (narrowed once on the host, not per thread) ----
+// opt = 0 Adam: b1, b2, omb1 = 1-b1, omb2 = 1-b2, step_size = lr/(1-b1^t), rsqrt_bc2 = 1/sqrt(1-b2^t)
+// opt = 1 RMSprop: b1 = momentum, b2 = alpha, omb2 = 1-alpha, step_size = lr
+// opt = 2 SGD: b1 = momentum, omb1 = 1-dampening, step_size = lr, first = 1 at the first step of the anneal
 template <typename T>
 struct Sc {
     T inv_beta, step_size, rsqrt_bc2, eps, b1, b2, omb1, omb2, wd, two_lambda;
+    T gamma;    // gamma_grad of S20; 1 for the exact gradient
+    int opt;    // 0 Adam, 1 RMSprop, 2 SGD
+    int first;  // SGD: the momentum buffer starts as the first gradient
+    int disc;   // manipulated gradients (S25/S27/S30): neighbours enter as one-hot vectors, coupling term normalised
     Sc() = default;
     __host__ explicit Sc(const StepScalars &s)
         : inv_beta((T)s.inv_beta), step_size((T)s.step_size), rsqrt_bc2((T)s.rsqrt_bc2), eps((T)s.eps), b1((T)s.b1),
-          b2((T)s.b2), omb1((T)s.one_minus_b1), omb2((T)s.one_minus_b2), wd((T)s.wd), two_lambda((T)s.two_lambda) {}
+          b2((T)s.b2), omb1((T)s.one_minus_b1), omb2((T)s.one_minus_b2), wd((T)s.wd), two_lambda((T)s.two_lambda),
+          gamma((T)s.gamma), opt(s.opt), first(s.first), disc(s.disc) {}
+    // which moment arrays the optimiser touches (the others are neither read nor written: 8 B per field each)
+    __host__ __device__ bool uses_m1() const { return opt == 0 || b1 > (T)0; }
+    __host__ __device__ bool uses_m2() const { return opt != 2; }
 };
 
 // fp64 (wide phase): accurate libm.  fp32 (bulk): hardware approximations (ex2/rcp/sqrt MUFU ops, <= 2 ulp),
@@ -169,14 +180,50 @@ __device__ __forceinline__ T sigmoid_of(T h) {
     return h < (T)0 ? e * r : r;
 }
 
-// Adam (Kingma & Ba as arranged by torch.optim.Adam): returns the new field.
+// Optimiser update (Adam, RMSprop and SGD "as provided by PyTorch"): returns the new field.
+//   Adam    : Kingma & Ba as arranged by torch.optim.Adam
+//   RMSprop : v = alpha v + (1-alpha) g^2; d = g / (sqrt(v) + eps); momentum: b = mom b + d, h -= lr b; else h -= lr d
+//   SGD     : b = g at the first step, b = mom b + (1-dampening) g after; h -= lr b   (mom = 0: h -= lr g)
+// m1 is Adam's first moment / the momentum buffer b, m2 is Adam's second moment / RMSprop's v.
+// Every multiply-add is written as an explicit fma so that all kernels (stepwise, persistent, Potts, dense) round
+// alike whatever contraction the compiler would have picked.
 template <typename T>
-__device__ __forceinline__ T adam_update(T h, T g, T &m1, T &m2, const Sc<T> &sc) {
-    g = g + sc.wd * h;
-    m1 = sc.b1 * m1 + sc.omb1 * g;
-    m2 = sc.b2 * m2 + sc.omb2 * g * g;
-    const T denom = fsqrt(m2) * sc.rsqrt_bc2 + sc.eps;
-    return h - sc.step_size * fdiv(m1, denom);
+__device__ __forceinline__ T opt_update(T h, T g, T &m1, T &m2, const Sc<T> &sc) {
+    g = fma(sc.wd, h, g);
+    if (sc.opt == 0) {
+        m1 = fma(sc.b1, m1, sc.omb1 * g);
+        m2 = fma(sc.b2, m2, (sc.omb2 * g) * g);
+        const T denom = fma(fsqrt(m2), sc.rsqrt_bc2, sc.eps);
+        return fma(-sc.step_size, fdiv(m1, denom), h);
+    }
+    if (sc.opt == 1) {
+        m2 = fma(sc.b2, m2, (sc.omb2 * g) * g);
+        const T d = fdiv(g, fsqrt(m2) + sc.eps);
+        if (sc.b1 > (T)0) {
+            m1 = fma(sc.b1, m1, d);
+            return fma(-sc.step_size, m1, h);
+        }
+        return fma(-sc.step_size, d, h);
+    }
+    if (sc.b1 > (T)0) {
+        m1 = sc.first ? g : fma(sc.b1, m1, sc.omb1 * g);
+        return fma(-sc.step_size, m1, h);
+    }
+    return fma(-sc.step_size, g, h);
+}
+
+// Two-state field gradient S29: g^h = gamma [c_i dU/dp + h/beta] p(1-p), ln(p/(1-p)) = h.  c_i = 1 and
+// gamma = 1 give the exact gradient.  The fused multiply-add is written out so that every kernel rounds alike.
+template <typename T>
+__device__ __forceinline__ T q2_grad(T dU, T ci, T h, const Sc<T> &sc) {
+    const T cd = ci * dU;
+    return sc.gamma * (fma(h, sc.inv_beta, cd) * p1mp_of(h));
+}
+
+// sgn(m) = sgn(h) with sgn(0) = 0: the two-state one-hot vector as a magnetisation, 2 e(+1) - 1 (S29)
+template <typename T>
+__device__ __forceinline__ T sign_of(T h) {
+    return h > (T)0 ? (T)1 : (h < (T)0 ? (T)-1 : (T)0);
 }
 
 }  // namespace fem

@@ -25,7 +25,7 @@ cudaError_t persist_run(Handle *hd, bool wide, int t_begin, int t_end, StepScala
 static std::string g_create_error;
 
 struct Layout {
-    size_t row_ptr, col, w, J, Jlo, glo0, glo1, field, occ_ptr, occ, clause_ptr, lits;
+    size_t row_ptr, col, w, rowsum, J, Jlo, glo0, glo1, field, occ_ptr, occ, clause_ptr, lits;
     size_t h, m1, m2, g0, g1, stage, hW, m1W, m2W, gW0, gW1, colsum0, colsum1, colsum2, cfg, e_part_i, e_part_d, part_part, e_int, e_real, part,
         best, total;
 };
@@ -88,6 +88,7 @@ static Layout make_layout(const fem_problem *pb, const ProblemShape &s, int R_ca
     L.row_ptr = take(((size_t)pb->n + 1) * 4);
     L.col = take((size_t)s.nnz * 4);
     L.w = take(s.weighted ? (size_t)s.nnz * 4 : 0);
+    L.rowsum = take(s.nnz > 0 || pb->row_ptr ? (size_t)pb->n * 8 : 0);
     L.J = take(s.dense ? (size_t)pb->n * pb->n * 4 : 0);
     L.Jlo = take(s.dense ? (size_t)pb->n * pb->n * 4 : 0);
     L.glo0 = take(s.dense ? state : 0);
@@ -224,7 +225,7 @@ using namespace fem;
 
 extern "C" {
 
-int32_t fem_abi_version(void) { return 1; }
+int32_t fem_abi_version(void) { return 2; }
 
 const char *fem_last_error(const fem_handle *h) {
     return h ? reinterpret_cast<const Handle *>(h)->err.c_str() : g_create_error.c_str();
@@ -379,6 +380,15 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
         if (pb->kind == FEM_ISING) hd->integral_weights = false;
         hd->structure_bytes = (dp.uniform_deg > 0 ? 0 : 4 * ((int64_t)pb->n + 1)) + (s.weighted ? 8 : 4) * s.nnz;
         if (pb->kind != FEM_BMINCUT) persist_prepare(hd, pb->row_ptr);
+        {   // sum_j |W_ij| per node, in double in CSR order (the normalisation factors of the manipulated gradients)
+            std::vector<double> rs((size_t)pb->n, 0.0);
+            for (int i = 0; i < pb->n; ++i)
+                for (int64_t e = pb->row_ptr[i]; e < pb->row_ptr[i + 1]; ++e)
+                    rs[i] += std::fabs(pb->weight ? (double)pb->weight[e] : 1.0);
+            up(at(L.rowsum), rs.data(), rs.size() * 8, "upload rowsum");
+            hd->rowsum = reinterpret_cast<double *>(at(L.rowsum));
+            if (ok) ok = cuda_ok(hd, cudaStreamSynchronize(hd->stream), "upload rowsum");  // rs is a local
+        }
     }
     hd->lambda_last = pb->lambda;
     {
@@ -559,8 +569,17 @@ fem_status fem_anneal(fem_handle *h, const fem_schedule *sch, int32_t R, uint64_
     if (sch->steps < 0 || (sch->steps > 0 && !sch->beta)) return fail(hd, FEM_EINVAL, "schedule needs beta[steps]");
     if (stop_after < hd->t_done || stop_after > sch->steps) return fail(hd, FEM_EINVAL, "stop_after must be in [t_done, steps]");
     if ((hd->t_done > 0 || hd->injected) && R != hd->R) return fail(hd, FEM_EINVAL, "R differs from the replicas already in flight");
-    if (!(sch->lr > 0) || !(sch->beta1 >= 0 && sch->beta1 < 1) || !(sch->beta2 >= 0 && sch->beta2 < 1) || !(sch->eps >= 0))
+    if (sch->optimizer < FEM_ADAM || sch->optimizer > FEM_SGD) return fail(hd, FEM_EINVAL, "unknown optimizer");
+    if (!(sch->lr > 0) || !(sch->eps >= 0) || !std::isfinite(sch->weight_decay)) return fail(hd, FEM_EINVAL, "bad lr / eps / weight_decay");
+    if (sch->optimizer == FEM_ADAM && (!(sch->beta1 >= 0 && sch->beta1 < 1) || !(sch->beta2 >= 0 && sch->beta2 < 1)))
         return fail(hd, FEM_EINVAL, "bad Adam parameters");
+    if (sch->optimizer == FEM_RMSPROP && (!(sch->alpha >= 0 && sch->alpha < 1) || !(sch->momentum >= 0)))
+        return fail(hd, FEM_EINVAL, "bad RMSprop parameters");
+    if (sch->optimizer == FEM_SGD && (!(sch->momentum >= 0) || !(sch->dampening >= 0 && sch->dampening <= 1)))
+        return fail(hd, FEM_EINVAL, "bad SGD parameters");
+    if (sch->manipulated != 0 && sch->manipulated != 1) return fail(hd, FEM_EINVAL, "manipulated must be 0 or 1");
+    if (sch->manipulated && (!(sch->gamma_grad > 0) || !std::isfinite(sch->gamma_grad)))
+        return fail(hd, FEM_EINVAL, "gamma_grad must be finite and > 0");
     for (int t = hd->t_done; t < stop_after; ++t)
         if (!(sch->beta[t] > 0) || !std::isfinite(sch->beta[t])) return fail(hd, FEM_EINVAL, "beta[t] must be finite and > 0");
 
@@ -580,23 +599,41 @@ fem_status fem_anneal(fem_handle *h, const fem_schedule *sch, int32_t R, uint64_
         hd->gather_valid = false;
         hd->tc_ready = false;
     }
-    ensure_gather(hd);
     const int nb = hd->R / hd->Rb;
+    // one-hot neighbours only where the paper manipulates the gradient (graph kinds with a CSR)
+    const bool disc = sch->manipulated && hd->rowsum != nullptr;
+    if (hd->gather_valid && hd->gather_disc != disc) hd->gather_valid = false;
+    hd->gather_disc = disc;
+    hd->plain_adam = sch->optimizer == FEM_ADAM && !sch->manipulated;
     auto scalars = [&](int t) {
         StepScalars sc;
         sc.inv_beta = 1.0 / sch->beta[t];
-        sc.step_size = sch->lr / (1.0 - std::pow(sch->beta1, (double)(t + 1)));
-        sc.rsqrt_bc2 = 1.0 / std::sqrt(1.0 - std::pow(sch->beta2, (double)(t + 1)));
         sc.eps = sch->eps;
-        sc.b1 = sch->beta1;
-        sc.b2 = sch->beta2;
-        sc.one_minus_b1 = 1.0 - sch->beta1;
-        sc.one_minus_b2 = 1.0 - sch->beta2;
         sc.wd = sch->weight_decay;
+        sc.opt = sch->optimizer;
+        sc.first = t == 0;
+        sc.disc = disc;
+        sc.gamma = sch->manipulated ? sch->gamma_grad : 1.0;
+        if (sch->optimizer == FEM_ADAM) {
+            sc.step_size = sch->lr / (1.0 - std::pow(sch->beta1, (double)(t + 1)));
+            sc.rsqrt_bc2 = 1.0 / std::sqrt(1.0 - std::pow(sch->beta2, (double)(t + 1)));
+            sc.b1 = sch->beta1;
+            sc.b2 = sch->beta2;
+            sc.one_minus_b1 = 1.0 - sch->beta1;
+            sc.one_minus_b2 = 1.0 - sch->beta2;
+        } else {
+            sc.step_size = sch->lr;
+            sc.rsqrt_bc2 = 1.0;
+            sc.b1 = sch->momentum;
+            sc.b2 = sch->optimizer == FEM_RMSPROP ? sch->alpha : 0.0;
+            sc.one_minus_b1 = 1.0 - sch->dampening;
+            sc.one_minus_b2 = 1.0 - sc.b2;
+        }
         sc.two_lambda = 2.0 * (sch->lambda ? sch->lambda[t] : hd->pb.lambda);
         sc.t = t;
         return sc;
     };
+    ensure_gather(hd);
     auto one_step = [&](int t, int b0, int bc) {
         if (hd->dp.kind == FEM_BMINCUT) launch_potts(hd, scalars(t), hd->wide_live, true, b0, bc);
         else launch_step_q2(hd, scalars(t), hd->wide_live, b0, bc);

@@ -29,6 +29,8 @@ struct StepScalars {
     double rsqrt_bc2;  // 1 / sqrt(1 - beta2^(t+1))
     double eps, b1, b2, one_minus_b1, one_minus_b2, wd;
     double two_lambda;  // Potts balance term 2*lambda_t
+    double gamma;       // gamma_grad (S20); 1 for the exact gradient
+    int opt, first, disc;  // optimiser kind, SGD first-step flag, manipulated gradients (see Sc<T>)
     int t;              // step number (the Potts column-sum buffers rotate with it)
 };
 
@@ -81,6 +83,9 @@ struct Handle {
     alignas(64) unsigned char tc_maps[6 * 128];  // CUtensorMap x6: J, Jlo, GT[0], GTlo[0], GT[1], GTlo[1]
     int tc_maps_R = -1;
     bool tc_ready = false;                   // g[cur]/glo[cur] hold GT / GT_lo of the current fields
+    double *rowsum = nullptr;  // graph kinds: sum_j |W_ij| per node (manipulated gradients: c_i, c^f_i, c^a_i)
+    bool plain_adam = true;    // Adam on the exact gradient: the only update the tcgen05 dense step implements
+    bool gather_disc = false;  // the gather buffers hold one-hot values (manipulated gradients), not marginals
     long long *colsum[3] = {nullptr, nullptr, nullptr};  // Potts column sums S[q][R] in fixed point, rotating
     double colsum_scale = 1.0;                            // fixed-point scale (a power of two)
     int8_t *cfg = nullptr;                   // [rows*R_cap]

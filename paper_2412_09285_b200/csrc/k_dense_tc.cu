@@ -234,7 +234,7 @@ dense_tc_step_kernel(const __grid_constant__ CUtensorMap tmJ, const __grid_const
                 for (int k = 0; k < 16; ++k) {
                     const float hk = hv[k];
                     const float g = (-2.0f * f[k] + hk * sc.inv_beta) * p1mp_of(hk);  // dU/dp = -2 sum_j J_ij m_j
-                    hv[k] = adam_update(hk, g, a1[k], a2[k], sc);
+                    hv[k] = opt_update(hk, g, a1[k], a2[k], sc);
                     const float mg = mag_of(hv[k]);
                     const size_t go = (size_t)(n0 + c0 + k) * p.n + i;  // GT[a][i]: lanes = consecutive i
                     p.gt_out[go] = mg;

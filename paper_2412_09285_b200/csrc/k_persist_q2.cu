@@ -41,7 +41,10 @@ struct PersistParams {
     int nsteps;
     int chunk;           // variables per CTA of the cluster (multiple of 32)
     int ell_cap;         // sliced-ELL entries reserved per CTA
-    T eps, b1, b2, omb1, omb2, wd;
+    const double *rowsum;  // sum_j |W_ij| per node (manipulated gradients)
+    T eps, b1, b2, omb1, omb2, wd, gamma;
+    int opt, disc;
+    int first_step;      // index in this chunk of the anneal's step 0 (SGD momentum buffer starts there), or -1
     T inv_beta[PersistChunk<T>::kSteps];
     T step_size[PersistChunk<T>::kSteps];
     T rsqrt_bc2[PersistChunk<T>::kSteps];
@@ -107,6 +110,18 @@ __global__ void __launch_bounds__(1024, 1) persist_q2_kernel(const __grid_consta
     Sc<T> sc;
     sc.eps = p.eps; sc.b1 = p.b1; sc.b2 = p.b2; sc.omb1 = p.omb1; sc.omb2 = p.omb2; sc.wd = p.wd;
     sc.two_lambda = (T)0;
+    sc.gamma = p.gamma; sc.opt = p.opt; sc.disc = p.disc; sc.first = 0;
+    // manipulated gradients: c_i = 1 / sum_j |W_ij| (Ising: |2 J_ij|), static, so it lives in a register
+    T ci[IPT];
+#pragma unroll
+    for (int k = 0; k < IPT; ++k) {
+        ci[k] = (T)1;
+        const int i = v_begin + k * nt + tid;
+        if (p.disc && i < v_end) {
+            const double rs = p.rowsum[i] * (ISING ? 2.0 : 1.0);
+            ci[k] = rs > 0.0 ? (T)(1.0 / rs) : (T)0;
+        }
+    }
     int cur = 0;
     for (int t = 0; t < p.nsteps; ++t) {
         const T *__restrict__ gi = gbuf + (size_t)cur * n;
@@ -114,6 +129,7 @@ __global__ void __launch_bounds__(1024, 1) persist_q2_kernel(const __grid_consta
         sc.inv_beta = p.inv_beta[t];
         sc.step_size = p.step_size[t];
         sc.rsqrt_bc2 = p.rsqrt_bc2[t];
+        sc.first = t == p.first_step;
 #pragma unroll
         for (int k = 0; k < IPT; ++k) {
             const int i = v_begin + k * nt + tid;
@@ -123,15 +139,15 @@ __global__ void __launch_bounds__(1024, 1) persist_q2_kernel(const __grid_consta
                 if (WEIGHTED) {
                     const float *__restrict__ wp = ws + off[k];
 #pragma unroll 8
-                    for (int j = 0; j < deg[k]; ++j) dU += (T)wp[j * 32] * gi[cp[j * 32]];
+                    for (int j = 0; j < deg[k]; ++j) dU = fma((T)wp[j * 32], gi[cp[j * 32]], dU);
                 } else {
 #pragma unroll 8
                     for (int j = 0; j < deg[k]; ++j) dU += gi[cp[j * 32]];  // == fma(1, m_j, dU) of the stepwise kernel
                 }
                 if (ISING) dU = (T)-2 * dU;
-                const T g = (dU + h[k] * sc.inv_beta) * p1mp_of(h[k]);
-                h[k] = adam_update(h[k], g, m1[k], m2[k], sc);
-                const T mg = mag_of(h[k]);
+                const T g = q2_grad(dU, ci[k], h[k], sc);
+                h[k] = opt_update(h[k], g, m1[k], m2[k], sc);
+                const T mg = sc.disc ? sign_of(h[k]) : mag_of(h[k]);
                 if (CS > 1) {
                     for (unsigned pr = 0; pr < CS; ++pr) cluster.map_shared_rank(go, pr)[i] = mg;
                 } else {
@@ -280,12 +296,16 @@ static cudaError_t persist_run_t(Handle *hd, int t_begin, int t_end, F &&scalars
         p.nsteps = tb - ta;
         p.chunk = g.chunk;
         p.ell_cap = (int)hd->persist_ell[a];
+        p.rowsum = hd->rowsum;
+        p.first_step = -1;
         for (int t = ta; t < tb; ++t) {
             const StepScalars s = scalars(t);
             if (t == ta) {
                 const Sc<T> c(s);
                 p.eps = c.eps; p.b1 = c.b1; p.b2 = c.b2; p.omb1 = c.omb1; p.omb2 = c.omb2; p.wd = c.wd;
+                p.gamma = c.gamma; p.opt = c.opt; p.disc = c.disc;
             }
+            if (s.first) p.first_step = t - ta;
             p.inv_beta[t - ta] = (T)s.inv_beta;
             p.step_size[t - ta] = (T)s.step_size;
             p.rsqrt_bc2[t - ta] = (T)s.rsqrt_bc2;

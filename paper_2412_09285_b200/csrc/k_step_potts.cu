@@ -20,10 +20,12 @@ struct PottsParams {
     BlockArrays<T> a;
     DevProblem dp;
     Sc<T> sc;
+    const double *rowsum;   // sum_j W_ij per node (manipulated gradients: c^f_i, c^a_i)
     const long long *S_in;  // fixed-point column sums of D(t), [q*Rb] per replica block
     long long *S_out;       // accumulated by this launch: column sums of D(t+1)
     long long *S_zero;      // cleared by this launch (the buffer the launch after next accumulates into)
     double fx_scale, fx_inv;
+    int disc_out;        // the gathered quantity is the centred one-hot vector (manipulated gradients)
     int lps;             // lanes per state = Rb / VEC
     int team;            // QPAD * lps lanes per variable (<= 32)
     int teams_per_warp;  // 32 / team
@@ -53,6 +55,14 @@ __global__ void __launch_bounds__(kThreads) potts_team_kernel(const PottsParams<
     for (int k = 0; k < kStages; ++k)
         partner[k] = tw < p.teams_per_warp ? tw * p.team + ((s ^ (1 << k)) * p.lps + rl) : lane;
 
+    // centred one-hot of the team's fields: 1 - 1/q on the lowest state among the maxima (rounding rule R3), -1/q
+    // elsewhere (S27's e_j; constants in s cancel in S20 like for the centred marginals)
+    auto one_hot = [&](T hv, T mx, bool okk, T inv_q_) -> T {
+        int cand = (okk && hv == mx) ? s : 1 << 30;
+#pragma unroll
+        for (int k = 0; k < kStages; ++k) cand = min(cand, __shfl_sync(0xffffffffu, cand, partner[k]));
+        return (cand == s ? (T)1 : (T)0) - inv_q_;
+    };
     const int64_t blk = (int64_t)blockIdx.y * p.a.blk_stride;
     const unsigned lo = (unsigned)(s * p.lps + rl) * VEC;  // offset inside a row
     const T *__restrict__ gin = p.a.g_in + blk + lo;
@@ -94,7 +104,7 @@ __global__ void __launch_bounds__(kThreads) potts_team_kernel(const PottsParams<
         }
         if (STEP) {
             // softmax of h(t) across the team's states
-            T P[VEC];
+            T P[VEC], own[VEC];  // own: what the balance term subtracts (P_i, or the centred one-hot e_i when manipulated)
 #pragma unroll
             for (int v = 0; v < VEC; ++v) {
                 T mx = h[v];
@@ -105,6 +115,16 @@ __global__ void __launch_bounds__(kThreads) potts_team_kernel(const PottsParams<
 #pragma unroll
                 for (int k = 0; k < kStages; ++k) z += shfl_any(z, partner[k]);
                 P[v] = e * frcp(z);
+                own[v] = P[v];
+                if (sc.disc) own[v] = one_hot(h[v], mx, ok, inv_q);
+            }
+            // manipulated gradients (S27): c^f = q / sum_j W_ij on the cut term, lambda c^a with
+            // c^a = q / sqrt(sum_j W_ij) on the balance term (S26's 2 lambda becomes lambda); no neighbours: 0
+            T cf = (T)1, lam_c = sc.two_lambda;
+            if (sc.disc) {
+                const double rs = ok ? __ldg(p.rowsum + i) : 0.0;
+                cf = rs > 0.0 ? (T)((double)q / rs) : (T)0;
+                lam_c = rs > 0.0 ? (T)(0.5 * (double)sc.two_lambda * ((double)q / sqrt(rs))) : (T)0;
             }
             // coupling contraction f(s) = sum_j W_ij D_j(s): kGatherChunk neighbour rows in flight
             T f[VEC];
@@ -138,27 +158,28 @@ __global__ void __launch_bounds__(kThreads) potts_team_kernel(const PottsParams<
                 }
             }
             // g^p (S26), then g^h = P (g^p - <g^p>_P) (S20), Adam
-            R m1, m2, hn;
+            R m1 = {}, m2 = {}, hn;
+            const bool use_m1 = sc.uses_m1(), use_m2 = sc.uses_m2();
             if (ok) {
-                m1 = R::ld_stream(p.a.m1 + off);
-                m2 = R::ld_stream(p.a.m2 + off);
+                if (use_m1) m1 = R::ld_stream(p.a.m1 + off);
+                if (use_m2) m2 = R::ld_stream(p.a.m2 + off);
             }
 #pragma unroll
             for (int v = 0; v < VEC; ++v) {
-                const T gp = ok ? -f[v] + sc.two_lambda * (Ss[v] - P[v]) + h[v] * sc.inv_beta : (T)0;
+                const T gp = ok ? -(cf * f[v]) + lam_c * (Ss[v] - own[v]) + h[v] * sc.inv_beta : (T)0;
                 T gbar = P[v] * gp;
 #pragma unroll
                 for (int k = 0; k < kStages; ++k) gbar += shfl_any(gbar, partner[k]);
                 if (ok) {
-                    const T g = P[v] * (gp - gbar);
-                    hn.v[v] = adam_update(h[v], g, m1.v[v], m2.v[v], sc);
+                    const T g = sc.gamma * (P[v] * (gp - gbar));
+                    hn.v[v] = opt_update(h[v], g, m1.v[v], m2.v[v], sc);
                     h[v] = hn.v[v];
                 }
             }
             if (ok) {
                 hn.st_stream(p.a.h + off);
-                m1.st_stream(p.a.m1 + off);
-                m2.st_stream(p.a.m2 + off);
+                if (use_m1) m1.st_stream(p.a.m1 + off);
+                if (use_m2) m2.st_stream(p.a.m2 + off);
             }
         }
         // centred marginals D = P - 1/q of the (new) fields -> g_out, and their column sums.  Constants in s
@@ -175,6 +196,7 @@ __global__ void __launch_bounds__(kThreads) potts_team_kernel(const PottsParams<
 #pragma unroll
             for (int k = 0; k < kStages; ++k) z += shfl_any(z, partner[k]);
             po.v[v] = e * frcp(z) - inv_q;
+            if (p.disc_out) po.v[v] = one_hot(h[v], mx, ok, inv_q);
             if (ok) colacc[v] += __double2ll_rn((double)po.v[v] * p.fx_scale);
         }
         if (ok) po.st(p.a.g_out + off);
@@ -239,6 +261,8 @@ static void launch_potts_typed(Handle *hd, const StepScalars &sc, bool step, int
     p.S_in = hd->colsum[t % 3] + so;
     p.S_out = hd->colsum[(step ? t + 1 : t) % 3] + so;
     p.S_zero = hd->colsum[(step ? t + 2 : t + 1) % 3] + so;
+    p.rowsum = hd->rowsum;
+    p.disc_out = hd->gather_disc ? 1 : 0;
     p.fx_scale = hd->colsum_scale;
     p.fx_inv = 1.0 / hd->colsum_scale;
     const int vec = potts_vec(Rb);

@@ -18,6 +18,7 @@ struct Q2Params {
     DevProblem dp;
     Sc<T> sc;
     const T *field;     // dense Ising: precomputed J*m, same layout as h
+    const double *rowsum;  // sum_j |W_ij| per node (manipulated gradients), or nullptr
     unsigned rv;        // Rb / VEC lanes per variable
     int rv_shift;       // log2(rv) when rv is a power of two, else -1
     unsigned total;     // n * rv threads per replica block
@@ -49,9 +50,12 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
         }
     }
     pdl_wait();
+    const Sc<T> &sc = p.sc;
+    const bool use_m1 = sc.uses_m1(), use_m2 = sc.uses_m2();  // uniform: SGD keeps no second moment (8 B per field less)
     const R h4 = R::ld_stream(p.a.h + off);
-    R m1 = R::ld_stream(p.a.m1 + off);
-    R m2 = R::ld_stream(p.a.m2 + off);
+    R m1 = {}, m2 = {};
+    if (use_m1) m1 = R::ld_stream(p.a.m1 + off);
+    if (use_m2) m2 = R::ld_stream(p.a.m2 + off);
 
     T dU[VEC];
 #pragma unroll
@@ -67,7 +71,7 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
 #pragma unroll
             for (int k = 0; k < DEG; ++k)
 #pragma unroll
-                for (int v = 0; v < VEC; ++v) dU[v] += (T)wj[k] * nb[k].v[v];
+                for (int v = 0; v < VEC; ++v) dU[v] = fma((T)wj[k], nb[k].v[v], dU[v]);
         } else {
             const int e0 = __ldg(p.dp.row_ptr + i), e1 = __ldg(p.dp.row_ptr + i + 1);
 #pragma unroll 4
@@ -76,7 +80,7 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
                 const float wj = w ? __ldg(w + e) : 1.0f;
                 const R nb = R::ld(gin + (unsigned)j * Rb);
 #pragma unroll
-                for (int v = 0; v < VEC; ++v) dU[v] += (T)wj * nb.v[v];
+                for (int v = 0; v < VEC; ++v) dU[v] = fma((T)wj, nb.v[v], dU[v]);
             }
         }
         if (MODE == MODE_ISING) {
@@ -126,18 +130,24 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
         }
     }
 
-    const Sc<T> &sc = p.sc;
+    // manipulated gradients (S29/S30): the gathered values are sgn(m_j) and the coupling term is
+    // normalised by c_i = 1 / sum_j |W_ij| (Ising: |2 J_ij|; nodes without neighbours: 0); all kinds: times gamma_grad
+    T ci = (T)1;
+    if (sc.disc) {  // only set for the sparse graph kinds (fem_anneal)
+        const double rs = __ldg(p.rowsum + i) * (MODE == MODE_ISING ? 2.0 : 1.0);
+        ci = rs > 0.0 ? (T)(1.0 / rs) : (T)0;
+    }
     R hn, gn;
 #pragma unroll
     for (int v = 0; v < VEC; ++v) {
         const T h = h4.v[v];
-        const T g = (dU[v] + h * sc.inv_beta) * p1mp_of(h);  // S29 with ln(p/(1-p)) = h
-        hn.v[v] = adam_update(h, g, m1.v[v], m2.v[v], sc);
-        gn.v[v] = mag_of(hn.v[v]);
+        const T g = q2_grad(dU[v], ci, h, sc);  // S29 with ln(p/(1-p)) = h
+        hn.v[v] = opt_update(h, g, m1.v[v], m2.v[v], sc);
+        gn.v[v] = sc.disc ? sign_of(hn.v[v]) : mag_of(hn.v[v]);
     }
     hn.st_stream(p.a.h + off);
-    m1.st_stream(p.a.m1 + off);
-    m2.st_stream(p.a.m2 + off);
+    if (use_m1) m1.st_stream(p.a.m1 + off);
+    if (use_m2) m2.st_stream(p.a.m2 + off);
     gn.st(p.a.g_out + off);
 }
 
@@ -145,13 +155,13 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
 // the constant-1 row that pads short clauses, in both gather buffers.
 template <typename T>
 __global__ void __launch_bounds__(kThreads) q2_prepare_kernel(const T *h, T *g, T *g_other, int64_t blk_stride, int Rb,
-                                                              int n, int nblocks) {
+                                                              int n, int nblocks, int disc) {
     const int64_t per = (int64_t)n * Rb;
     const int64_t idx = (int64_t)blockIdx.x * kThreads + threadIdx.x;
     if (idx >= per * nblocks) return;
     const int64_t b = idx / per, r = idx - b * per;
     const int64_t off = b * blk_stride + r;
-    g[off] = (T)mag_of((double)h[off]);
+    g[off] = disc ? (T)sign_of(h[off]) : (T)mag_of((double)h[off]);
     if (r < Rb) {
         g[b * blk_stride + per + r] = (T)1;
         g_other[b * blk_stride + per + r] = (T)1;
@@ -241,7 +251,7 @@ bool launch_step_dense_tc(Handle *hd, const StepScalars &sc);  // k_dense_tc.cu
 template <typename T>
 static void launch_step_q2_t(Handle *hd, const StepScalars &sc, int blk_begin, int blk_count) {
     using S = StateOf<T>;
-    if (std::is_same<T, float>::value && hd->dp.kind == FEM_ISING && hd->dp.J && blk_begin == 0 && blk_count == 1 &&
+    if (std::is_same<T, float>::value && hd->dp.kind == FEM_ISING && hd->dp.J && blk_begin == 0 && blk_count == 1 && hd->plain_adam &&
         launch_step_dense_tc(hd, sc))
         return;  // dense couplings: tcgen05 GEMM with the update fused in its epilogue
     const int Rb = hd->Rb;
@@ -257,6 +267,7 @@ static void launch_step_q2_t(Handle *hd, const StepScalars &sc, int blk_begin, i
     p.dp = hd->dp;
     p.sc = Sc<T>(sc);
     p.field = nullptr;
+    p.rowsum = hd->rowsum;
     int mode = hd->dp.kind == FEM_MAXCUT ? MODE_MAXCUT : hd->dp.kind == FEM_MAXSAT ? MODE_SAT : MODE_ISING;
     if (hd->dp.kind == FEM_ISING && hd->dp.J) {
         mode = MODE_FIELD;
@@ -290,10 +301,10 @@ void launch_prepare_q2(Handle *hd, bool wide) {
     const unsigned grid = (unsigned)ceil_div(total, kThreads);
     if (wide)
         q2_prepare_kernel<double><<<grid, kThreads, 0, hd->stream>>>(hd->hW, hd->gW[hd->cur], hd->gW[hd->cur ^ 1],
-                                                                     hd->rows * hd->Rb, hd->Rb, hd->dp.n, nb);
+                                                                     hd->rows * hd->Rb, hd->Rb, hd->dp.n, nb, hd->gather_disc ? 1 : 0);
     else
         q2_prepare_kernel<float><<<grid, kThreads, 0, hd->stream>>>(hd->h, hd->g[hd->cur], hd->g[hd->cur ^ 1],
-                                                                    hd->rows * hd->Rb, hd->Rb, hd->dp.n, nb);
+                                                                    hd->rows * hd->Rb, hd->Rb, hd->dp.n, nb, hd->gather_disc ? 1 : 0);
     hd->launches++;
 }
 

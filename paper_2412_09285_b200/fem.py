@@ -47,7 +47,12 @@ class CSchedule(C.Structure):
         ("steps", C.c_int32), ("beta", C.c_void_p), ("lambda_", C.c_void_p),
         ("lr", C.c_double), ("beta1", C.c_double), ("beta2", C.c_double), ("eps", C.c_double),
         ("weight_decay", C.c_double), ("init_scale", C.c_double), ("precise_steps", C.c_int32),
+        ("optimizer", C.c_int32), ("alpha", C.c_double), ("momentum", C.c_double), ("dampening", C.c_double),
+        ("manipulated", C.c_int32), ("gamma_grad", C.c_double),
     ]
+
+
+ADAM, RMSPROP, SGD = 0, 1, 2   # fem_optimizer
 
 
 _lib = None
@@ -93,7 +98,7 @@ def _ptr(a: Optional[np.ndarray]):
 
 @dataclass
 class Schedule:
-    """Host-side schedule: beta[t] (and optional lambda[t]) plus Adam settings."""
+    """Host-side schedule: beta[t] (and optional lambda[t]), the optimiser and the gradient mode."""
     beta: np.ndarray
     lr: float = 0.1
     beta1: float = 0.9
@@ -103,13 +108,20 @@ class Schedule:
     init_scale: float = 1e-3
     precise_steps: int = 8
     lam: Optional[np.ndarray] = None
+    optimizer: int = ADAM          # ADAM / RMSPROP / SGD, PyTorch semantics
+    alpha: float = 0.99            # RMSprop smoothing constant
+    momentum: float = 0.0          # RMSprop / SGD
+    dampening: float = 0.0         # SGD
+    manipulated: bool = False      # manipulated gradients S25/S27/S30
+    gamma_grad: float = 1.0        # S20
 
     def c(self) -> CSchedule:
         self.beta = np.ascontiguousarray(self.beta, dtype=np.float64)
         if self.lam is not None:
             self.lam = np.ascontiguousarray(self.lam, dtype=np.float64)
         return CSchedule(int(self.beta.size), _ptr(self.beta), _ptr(self.lam), self.lr, self.beta1, self.beta2, self.eps,
-                         self.weight_decay, self.init_scale, self.precise_steps)
+                         self.weight_decay, self.init_scale, self.precise_steps, int(self.optimizer), self.alpha,
+                         self.momentum, self.dampening, 1 if self.manipulated else 0, self.gamma_grad)
 
 
 def linear_temperature_schedule(T_max: float, T_min: float, steps: int) -> np.ndarray:

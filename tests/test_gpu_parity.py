@@ -270,14 +270,18 @@ def _persist_cases():
     }
 
 
+@pytest.mark.parametrize("mode", ["adam_exact", "rmsprop_manipulated", "sgd_exact"])
 @pytest.mark.parametrize("name", list(_persist_cases()))
-def test_persistent_kernel_bit_identical_to_stepwise(fem, name):
+def test_persistent_kernel_bit_identical_to_stepwise(fem, name, mode):
     """Small sparse two-state problems run in the replica-persistent kernel (one CTA per replica, state in
     registers, gathers from shared memory).  Its arithmetic is the stepwise kernel's, so fields, moments and
     energies must be bit-identical, including across a resume (stop_after) and the fp64 wide phase."""
     inst, R = _persist_cases()[name]()
     steps = 300                                                      # spans two parameter chunks of the fp32 kernel
-    sch = fem.Schedule(beta=fem.linear_temperature_schedule(1.0, 0.01, steps), precise_steps=8)
+    extra = {"adam_exact": {}, "rmsprop_manipulated": dict(optimizer=1, lr=0.03, alpha=0.9, momentum=0.5,
+                                                            manipulated=True, gamma_grad=0.9),
+             "sgd_exact": dict(optimizer=2, lr=0.3, momentum=0.7, dampening=0.2)}[mode]
+    sch = fem.Schedule(beta=fem.linear_temperature_schedule(1.0, 0.01, steps), precise_steps=8, **extra)
     out = {}
     for persistent in (0, 1, 2, 3, 5, 9):                             # off, automatic, clusters of 1, 2, 4, 8 CTAs per replica
         eng = fem.Fem(inst, R)
