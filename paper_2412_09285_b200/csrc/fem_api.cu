@@ -492,8 +492,10 @@ int64_t fem_get_info(const fem_handle *h, const char *key) {
     if (!strcmp(key, "step_bytes")) {
         // algorithmic HBM bytes of one fused step: 24 B per field (read and write h, m1, m2)
         // plus the problem structure once
+        // (8 B per moment array the optimiser of the last fem_anneal does not keep less: SGD has no second moment,
+        // RMSprop / SGD without momentum no first)
         const int64_t fields = (int64_t)hd->dp.n * hd->dp.F * hd->R;
-        return 24 * fields + hd->structure_bytes;
+        return hd->bytes_per_field * fields + hd->structure_bytes;
     }
     return -1;
 }
@@ -605,6 +607,7 @@ fem_status fem_anneal(fem_handle *h, const fem_schedule *sch, int32_t R, uint64_
     if (hd->gather_valid && hd->gather_disc != disc) hd->gather_valid = false;
     hd->gather_disc = disc;
     hd->plain_adam = sch->optimizer == FEM_ADAM && !sch->manipulated;
+    hd->bytes_per_field = 8 + (sch->optimizer == FEM_ADAM || sch->momentum > 0 ? 8 : 0) + (sch->optimizer != FEM_SGD ? 8 : 0);
     auto scalars = [&](int t) {
         StepScalars sc;
         sc.inv_beta = 1.0 / sch->beta[t];

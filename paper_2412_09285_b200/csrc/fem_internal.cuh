@@ -84,6 +84,7 @@ struct Handle {
     int tc_maps_R = -1;
     bool tc_ready = false;                   // g[cur]/glo[cur] hold GT / GT_lo of the current fields
     double *rowsum = nullptr;  // graph kinds: sum_j |W_ij| per node (manipulated gradients: c_i, c^f_i, c^a_i)
+    int bytes_per_field = 24;  // algorithmic HBM bytes per field per step: read + write of h and of the moments in use
     bool plain_adam = true;    // Adam on the exact gradient: the only update the tcgen05 dense step implements
     bool gather_disc = false;  // the gather buffers hold one-hot values (manipulated gradients), not marginals
     long long *colsum[3] = {nullptr, nullptr, nullptr};  // Potts column sums S[q][R] in fixed point, rotating

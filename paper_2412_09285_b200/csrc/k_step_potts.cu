@@ -37,7 +37,7 @@ __device__ __forceinline__ double shfl_any(double v, int src) { return __shfl_sy
 
 constexpr int kGatherChunk = 5;  // neighbour rows in flight per lane
 
-template <typename T, int QPAD, int VEC, bool STEP>
+template <typename T, int QPAD, int VEC, bool STEP, bool DISC>
 __global__ void __launch_bounds__(kThreads) potts_team_kernel(const PottsParams<T> p) {
     using R = Row<T, VEC>;
     constexpr int kStages = QPAD == 32 ? 5 : QPAD == 16 ? 4 : QPAD == 8 ? 3 : QPAD == 4 ? 2 : 1;
@@ -116,12 +116,12 @@ __global__ void __launch_bounds__(kThreads) potts_team_kernel(const PottsParams<
                 for (int k = 0; k < kStages; ++k) z += shfl_any(z, partner[k]);
                 P[v] = e * frcp(z);
                 own[v] = P[v];
-                if (sc.disc) own[v] = one_hot(h[v], mx, ok, inv_q);
+                if (DISC) own[v] = one_hot(h[v], mx, ok, inv_q);
             }
             // manipulated gradients (S27): c^f = q / sum_j W_ij on the cut term, lambda c^a with
             // c^a = q / sqrt(sum_j W_ij) on the balance term (S26's 2 lambda becomes lambda); no neighbours: 0
             T cf = (T)1, lam_c = sc.two_lambda;
-            if (sc.disc) {
+            if (DISC) {
                 const double rs = ok ? __ldg(p.rowsum + i) : 0.0;
                 cf = rs > 0.0 ? (T)((double)q / rs) : (T)0;
                 lam_c = rs > 0.0 ? (T)(0.5 * (double)sc.two_lambda * ((double)q / sqrt(rs))) : (T)0;
@@ -166,7 +166,11 @@ __global__ void __launch_bounds__(kThreads) potts_team_kernel(const PottsParams<
             }
 #pragma unroll
             for (int v = 0; v < VEC; ++v) {
-                const T gp = ok ? -(cf * f[v]) + lam_c * (Ss[v] - own[v]) + h[v] * sc.inv_beta : (T)0;
+                T gp = (T)0;
+                if (ok) {
+                    if (DISC) gp = -(cf * f[v]) + lam_c * (Ss[v] - own[v]) + h[v] * sc.inv_beta;
+                    else gp = -f[v] + sc.two_lambda * (Ss[v] - P[v]) + h[v] * sc.inv_beta;
+                }
                 T gbar = P[v] * gp;
 #pragma unroll
                 for (int k = 0; k < kStages; ++k) gbar += shfl_any(gbar, partner[k]);
@@ -196,7 +200,7 @@ __global__ void __launch_bounds__(kThreads) potts_team_kernel(const PottsParams<
 #pragma unroll
             for (int k = 0; k < kStages; ++k) z += shfl_any(z, partner[k]);
             po.v[v] = e * frcp(z) - inv_q;
-            if (p.disc_out) po.v[v] = one_hot(h[v], mx, ok, inv_q);
+            if (DISC) po.v[v] = one_hot(h[v], mx, ok, inv_q);
             if (ok) colacc[v] += __double2ll_rn((double)po.v[v] * p.fx_scale);
         }
         if (ok) po.st(p.a.g_out + off);
@@ -219,8 +223,12 @@ __global__ void __launch_bounds__(kThreads) potts_team_kernel(const PottsParams<
 
 template <typename T, int QPAD, int VEC>
 static void launch_potts_t(Handle *hd, const PottsParams<T> &p, dim3 grid, bool step) {
-    if (step) launch_pdl(potts_team_kernel<T, QPAD, VEC, true>, grid, dim3(kThreads), hd->stream, p);
-    else launch_pdl(potts_team_kernel<T, QPAD, VEC, false>, grid, dim3(kThreads), hd->stream, p);
+    // DISC (manipulated gradients) is a template parameter so that the exact-gradient kernel carries none of it
+    const bool disc = p.disc_out != 0;
+    if (step && disc) launch_pdl(potts_team_kernel<T, QPAD, VEC, true, true>, grid, dim3(kThreads), hd->stream, p);
+    else if (step) launch_pdl(potts_team_kernel<T, QPAD, VEC, true, false>, grid, dim3(kThreads), hd->stream, p);
+    else if (disc) launch_pdl(potts_team_kernel<T, QPAD, VEC, false, true>, grid, dim3(kThreads), hd->stream, p);
+    else launch_pdl(potts_team_kernel<T, QPAD, VEC, false, false>, grid, dim3(kThreads), hd->stream, p);
 }
 
 template <typename T, int QPAD>
