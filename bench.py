@@ -62,19 +62,21 @@ def load_traffic(workload: str):
 
 
 class ClockSampler:
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+    Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index: int):
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
-                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                       "--format=csv,noheader,nounits", "-lms", "20"], stdout=self.f,
                                       stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
 
-    def stop(self):
+    def stop(self, t_begin=None, t_end=None):
+        """Samples whose wall-clock timestamp falls in [t_begin, t_end] (the timed region); if the region was shorter
+        than the sampling period, the samples nearest to it."""
         if self.p is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         self.p.terminate()
@@ -84,27 +86,31 @@ class ClockSampler:
             self.p.kill()
         self.f.flush()
         self.f.seek(0)
-        sm, mx, reasons = [], [], set()
+        import datetime
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = []
         for line in self.f:
             parts = [x.strip() for x in line.split(",")]
-            if len(parts) < 7:
+            if len(parts) < 8:
                 continue
             try:
-                sm.append(float(parts[0]))
-                mx.append(float(parts[1]))
+                ts = datetime.datetime.strptime(parts[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                rows.append((ts, float(parts[1]), float(parts[2]),
+                             [nm for nm, val in zip(names, parts[4:8]) if val.lower().startswith("active")]))
             except ValueError:
                 continue
-            for nm, val in zip(names, parts[3:7]):
-                if val.lower().startswith("active"):
-                    reasons.add(nm)
         self.f.close()
         os.unlink(self.f.name)
-        # under load = the upper half of the samples (idle samples before/after the region drop out)
-        sm_sorted = sorted(sm)
-        load = sm_sorted[len(sm_sorted) // 2:] if sm_sorted else []
-        return {"sm_mhz": float(np.median(load)) if load else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        inside = [r for r in rows if t_begin is not None and t_begin <= r[0] <= t_end]
+        where = "inside the timed region"
+        if not inside:
+            mid = 0.5 * ((t_begin or rows[-1][0]) + (t_end or rows[-1][0]))
+            inside = sorted(rows, key=lambda r: abs(r[0] - mid))[:3]
+            where = "nearest to the timed region (shorter than the 20 ms sampling period)"
+        return {"sm_mhz": float(np.median([r[1] for r in inside])), "sm_max_mhz": max(r[2] for r in inside),
+                "reasons": sorted({x for r in inside for x in r[3]}), "samples": len(inside), "sampled": where}
 
 
 def oracle_sample(cfg, inst, seconds_target: float = 12.0):
@@ -259,11 +265,12 @@ def main():
             ev.append((a, b, eng.info("launches") - l0 - (1 if K > 0 else 0)))
         eng.readout()                                          # rounding + energies + argmin
 
+    sampler = ClockSampler(local_rank) if rank == 0 else None   # started before warm-up: nvidia-smi takes a while to start
     for w in range(args.warmup):
         one_pass(multigpu.replica_seed(1000 + w, rank))
     barrier()
     launches0 = eng.info("launches")
-    sampler = ClockSampler(local_rank) if rank == 0 else None
+    wall_begin = time.time()
     bulk_events = []
     start, end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     start.record()
@@ -272,7 +279,8 @@ def main():
     end.record()
     barrier()
     elapsed_ms = start.elapsed_time(end)
-    clocks = sampler.stop() if sampler else None
+    wall_end = time.time()
+    clocks = sampler.stop(wall_begin, wall_end) if sampler else None
     launches = eng.info("launches") - launches0
     res = eng.result()
     bulk_ms = sum(a.elapsed_time(b) for a, b, _ in bulk_events)
