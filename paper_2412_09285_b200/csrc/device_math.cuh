@@ -83,6 +83,44 @@ struct Row {
     }
 };
 
+// ---- compact gather buffer of the manipulated gradients ----
+// With one-hot neighbours (S25/S27/S30) the gathered quantity is an integer: sgn(m_j) in {-1, 0, +1} for the
+// two-state kinds, the state id argmax_s h_j(s) for the Potts kind.  It is stored as ONE BYTE per (variable,
+// replica) -- element (i, r) of a replica block at byte i*Rb + r of the fp32 gather array's memory -- so a
+// neighbour gather moves 1 byte where the exact gradient moves 4 (two-state) or 4q (Potts) bytes
+// (SURVEY.md section 8(f) row 1).  VEC consecutive replicas travel as one 8-, 16- or 32-bit access.
+template <int VEC>
+__device__ __forceinline__ void ld_bytes(const signed char *p, int (&out)[VEC]) {
+    if constexpr (VEC == 4) {
+        const int w = __ldg(reinterpret_cast<const int *>(p));
+#pragma unroll
+        for (int v = 0; v < 4; ++v) out[v] = (int)(signed char)((w >> (8 * v)) & 0xff);
+    } else if constexpr (VEC == 2) {
+        const short w = __ldg(reinterpret_cast<const short *>(p));
+        out[0] = (int)(signed char)(w & 0xff);
+        out[1] = (int)(signed char)((w >> 8) & 0xff);
+    } else {
+        out[0] = (int)__ldg(p);
+    }
+}
+// the same VEC bytes left packed in one word (byte v = replica v), for kernels that keep many neighbours in flight
+template <int VEC>
+__device__ __forceinline__ unsigned ld_bytes_packed(const signed char *p) {
+    if constexpr (VEC == 4) return (unsigned)__ldg(reinterpret_cast<const int *>(p));
+    else if constexpr (VEC == 2) return (unsigned)(unsigned short)__ldg(reinterpret_cast<const short *>(p));
+    else return (unsigned)(unsigned char)__ldg(p);
+}
+template <int VEC>
+__device__ __forceinline__ void st_bytes(signed char *p, const int (&in)[VEC]) {
+    if constexpr (VEC == 4) {
+        *reinterpret_cast<int *>(p) = (in[0] & 0xff) | ((in[1] & 0xff) << 8) | ((in[2] & 0xff) << 16) | ((in[3] & 0xff) << 24);
+    } else if constexpr (VEC == 2) {
+        *reinterpret_cast<short *>(p) = (short)((in[0] & 0xff) | ((in[1] & 0xff) << 8));
+    } else {
+        *p = (signed char)in[0];
+    }
+}
+
 // ---- programmatic dependent launch (PDL): consecutive step kernels overlap launch latency and tail ----
 // pdl_trigger lets the NEXT kernel in the stream start being scheduled once every CTA of this grid has
 // started; pdl_wait blocks until the PREVIOUS grid has completed and its writes are visible.  Only loads

@@ -115,11 +115,13 @@ __global__ void __launch_bounds__(kThreads) narrow_kernel(const double *hW, cons
     const int64_t idx = (int64_t)blockIdx.x * kThreads + threadIdx.x;
     if (idx < count) {
         h[idx] = (float)hW[idx];
-        if (!fields_only) {
+        if (fields_only != 1) {
             m1[idx] = (float)m1W[idx];
             m2[idx] = (float)m2W[idx];
-            g[idx] = (float)gW[idx];
-            g_other[idx] = (float)gW[idx];  // carries the constant-1 pad rows into both buffers
+            if (fields_only == 0) {  // 2: the gather arrays hold bytes shared by both precisions (manipulated gradients)
+                g[idx] = (float)gW[idx];
+                g_other[idx] = (float)gW[idx];  // carries the constant-1 pad rows into both buffers
+            }
         }
     }
 }
@@ -148,7 +150,7 @@ void launch_narrow(Handle *hd, bool fields_only) {
     const int64_t count = hd->rows * (int64_t)hd->R;
     narrow_kernel<<<(unsigned)ceil_div(count, kThreads), kThreads, 0, hd->stream>>>(
         hd->hW, hd->m1W, hd->m2W, hd->gW[hd->cur], hd->h, hd->m1, hd->m2, hd->g[hd->cur], hd->g[hd->cur ^ 1], count,
-        fields_only ? 1 : 0);
+        fields_only ? 1 : (hd->gather_disc ? 2 : 0));
     hd->launches++;
 }
 

@@ -42,6 +42,8 @@ struct PersistParams {
     int chunk;           // variables per CTA of the cluster (multiple of 32)
     int ell_cap;         // sliced-ELL entries reserved per CTA
     const double *rowsum;  // sum_j |W_ij| per node (manipulated gradients)
+    const signed char *g8_in;  // manipulated gradients: sgn(m) as bytes in the gather arrays (device_math.cuh)
+    signed char *g8_out;
     T eps, b1, b2, omb1, omb2, wd, gamma;
     int opt, disc;
     int first_step;      // index in this chunk of the anneal's step 0 (SGD momentum buffer starts there), or -1
@@ -89,7 +91,8 @@ __global__ void __launch_bounds__(1024, 1) persist_q2_kernel(const __grid_consta
         for (int s = 16; s > 0; s >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, s));
         if (lane == 0) unit_off[k * nwarps + warp + 1] = mx * 32;
     }
-    for (int i = tid; i < n; i += nt) gbuf[i] = p.g_in[base + (int64_t)i * p.Rb];
+    for (int i = tid; i < n; i += nt)
+        gbuf[i] = p.disc ? (T)(int)p.g8_in[base + (int64_t)i * p.Rb] : p.g_in[base + (int64_t)i * p.Rb];
     if (tid == 0) unit_off[0] = 0;
     __syncthreads();
     if (tid == 0)
@@ -170,7 +173,8 @@ __global__ void __launch_bounds__(1024, 1) persist_q2_kernel(const __grid_consta
             p.h[o] = h[k];
             p.m1[o] = m1[k];
             p.m2[o] = m2[k];
-            p.g_out[o] = gbuf[(size_t)cur * n + i];
+            if (p.disc) p.g8_out[o] = (signed char)(int)gbuf[(size_t)cur * n + i];
+            else p.g_out[o] = gbuf[(size_t)cur * n + i];
         }
     }
 }
@@ -297,6 +301,8 @@ static cudaError_t persist_run_t(Handle *hd, int t_begin, int t_end, F &&scalars
         p.chunk = g.chunk;
         p.ell_cap = (int)hd->persist_ell[a];
         p.rowsum = hd->rowsum;
+        p.g8_in = reinterpret_cast<const signed char *>(hd->g[hd->cur]);
+        p.g8_out = reinterpret_cast<signed char *>(hd->g[cur_after]);
         p.first_step = -1;
         for (int t = ta; t < tb; ++t) {
             const StepScalars s = scalars(t);

@@ -11,6 +11,9 @@
 // S20, like the "+1"), the chain rule, Adam, and the next marginals.  The column sums S_s of the NEXT step
 // are a by-product: every lane adds its new D' in 64-bit fixed point, so the sum is exact, independent of
 // the order and of the replica blocking, and integer atomics keep it deterministic (no float atomics).
+#include <algorithm>
+#include <map>
+
 #include "device_math.cuh"
 
 namespace fem {
@@ -21,6 +24,8 @@ struct PottsParams {
     DevProblem dp;
     Sc<T> sc;
     const double *rowsum;   // sum_j W_ij per node (manipulated gradients: c^f_i, c^a_i)
+    const signed char *g8_in;  // manipulated gradients: the state id argmax_s h_j(s), one byte per (variable, replica)
+    signed char *g8_out;       // (device_math.cuh); byte offsets of a replica block = its element offsets
     const long long *S_in;  // fixed-point column sums of D(t), [q*Rb] per replica block
     long long *S_out;       // accumulated by this launch: column sums of D(t+1)
     long long *S_zero;      // cleared by this launch (the buffer the launch after next accumulates into)
@@ -38,7 +43,7 @@ __device__ __forceinline__ double shfl_any(double v, int src) { return __shfl_sy
 constexpr int kGatherChunk = 5;  // neighbour rows in flight per lane
 
 template <typename T, int QPAD, int VEC, bool STEP, bool DISC>
-__global__ void __launch_bounds__(kThreads) potts_team_kernel(const PottsParams<T> p) {
+__global__ void __launch_bounds__(kThreads, DISC ? 3 : 4) potts_team_kernel(const PottsParams<T> p) {
     using R = Row<T, VEC>;
     constexpr int kStages = QPAD == 32 ? 5 : QPAD == 16 ? 4 : QPAD == 8 ? 3 : QPAD == 4 ? 2 : 1;
     __shared__ unsigned long long cta_sum[32 * VEC];
@@ -57,11 +62,11 @@ __global__ void __launch_bounds__(kThreads) potts_team_kernel(const PottsParams<
 
     // centred one-hot of the team's fields: 1 - 1/q on the lowest state among the maxima (rounding rule R3), -1/q
     // elsewhere (S27's e_j; constants in s cancel in S20 like for the centred marginals)
-    auto one_hot = [&](T hv, T mx, bool okk, T inv_q_) -> T {
+    auto winner = [&](T hv, T mx, bool okk) -> int {
         int cand = (okk && hv == mx) ? s : 1 << 30;
 #pragma unroll
         for (int k = 0; k < kStages; ++k) cand = min(cand, __shfl_sync(0xffffffffu, cand, partner[k]));
-        return (cand == s ? (T)1 : (T)0) - inv_q_;
+        return cand;
     };
     const int64_t blk = (int64_t)blockIdx.y * p.a.blk_stride;
     const unsigned lo = (unsigned)(s * p.lps + rl) * VEC;  // offset inside a row
@@ -103,6 +108,8 @@ __global__ void __launch_bounds__(kThreads) potts_team_kernel(const PottsParams<
             for (int v = 0; v < VEC; ++v) h[v] = ok ? r.v[v] : neg_big;
         }
         if (STEP) {
+            unsigned own_ids = 0;
+            if (DISC && ok) own_ids = ld_bytes_packed<VEC>(p.g8_in + blk + (int64_t)i * p.a.Rb + (unsigned)rl * VEC);
             // softmax of h(t) across the team's states
             T P[VEC], own[VEC];  // own: what the balance term subtracts (P_i, or the centred one-hot e_i when manipulated)
 #pragma unroll
@@ -116,7 +123,8 @@ __global__ void __launch_bounds__(kThreads) potts_team_kernel(const PottsParams<
                 for (int k = 0; k < kStages; ++k) z += shfl_any(z, partner[k]);
                 P[v] = e * frcp(z);
                 own[v] = P[v];
-                if (DISC) own[v] = one_hot(h[v], mx, ok, inv_q);
+                // manipulated: the variable's own one-hot vector is the state id the previous launch stored for it
+                if (DISC) own[v] = ((((own_ids >> (8 * v)) & 0xffu) == (unsigned)s) ? (T)1 : (T)0) - inv_q;
             }
             // manipulated gradients (S27): c^f = q / sum_j W_ij on the cut term, lambda c^a with
             // c^a = q / sqrt(sum_j W_ij) on the balance term (S26's 2 lambda becomes lambda); no neighbours: 0
@@ -139,6 +147,32 @@ __global__ void __launch_bounds__(kThreads) potts_team_kernel(const PottsParams<
                     e0 = __ldg(p.dp.row_ptr + i);
                     e1 = __ldg(p.dp.row_ptr + i + 1);
                 }
+                if (DISC) {
+                    // one-hot neighbours: f(s) = sum_j W_ij [state_j == s]; a neighbour is VEC bytes per lane.  Centred
+                    // by sum_j W_ij / q (constant in s, cancels in S20) so that f stays as small as in the exact path.
+                    constexpr int kIds = 10;
+                    const signed char *__restrict__ gin8 = p.g8_in + blk + (unsigned)rl * VEC;
+                    for (int e = e0; e < e1; e += kIds) {
+                        unsigned jj[kIds];
+                        T ww[kIds];
+                        unsigned ids[kIds];  // VEC state ids per neighbour, packed
+#pragma unroll
+                        for (int k = 0; k < kIds; ++k) {
+                            const bool in = e + k < e1;
+                            jj[k] = in ? (unsigned)__ldg(p.dp.col + e + k) : (unsigned)i;
+                            ww[k] = in ? (p.dp.w ? (T)__ldg(p.dp.w + e + k) : (T)1) : (T)0;
+                        }
+#pragma unroll
+                        for (int k = 0; k < kIds; ++k) ids[k] = ld_bytes_packed<VEC>(gin8 + jj[k] * (unsigned)p.a.Rb);
+#pragma unroll
+                        for (int k = 0; k < kIds; ++k)
+#pragma unroll
+                            for (int v = 0; v < VEC; ++v) f[v] += ((ids[k] >> (8 * v)) & 0xffu) == (unsigned)s ? ww[k] : (T)0;
+                    }
+                    const T shift = (T)(__ldg(p.rowsum + i) / (double)q);
+#pragma unroll
+                    for (int v = 0; v < VEC; ++v) f[v] -= shift;
+                } else {
                 for (int e = e0; e < e1; e += kGatherChunk) {
                     unsigned jj[kGatherChunk];
                     T ww[kGatherChunk];
@@ -155,6 +189,7 @@ __global__ void __launch_bounds__(kThreads) potts_team_kernel(const PottsParams<
                     for (int k = 0; k < kGatherChunk; ++k)
 #pragma unroll
                         for (int v = 0; v < VEC; ++v) f[v] += ww[k] * nb[k].v[v];
+                }
                 }
             }
             // g^p (S26), then g^h = P (g^p - <g^p>_P) (S20), Adam
@@ -190,8 +225,10 @@ __global__ void __launch_bounds__(kThreads) potts_team_kernel(const PottsParams<
         // cancel in S20, and near the uniform start the deviation from 1/q is all the signal there is, so it
         // is what gets stored and gathered.
         R po;
+        int win[VEC];
 #pragma unroll
         for (int v = 0; v < VEC; ++v) {
+            win[v] = 0;
             T mx = h[v];
 #pragma unroll
             for (int k = 0; k < kStages; ++k) mx = fmax(mx, shfl_any(mx, partner[k]));
@@ -200,10 +237,17 @@ __global__ void __launch_bounds__(kThreads) potts_team_kernel(const PottsParams<
 #pragma unroll
             for (int k = 0; k < kStages; ++k) z += shfl_any(z, partner[k]);
             po.v[v] = e * frcp(z) - inv_q;
-            if (DISC) po.v[v] = one_hot(h[v], mx, ok, inv_q);
+            if (DISC) {
+                win[v] = winner(h[v], mx, ok);
+                po.v[v] = (win[v] == s ? (T)1 : (T)0) - inv_q;
+            }
             if (ok) colacc[v] += __double2ll_rn((double)po.v[v] * p.fx_scale);
         }
-        if (ok) po.st(p.a.g_out + off);
+        if (DISC) {  // the state-0 lane of each replica group stores the VEC winners as bytes
+            if (ok && s == 0) st_bytes<VEC>(p.g8_out + blk + (int64_t)i * p.a.Rb + (unsigned)rl * VEC, win);
+        } else if (ok) {
+            po.st(p.a.g_out + off);
+        }
     }
 
     // column sums: exact integer adds -- lanes -> CTA (shared atomics) -> grid (global atomics)
@@ -221,14 +265,30 @@ __global__ void __launch_bounds__(kThreads) potts_team_kernel(const PottsParams<
     }
 }
 
+// grid-stride kernel: never more CTAs than are resident at once (occupancy x SMs), so no second wave
+template <typename T, int QPAD, int VEC, bool STEP, bool DISC>
+static void launch_potts_one(Handle *hd, const PottsParams<T> &p, dim3 grid) {
+    static std::map<int, int> resident;  // per device SM count: CTAs resident at once for THIS instantiation
+    int &r = resident[hd->sm_count];
+    if (r == 0) {
+        int occ = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, potts_team_kernel<T, QPAD, VEC, STEP, DISC>, kThreads, 0) !=
+                cudaSuccess || occ < 1)
+            occ = 1;
+        r = occ * hd->sm_count;
+    }
+    grid.x = std::min<unsigned>(grid.x, (unsigned)r);
+    launch_pdl(potts_team_kernel<T, QPAD, VEC, STEP, DISC>, grid, dim3(kThreads), hd->stream, p);
+}
+
 template <typename T, int QPAD, int VEC>
 static void launch_potts_t(Handle *hd, const PottsParams<T> &p, dim3 grid, bool step) {
     // DISC (manipulated gradients) is a template parameter so that the exact-gradient kernel carries none of it
     const bool disc = p.disc_out != 0;
-    if (step && disc) launch_pdl(potts_team_kernel<T, QPAD, VEC, true, true>, grid, dim3(kThreads), hd->stream, p);
-    else if (step) launch_pdl(potts_team_kernel<T, QPAD, VEC, true, false>, grid, dim3(kThreads), hd->stream, p);
-    else if (disc) launch_pdl(potts_team_kernel<T, QPAD, VEC, false, true>, grid, dim3(kThreads), hd->stream, p);
-    else launch_pdl(potts_team_kernel<T, QPAD, VEC, false, false>, grid, dim3(kThreads), hd->stream, p);
+    if (step && disc) launch_potts_one<T, QPAD, VEC, true, true>(hd, p, grid);
+    else if (step) launch_potts_one<T, QPAD, VEC, true, false>(hd, p, grid);
+    else if (disc) launch_potts_one<T, QPAD, VEC, false, true>(hd, p, grid);
+    else launch_potts_one<T, QPAD, VEC, false, false>(hd, p, grid);
 }
 
 template <typename T, int QPAD>
@@ -270,6 +330,8 @@ static void launch_potts_typed(Handle *hd, const StepScalars &sc, bool step, int
     p.S_out = hd->colsum[(step ? t + 1 : t) % 3] + so;
     p.S_zero = hd->colsum[(step ? t + 2 : t + 1) % 3] + so;
     p.rowsum = hd->rowsum;
+    p.g8_in = reinterpret_cast<const signed char *>(hd->g[hd->cur]) + base;
+    p.g8_out = reinterpret_cast<signed char *>(step ? hd->g[hd->cur ^ 1] : hd->g[hd->cur]) + base;
     p.disc_out = hd->gather_disc ? 1 : 0;
     p.fx_scale = hd->colsum_scale;
     p.fx_inv = 1.0 / hd->colsum_scale;

@@ -19,6 +19,8 @@ struct Q2Params {
     Sc<T> sc;
     const T *field;     // dense Ising: precomputed J*m, same layout as h
     const double *rowsum;  // sum_j |W_ij| per node (manipulated gradients), or nullptr
+    const signed char *g8_in;  // manipulated gradients: sgn(m) as bytes (device_math.cuh), same offsets as g_in
+    signed char *g8_out;
     unsigned rv;        // Rb / VEC lanes per variable
     int rv_shift;       // log2(rv) when rv is a power of two, else -1
     unsigned total;     // n * rv threads per replica block
@@ -38,6 +40,20 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
     const unsigned Rb = p.a.Rb;
     const int64_t off = blk + (i * Rb + c);  // a replica block holds < 2^32 elements (checked at fem_anneal)
     const T *__restrict__ gin = p.a.g_in + blk + c;
+    const signed char *__restrict__ gin8 = p.g8_in + blk + c;
+    const bool disc = p.sc.disc != 0;  // uniform; only ever set for the sparse graph kinds
+    // one neighbour row: VEC floats (exact gradient) or VEC bytes holding sgn(m_j) (manipulated gradients)
+    auto gather = [&](unsigned j) -> R {
+        if ((MODE == MODE_MAXCUT || MODE == MODE_ISING) && disc) {
+            int b[VEC];
+            ld_bytes<VEC>(gin8 + j * Rb, b);
+            R r;
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) r.v[v] = (T)b[v];
+            return r;
+        }
+        return R::ld(gin + j * Rb);
+    };
 
     // static structure first (legal before pdl_wait), then everything the previous step wrote
     int jj[DEG > 0 ? DEG : 1];
@@ -67,7 +83,7 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
         if (DEG > 0) {
             R nb[DEG > 0 ? DEG : 1];
 #pragma unroll
-            for (int k = 0; k < DEG; ++k) nb[k] = R::ld(gin + (unsigned)jj[k] * Rb);
+            for (int k = 0; k < DEG; ++k) nb[k] = gather((unsigned)jj[k]);
 #pragma unroll
             for (int k = 0; k < DEG; ++k)
 #pragma unroll
@@ -78,7 +94,7 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
             for (int e = e0; e < e1; ++e) {
                 const int j = __ldg(col + e);
                 const float wj = w ? __ldg(w + e) : 1.0f;
-                const R nb = R::ld(gin + (unsigned)j * Rb);
+                const R nb = gather((unsigned)j);
 #pragma unroll
                 for (int v = 0; v < VEC; ++v) dU[v] = fma((T)wj, nb.v[v], dU[v]);
             }
@@ -143,25 +159,36 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
         const T h = h4.v[v];
         const T g = q2_grad(dU[v], ci, h, sc);  // S29 with ln(p/(1-p)) = h
         hn.v[v] = opt_update(h, g, m1.v[v], m2.v[v], sc);
-        gn.v[v] = sc.disc ? sign_of(hn.v[v]) : mag_of(hn.v[v]);
+        gn.v[v] = disc ? sign_of(hn.v[v]) : mag_of(hn.v[v]);
     }
     hn.st_stream(p.a.h + off);
     if (use_m1) m1.st_stream(p.a.m1 + off);
     if (use_m2) m2.st_stream(p.a.m2 + off);
-    gn.st(p.a.g_out + off);
+    if (disc) {
+        int b[VEC];
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) b[v] = (int)gn.v[v];
+        st_bytes<VEC>(p.g8_out + off, b);
+    } else {
+        gn.st(p.a.g_out + off);
+    }
 }
 
 // Gathered quantity m = tanh(h/2) from the fields (used at t = 0 and after fem_set_fields); also writes
 // the constant-1 row that pads short clauses, in both gather buffers.
 template <typename T>
 __global__ void __launch_bounds__(kThreads) q2_prepare_kernel(const T *h, T *g, T *g_other, int64_t blk_stride, int Rb,
-                                                              int n, int nblocks, int disc) {
+                                                              int n, int nblocks, int disc, signed char *g8) {
     const int64_t per = (int64_t)n * Rb;
     const int64_t idx = (int64_t)blockIdx.x * kThreads + threadIdx.x;
     if (idx >= per * nblocks) return;
     const int64_t b = idx / per, r = idx - b * per;
     const int64_t off = b * blk_stride + r;
-    g[off] = disc ? (T)sign_of(h[off]) : (T)mag_of((double)h[off]);
+    if (disc) {
+        g8[off] = (signed char)(int)sign_of(h[off]);
+        return;
+    }
+    g[off] = (T)mag_of((double)h[off]);
     if (r < Rb) {
         g[b * blk_stride + per + r] = (T)1;
         g_other[b * blk_stride + per + r] = (T)1;
@@ -268,6 +295,8 @@ static void launch_step_q2_t(Handle *hd, const StepScalars &sc, int blk_begin, i
     p.sc = Sc<T>(sc);
     p.field = nullptr;
     p.rowsum = hd->rowsum;
+    p.g8_in = reinterpret_cast<const signed char *>(hd->g[hd->cur]) + base;   // byte offsets = element offsets
+    p.g8_out = reinterpret_cast<signed char *>(hd->g[hd->cur ^ 1]) + base;
     int mode = hd->dp.kind == FEM_MAXCUT ? MODE_MAXCUT : hd->dp.kind == FEM_MAXSAT ? MODE_SAT : MODE_ISING;
     if (hd->dp.kind == FEM_ISING && hd->dp.J) {
         mode = MODE_FIELD;
@@ -301,10 +330,12 @@ void launch_prepare_q2(Handle *hd, bool wide) {
     const unsigned grid = (unsigned)ceil_div(total, kThreads);
     if (wide)
         q2_prepare_kernel<double><<<grid, kThreads, 0, hd->stream>>>(hd->hW, hd->gW[hd->cur], hd->gW[hd->cur ^ 1],
-                                                                     hd->rows * hd->Rb, hd->Rb, hd->dp.n, nb, hd->gather_disc ? 1 : 0);
+                                                                     hd->rows * hd->Rb, hd->Rb, hd->dp.n, nb, hd->gather_disc ? 1 : 0,
+                                                                     reinterpret_cast<signed char *>(hd->g[hd->cur]));
     else
         q2_prepare_kernel<float><<<grid, kThreads, 0, hd->stream>>>(hd->h, hd->g[hd->cur], hd->g[hd->cur ^ 1],
-                                                                    hd->rows * hd->Rb, hd->Rb, hd->dp.n, nb, hd->gather_disc ? 1 : 0);
+                                                                    hd->rows * hd->Rb, hd->Rb, hd->dp.n, nb, hd->gather_disc ? 1 : 0,
+                                                                     reinterpret_cast<signed char *>(hd->g[hd->cur]));
     hd->launches++;
 }
 
