@@ -32,6 +32,14 @@ struct Layout {
 
 static size_t align_up(size_t x) { return (x + 255) & ~size_t(255); }
 
+// entries per Max-SAT occurrence are padded to a power of two so that one occurrence is one aligned vector load
+static int occ_stride(int kmax) {
+    const int ks = std::max(1, kmax - 1);
+    int st = 1;
+    while (st < ks) st <<= 1;
+    return st;
+}
+
 struct ProblemShape {
     int64_t nnz = 0, nlits = 0, nocc = 0;
     int kmax = 0;
@@ -95,7 +103,7 @@ static Layout make_layout(const fem_problem *pb, const ProblemShape &s, int R_ca
     L.glo1 = take(s.dense ? state : 0);
     L.field = take(s.dense ? 2 * state : 0);  // fp64 in the wide phase
     L.occ_ptr = take(pb->kind == FEM_MAXSAT ? ((size_t)pb->n + 1) * 4 : 0);
-    L.occ = take((size_t)s.nocc * std::max(1, s.kmax - 1) * 4);
+    L.occ = take((size_t)s.nocc * occ_stride(s.kmax) * 4);
     L.clause_ptr = take(pb->kind == FEM_MAXSAT ? ((size_t)pb->m + 1) * 4 : 0);
     L.lits = take((size_t)s.nlits * 4);
     L.h = take(state);
@@ -292,6 +300,7 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
         const int ks = std::max(1, s.kmax - 1);
         dp.m = m;
         dp.kstride = ks;
+        const int kst = occ_stride(s.kmax);
         h_occ_ptr.assign((size_t)n + 1, 0);
         for (int c = 0; c < m; ++c) {
             for (int64_t x = pb->clause_ptr[c]; x < pb->clause_ptr[c + 1]; ++x) {
@@ -312,14 +321,14 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
             }
         }
         for (int i = 0; i < n; ++i) h_occ_ptr[(size_t)i + 1] += h_occ_ptr[i];
-        h_occ.assign((size_t)s.nocc * ks, (n << 1) | 1);  // padding: the constant-1 row, read as "p"
+        h_occ.assign((size_t)s.nocc * kst, (n << 1) | 1);  // padding: the constant-1 row, read as "p"
         std::vector<int> fill(h_occ_ptr.begin(), h_occ_ptr.end() - 1);
         for (int c = 0; c < m; ++c) {  // clause order inside each variable's list == the oracle's summation order
             const int64_t a = pb->clause_ptr[c], b = pb->clause_ptr[c + 1];
             for (int64_t x = a; x < b; ++x) {
                 const int lit = pb->lits[x];
                 const int v = (lit > 0 ? lit : -lit) - 1;
-                int *ent = h_occ.data() + (size_t)fill[v]++ * ks;
+                int *ent = h_occ.data() + (size_t)fill[v]++ * kst;
                 int k = 0;
                 for (int64_t y = a; y < b; ++y) {
                     if (y == x) continue;
@@ -340,7 +349,7 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
         dp.clause_ptr = reinterpret_cast<int *>(at(L.clause_ptr));
         dp.lits = reinterpret_cast<int *>(at(L.lits));
         hd->integral_weights = true;
-        hd->structure_bytes = 4 * ((int64_t)n + 1) + 4 * (int64_t)s.nocc * ks;
+        hd->structure_bytes = 4 * ((int64_t)n + 1) + 4 * (int64_t)s.nocc * kst;
     } else if (s.dense) {
         const int n = pb->n;
         for (int i = 0; i < n; ++i) {

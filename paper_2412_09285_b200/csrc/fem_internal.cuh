@@ -45,7 +45,7 @@ struct DevProblem {
     int64_t nnz;
     const float *J;  // dense Ising, n*n
     // Max-SAT, variable-centric: occurrences of variable i are occ_ptr[i]..occ_ptr[i+1]; occurrence o
-    // holds kstride = kmax-1 packed entries: (var << 1 | negated) of the OTHER literals of its clause,
+    // holds kstride = kmax-1 packed entries (stored with the stride padded to a power of two: 1, 2, 4 or 8 ints): (var << 1 | negated) of the OTHER literals of its clause,
     // padded with (n << 1 | 1) (the constant-1 row); bit 31 of entry 0 = own literal is positive.
     int m, kstride;
     const int *occ_ptr;

@@ -43,6 +43,12 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
     const signed char *__restrict__ gin8 = p.g8_in + blk + c;
     const bool disc = p.sc.disc != 0;  // uniform; only ever set for the sparse graph kinds
     // one neighbour row: VEC floats (exact gradient) or VEC bytes holding sgn(m_j) (manipulated gradients)
+    // row j of the gather array: one IMAD.WIDE (32 x 32 -> 64-bit product added to the base) instead of a 32-bit
+    // multiply plus a two-instruction 64-bit scale-and-add
+    const unsigned row_bytes = Rb * (unsigned)sizeof(T);
+    auto row_of = [&](unsigned j) -> const T * {
+        return reinterpret_cast<const T *>(reinterpret_cast<const char *>(gin) + (unsigned long long)j * row_bytes);
+    };
     auto gather = [&](unsigned j) -> R {
         if ((MODE == MODE_MAXCUT || MODE == MODE_ISING) && disc) {
             int b[VEC];
@@ -52,7 +58,7 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
             for (int v = 0; v < VEC; ++v) r.v[v] = (T)b[v];
             return r;
         }
-        return R::ld(gin + j * Rb);
+        return R::ld(row_of(j));
     };
 
     // static structure first (legal before pdl_wait), then everything the previous step wrote
@@ -113,18 +119,36 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
         const int o0 = __ldg(p.dp.occ_ptr + i), o1 = __ldg(p.dp.occ_ptr + i + 1);
         const unsigned pad = ((unsigned)p.dp.n << 1) | 1u;  // the constant-1 row, "negated": factor 0.5 + 0.5*1 = 1
         for (int o = o0; o < o1; o += B) {
-            unsigned pk[B][KS];
+            // one occurrence = KST entries (KS padded to a power of two): one aligned 4-, 8- or 16-byte load
+            constexpr int KST = KS <= 1 ? 1 : (KS <= 2 ? 2 : (KS <= 4 ? 4 : 8));
+            unsigned pk[B][KST];
 #pragma unroll
             for (int b = 0; b < B; ++b) {
-                const int *__restrict__ ent = p.dp.occ + (unsigned)(o + b) * (unsigned)KS;
+                const int *__restrict__ ent = p.dp.occ + (unsigned)(o + b) * (unsigned)KST;
+                if (o + b < o1) {
+                    if constexpr (KST == 1) {
+                        pk[b][0] = (unsigned)__ldg(ent);
+                    } else if constexpr (KST == 2) {
+                        const int2 t = __ldg(reinterpret_cast<const int2 *>(ent));
+                        pk[b][0] = (unsigned)t.x; pk[b][1] = (unsigned)t.y;
+                    } else {
 #pragma unroll
-                for (int x = 0; x < KS; ++x) pk[b][x] = (o + b < o1) ? (unsigned)__ldg(ent + x) : pad;
+                        for (int x4 = 0; x4 < KST / 4; ++x4) {
+                            const int4 t = __ldg(reinterpret_cast<const int4 *>(ent) + x4);
+                            pk[b][4 * x4] = (unsigned)t.x; pk[b][4 * x4 + 1] = (unsigned)t.y;
+                            pk[b][4 * x4 + 2] = (unsigned)t.z; pk[b][4 * x4 + 3] = (unsigned)t.w;
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int x = 0; x < KST; ++x) pk[b][x] = pad;
+                }
             }
             R mr[B][KS];
 #pragma unroll
             for (int b = 0; b < B; ++b)
 #pragma unroll
-                for (int x = 0; x < KS; ++x) mr[b][x] = R::ld(gin + ((pk[b][x] & 0x7fffffffu) >> 1) * Rb);
+                for (int x = 0; x < KS; ++x) mr[b][x] = R::ld(row_of((pk[b][x] & 0x7fffffffu) >> 1));
 #pragma unroll
             for (int b = 0; b < B; ++b) {
                 T prod[VEC];
