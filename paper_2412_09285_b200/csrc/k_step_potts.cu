@@ -37,13 +37,18 @@ struct PottsParams {
     unsigned row_len;    // q * Rb
 };
 
+__device__ __forceinline__ long long fixed_of(float x, float scale) { return __float2ll_rn(x * scale); }
+__device__ __forceinline__ long long fixed_of(double x, double scale) { return __double2ll_rn(x * scale); }
 __device__ __forceinline__ float shfl_any(float v, int src) { return __shfl_sync(0xffffffffu, v, src); }
 __device__ __forceinline__ double shfl_any(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
 
 constexpr int kGatherChunk = 5;  // neighbour rows in flight per lane
 
-template <typename T, int QPAD, int VEC, bool STEP, bool DISC>
-__global__ void __launch_bounds__(kThreads, DISC ? 3 : 4) potts_team_kernel(const PottsParams<T> p) {
+#ifndef POTTS_EXACT_MIN
+#define POTTS_EXACT_MIN 4
+#endif
+template <typename T, int QPAD, int VEC, bool STEP, bool DISC, bool UNITW>
+__global__ void __launch_bounds__(kThreads, DISC ? 3 : POTTS_EXACT_MIN) potts_team_kernel(const PottsParams<T> p) {
     using R = Row<T, VEC>;
     constexpr int kStages = QPAD == 32 ? 5 : QPAD == 16 ? 4 : QPAD == 8 ? 3 : QPAD == 4 ? 2 : 1;
     __shared__ unsigned long long cta_sum[32 * VEC];
@@ -73,6 +78,7 @@ __global__ void __launch_bounds__(kThreads, DISC ? 3 : 4) potts_team_kernel(cons
     const T *__restrict__ gin = p.a.g_in + blk + lo;
     const Sc<T> &sc = p.sc;
     const T inv_q = (T)1 / (T)q;
+    const T fx_scale_t = (T)p.fx_scale;
     const T neg_big = (T)-3.0e38;
     const int warps_total = gridDim.x * (kThreads / 32);
     const int warp_id = blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5);
@@ -108,32 +114,6 @@ __global__ void __launch_bounds__(kThreads, DISC ? 3 : 4) potts_team_kernel(cons
             for (int v = 0; v < VEC; ++v) h[v] = ok ? r.v[v] : neg_big;
         }
         if (STEP) {
-            unsigned own_ids = 0;
-            if (DISC && ok) own_ids = ld_bytes_packed<VEC>(p.g8_in + blk + (int64_t)i * p.a.Rb + (unsigned)rl * VEC);
-            // softmax of h(t) across the team's states
-            T P[VEC], own[VEC];  // own: what the balance term subtracts (P_i, or the centred one-hot e_i when manipulated)
-#pragma unroll
-            for (int v = 0; v < VEC; ++v) {
-                T mx = h[v];
-#pragma unroll
-                for (int k = 0; k < kStages; ++k) mx = fmax(mx, shfl_any(mx, partner[k]));
-                const T e = ok ? fexp(h[v] - mx) : (T)0;
-                T z = e;
-#pragma unroll
-                for (int k = 0; k < kStages; ++k) z += shfl_any(z, partner[k]);
-                P[v] = e * frcp(z);
-                own[v] = P[v];
-                // manipulated: the variable's own one-hot vector is the state id the previous launch stored for it
-                if (DISC) own[v] = ((((own_ids >> (8 * v)) & 0xffu) == (unsigned)s) ? (T)1 : (T)0) - inv_q;
-            }
-            // manipulated gradients (S27, PAPER.md:640-644): c^f = q / sum_j W_ij on the cut term, lambda c^a with
-            // c^a = q / sqrt(sum_j W_ij) on the balance term (S26's 2 lambda becomes lambda); no neighbours: 0
-            T cf = (T)1, lam_c = sc.two_lambda;
-            if (DISC) {
-                const double rs = ok ? __ldg(p.rowsum + i) : 0.0;
-                cf = rs > 0.0 ? (T)((double)q / rs) : (T)0;
-                lam_c = rs > 0.0 ? (T)(0.5 * (double)sc.two_lambda * ((double)q / sqrt(rs))) : (T)0;
-            }
             // coupling contraction f(s) = sum_j W_ij D_j(s): kGatherChunk neighbour rows in flight
             T f[VEC];
 #pragma unroll
@@ -160,7 +140,7 @@ __global__ void __launch_bounds__(kThreads, DISC ? 3 : 4) potts_team_kernel(cons
                         for (int k = 0; k < kIds; ++k) {
                             const bool in = e + k < e1;
                             jj[k] = in ? (unsigned)__ldg(p.dp.col + e + k) : (unsigned)i;
-                            ww[k] = in ? (p.dp.w ? (T)__ldg(p.dp.w + e + k) : (T)1) : (T)0;
+                            ww[k] = in ? (UNITW ? (T)1 : (T)__ldg(p.dp.w + e + k)) : (T)0;
                         }
 #pragma unroll
                         for (int k = 0; k < kIds; ++k) ids[k] = ld_bytes_packed<VEC>(gin8 + jj[k] * (unsigned)p.a.Rb);
@@ -173,6 +153,25 @@ __global__ void __launch_bounds__(kThreads, DISC ? 3 : 4) potts_team_kernel(cons
 #pragma unroll
                     for (int v = 0; v < VEC; ++v) f[v] -= shift;
                 } else {
+                const unsigned row_bytes = p.row_len * (unsigned)sizeof(T);
+                auto row_of = [&](unsigned j) -> const T * {  // one wide multiply-add per neighbour row
+                    return reinterpret_cast<const T *>(reinterpret_cast<const char *>(gin) + (unsigned long long)j * row_bytes);
+                };
+                if (UNITW && (e1 - e0) % kGatherChunk == 0) {
+                    // unit weights, whole chunks (10-regular graphs): indices, then kGatherChunk rows in flight, then adds
+                    for (int e = e0; e < e1; e += kGatherChunk) {
+                        unsigned jj[kGatherChunk];
+                        R nb[kGatherChunk];
+#pragma unroll
+                        for (int k = 0; k < kGatherChunk; ++k) jj[k] = (unsigned)__ldg(p.dp.col + e + k);
+#pragma unroll
+                        for (int k = 0; k < kGatherChunk; ++k) nb[k] = R::ld(row_of(jj[k]));
+#pragma unroll
+                        for (int k = 0; k < kGatherChunk; ++k)
+#pragma unroll
+                            for (int v = 0; v < VEC; ++v) f[v] += nb[k].v[v];  // == fma(1, D_j, f)
+                    }
+                } else {
                 for (int e = e0; e < e1; e += kGatherChunk) {
                     unsigned jj[kGatherChunk];
                     T ww[kGatherChunk];
@@ -181,16 +180,43 @@ __global__ void __launch_bounds__(kThreads, DISC ? 3 : 4) potts_team_kernel(cons
                     for (int k = 0; k < kGatherChunk; ++k) {
                         const bool in = e + k < e1;
                         jj[k] = in ? (unsigned)__ldg(p.dp.col + e + k) : (unsigned)i;
-                        ww[k] = in ? (p.dp.w ? (T)__ldg(p.dp.w + e + k) : (T)1) : (T)0;
+                        ww[k] = in ? (UNITW ? (T)1 : (T)__ldg(p.dp.w + e + k)) : (T)0;
                     }
 #pragma unroll
-                    for (int k = 0; k < kGatherChunk; ++k) nb[k] = R::ld(gin + jj[k] * p.row_len);
+                    for (int k = 0; k < kGatherChunk; ++k) nb[k] = R::ld(row_of(jj[k]));
 #pragma unroll
                     for (int k = 0; k < kGatherChunk; ++k)
 #pragma unroll
-                        for (int v = 0; v < VEC; ++v) f[v] += ww[k] * nb[k].v[v];
+                        for (int v = 0; v < VEC; ++v) f[v] = fma(ww[k], nb[k].v[v], f[v]);
                 }
                 }
+                }
+            }
+            unsigned own_ids = 0;
+            if (DISC && ok) own_ids = ld_bytes_packed<VEC>(p.g8_in + blk + (int64_t)i * p.a.Rb + (unsigned)rl * VEC);
+            // softmax of h(t) across the team's states
+            T P[VEC], own[VEC];  // own: what the balance term subtracts (P_i, or the centred one-hot e_i when manipulated)
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) {
+                T mx = h[v];
+#pragma unroll
+                for (int k = 0; k < kStages; ++k) mx = fmax(mx, shfl_any(mx, partner[k]));
+                const T e = ok ? fexp(h[v] - mx) : (T)0;
+                T z = e;
+#pragma unroll
+                for (int k = 0; k < kStages; ++k) z += shfl_any(z, partner[k]);
+                P[v] = e * frcp(z);
+                own[v] = P[v];
+                // manipulated: the variable's own one-hot vector is the state id the previous launch stored for it
+                if (DISC) own[v] = ((((own_ids >> (8 * v)) & 0xffu) == (unsigned)s) ? (T)1 : (T)0) - inv_q;
+            }
+            // manipulated gradients (S27, PAPER.md:640-644): c^f = q / sum_j W_ij on the cut term, lambda c^a with
+            // c^a = q / sqrt(sum_j W_ij) on the balance term (S26's 2 lambda becomes lambda); no neighbours: 0
+            T cf = (T)1, lam_c = sc.two_lambda;
+            if (DISC) {
+                const double rs = ok ? __ldg(p.rowsum + i) : 0.0;
+                cf = rs > 0.0 ? (T)((double)q / rs) : (T)0;
+                lam_c = rs > 0.0 ? (T)(0.5 * (double)sc.two_lambda * ((double)q / sqrt(rs))) : (T)0;
             }
             // g^p (S26), then g^h = P (g^p - <g^p>_P) (S20), Adam
             R m1 = {}, m2 = {}, hn;
@@ -241,7 +267,8 @@ __global__ void __launch_bounds__(kThreads, DISC ? 3 : 4) potts_team_kernel(cons
                 win[v] = winner(h[v], mx, ok);
                 po.v[v] = (win[v] == s ? (T)1 : (T)0) - inv_q;
             }
-            if (ok) colacc[v] += __double2ll_rn((double)po.v[v] * p.fx_scale);
+            // fixed point straight from the compute type: the scale is a power of two, so the product is exact
+            if (ok) colacc[v] += fixed_of(po.v[v], fx_scale_t);
         }
         if (DISC) {  // the state-0 lane of each replica group stores the VEC winners as bytes
             if (ok && s == 0) st_bytes<VEC>(p.g8_out + blk + (int64_t)i * p.a.Rb + (unsigned)rl * VEC, win);
@@ -266,19 +293,25 @@ __global__ void __launch_bounds__(kThreads, DISC ? 3 : 4) potts_team_kernel(cons
 }
 
 // grid-stride kernel: never more CTAs than are resident at once (occupancy x SMs), so no second wave
-template <typename T, int QPAD, int VEC, bool STEP, bool DISC>
-static void launch_potts_one(Handle *hd, const PottsParams<T> &p, dim3 grid) {
+template <typename T, int QPAD, int VEC, bool STEP, bool DISC, bool UNITW>
+static void launch_potts_w(Handle *hd, const PottsParams<T> &p, dim3 grid) {
     static std::map<int, int> resident;  // per device SM count: CTAs resident at once for THIS instantiation
     int &r = resident[hd->sm_count];
     if (r == 0) {
         int occ = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, potts_team_kernel<T, QPAD, VEC, STEP, DISC>, kThreads, 0) !=
-                cudaSuccess || occ < 1)
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, potts_team_kernel<T, QPAD, VEC, STEP, DISC, UNITW>, kThreads,
+                                                          0) != cudaSuccess || occ < 1)
             occ = 1;
         r = occ * hd->sm_count;
     }
     grid.x = std::min<unsigned>(grid.x, (unsigned)r);
-    launch_pdl(potts_team_kernel<T, QPAD, VEC, STEP, DISC>, grid, dim3(kThreads), hd->stream, p);
+    launch_pdl(potts_team_kernel<T, QPAD, VEC, STEP, DISC, UNITW>, grid, dim3(kThreads), hd->stream, p);
+}
+
+template <typename T, int QPAD, int VEC, bool STEP, bool DISC>
+static void launch_potts_one(Handle *hd, const PottsParams<T> &p, dim3 grid) {
+    if (p.dp.w) launch_potts_w<T, QPAD, VEC, STEP, DISC, false>(hd, p, grid);
+    else launch_potts_w<T, QPAD, VEC, STEP, DISC, true>(hd, p, grid);
 }
 
 template <typename T, int QPAD, int VEC>
