@@ -1,0 +1,137 @@
+"""GPU parity on the degenerate and extreme inputs of the path: empty and one-node graphs, isolated nodes, a star
+(one row of degree n-1), q = 2 and q = 32 Potts, clause lengths 1..8 mixed, a single replica, fewer replicas than
+the handle was created for, zero annealing steps.  Same bars as tests/test_gpu_parity.py."""
+import numpy as np
+import pytest
+
+from oracle import fem_oracle as fo
+from paper_2412_09285_b200 import workloads as wl
+from test_oracle_gradient import as_problem
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def fem():
+    from paper_2412_09285_b200 import fem as femlib
+    return femlib
+
+
+def _csr(n, edges, weights=None):
+    """Symmetric CSR from an undirected edge list."""
+    adj = [[] for _ in range(n)]
+    for k, (a, b) in enumerate(edges):
+        w = 1.0 if weights is None else weights[k]
+        adj[a].append((b, w))
+        adj[b].append((a, w))
+    row_ptr, col, wt = [0], [], []
+    for i in range(n):
+        for j, w in sorted(adj[i]):
+            col.append(j)
+            wt.append(w)
+        row_ptr.append(len(col))
+    return (np.array(row_ptr, np.int64), np.array(col, np.int32),
+            None if weights is None else np.array(wt, np.float32))
+
+
+def _graph(kind, n, edges, q=2, weights=None, lam=0.0):
+    rp, ci, w = _csr(n, edges, weights)
+    return wl.Instance(kind, n, q, rp, ci, w, lam=lam, name=f"edge_{kind}_{n}")
+
+
+def _mixed_sat(n, seed):
+    """Clauses of every length 1..8 (the ABI's range), distinct variables inside a clause."""
+    rng = np.random.default_rng(seed)
+    ptr, lits = [0], []
+    for k in list(range(1, 9)) * 6:
+        vs = rng.choice(n, size=k, replace=False) + 1
+        lits += [int(v if rng.random() < 0.5 else -v) for v in vs]
+        ptr.append(len(lits))
+    return wl.Instance(wl.MAXSAT, n, 2, m=len(ptr) - 1, clause_ptr=np.array(ptr, np.int64),
+                       lits=np.array(lits, np.int32), name="sat_mixed_k1to8")
+
+
+def cases():
+    rng = np.random.default_rng(0)
+    star = [(0, j) for j in range(1, 1500)]
+    ring = [(i, (i + 1) % 40) for i in range(40)]
+    return {
+        "one_node_no_edges": (_graph(wl.MAXCUT, 1, []), 3),
+        "empty_graph": (_graph(wl.MAXCUT, 37, []), 5),
+        "isolated_nodes": (_graph(wl.MAXCUT, 50, [(0, 1), (1, 2), (7, 9)], weights=[1.0, -2.0, 3.0]), 1),
+        "star_degree_1499": (_graph(wl.MAXCUT, 1500, star), 6),
+        "ising_two_spins": (_graph(wl.ISING, 2, [(0, 1)], weights=[0.75]), 4),
+        "potts_q2_ring": (_graph(wl.BMINCUT, 40, ring, q=2, lam=0.05), 8),
+        "potts_q32_ring": (_graph(wl.BMINCUT, 40, ring, q=32, lam=0.02), 3),
+        "potts_q7_isolated": (_graph(wl.BMINCUT, 30, [(0, 1), (2, 3)], q=7, lam=0.1), 5),
+        "sat_mixed_k1to8": (_mixed_sat(60, 5), 7),
+        "sat_unit_clauses_only": (wl.Instance(wl.MAXSAT, 5, 2, m=4, clause_ptr=np.array([0, 1, 2, 3, 4], np.int64),
+                                              lits=np.array([1, -2, 3, -1], np.int32), name="sat_units"), 2),
+        "dense_two_spins": (wl.Instance(wl.ISING, 2, 2, dense_J=np.array([[0, -0.4], [-0.4, 0]], np.float32),
+                                        name="dense2"), 32),
+    }
+
+
+CASES = cases()
+
+
+@pytest.mark.parametrize("manipulated", [False, True])
+@pytest.mark.parametrize("name", list(CASES))
+def test_degenerate_inputs_against_the_oracle(fem, name, manipulated):
+    inst, R = CASES[name]
+    pb = as_problem(inst)
+    beta = fem.linear_temperature_schedule(1.0, 0.05, 60)
+    h0 = fo.init_fields(4, R, inst.n, inst.fields_per_var).astype(np.float32)
+    st = fo.anneal_ex(fo.State(pb, h0.astype(np.float64)), beta, fo.Optimizer(), inst.lam, t_end=25,
+                      manipulated=manipulated, gamma=0.9)
+    P_ref = fo.marginals(pb, st.h)
+    for K, tol in ((25, 2e-7), (4, 1e-4)):
+        if manipulated and K == 4:
+            continue                                   # fp32 sgn / argmax decisions: covered step by step elsewhere
+        eng = fem.Fem(inst, R + 2)                     # more capacity than replicas in flight
+        eng.set_fields(h0)
+        eng.anneal(fem.Schedule(beta=beta, precise_steps=K, manipulated=manipulated, gamma_grad=0.9), R, stop_after=25)
+        P = eng.get_marginals().astype(np.float64)
+        assert np.max(np.abs(P - P_ref.reshape(P.shape))) < tol, (K, name)
+        res = eng.result()
+        cfg = eng.get_configs()
+        assert np.array_equal(cfg, fo.round_configs(pb, eng.get_fields().astype(np.float64)))
+        e_int, e_real, part = fo.energies(pb, cfg, inst.lam)
+        if inst.kind == wl.ISING:
+            assert np.allclose(res["energy"], e_real, rtol=1e-9, atol=1e-12)
+        else:
+            assert np.array_equal(res["energy_int"], e_int) and np.array_equal(res["energy"], e_real)
+        assert res["best_replica"] == fo.argmin(e_real)
+        eng.close()
+
+
+def test_zero_steps_reads_out_the_initial_fields(fem):
+    inst, R = CASES["potts_q7_isolated"]
+    pb = as_problem(inst)
+    eng = fem.Fem(inst, R)
+    eng.anneal(fem.Schedule(beta=fem.linear_temperature_schedule(1.0, 0.1, 10)), R, seed=11, stop_after=0)
+    h = eng.get_fields()
+    assert np.array_equal(eng.get_configs(), fo.round_configs(pb, h.astype(np.float64)))
+    P = eng.get_marginals().astype(np.float64)
+    assert np.max(np.abs(P - fo.marginals(pb, h.astype(np.float64)).reshape(P.shape))) < 2e-7
+    eng.close()
+
+
+def test_invalid_problems_are_rejected(fem):
+    ring = [(i, (i + 1) % 6) for i in range(6)]
+    good = _graph(wl.BMINCUT, 6, ring, q=3, lam=0.1)
+    for mutate in ("q33", "self_loop", "asymmetric", "negative_potts_weight", "repeated_variable"):
+        inst = good
+        if mutate == "q33":
+            inst = _graph(wl.BMINCUT, 6, ring, q=33)
+        elif mutate == "self_loop":
+            inst = wl.Instance(wl.MAXCUT, 2, 2, np.array([0, 1, 1], np.int64), np.array([0], np.int32), None)
+        elif mutate == "asymmetric":
+            inst = wl.Instance(wl.MAXCUT, 3, 2, np.array([0, 1, 1, 1], np.int64), np.array([1], np.int32), None)
+        elif mutate == "negative_potts_weight":
+            inst = _graph(wl.BMINCUT, 6, ring, q=3, weights=[1, 1, -1, 1, 1, 1])
+        elif mutate == "repeated_variable":
+            inst = wl.Instance(wl.MAXSAT, 3, 2, m=1, clause_ptr=np.array([0, 2], np.int64),
+                               lits=np.array([2, -2], np.int32))
+        with pytest.raises(fem.FemError):
+            fem.Fem(inst, 4)
