@@ -361,7 +361,9 @@ def main():
                         "kernel_share_of_step": bulk_ms / elapsed_ms}
         else:
             achieved = step_bytes / (kernel_us * 1e-6) / 1e9
-            kname = ("potts_team_kernel<float> (fused softmax + gather + balance + chain rule + Adam)"
+            kname = (("potts_tma_kernel (rows staged by cp.async.bulk one variable ahead; fused softmax + gather + balance + "
+                      "chain rule + optimiser)" if eng.info("tma_launches") > 0 else
+                      "potts_team_kernel<float> (fused softmax + gather + balance + chain rule + optimiser)")
                      if inst.kind == wl.BMINCUT else
                      "step_q2_kernel<float> (fused gather + entropy gradient + Adam)")
             roofline = {"bound": "hbm", "kernel": kname,

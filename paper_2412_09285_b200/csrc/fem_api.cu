@@ -476,6 +476,9 @@ fem_status fem_set_option(fem_handle *h, const char *key, int64_t value) {
     } else if (!strcmp(key, "persistent")) {
         if (value < 0 || value > 9) return fail(hd, FEM_EINVAL, "persistent must be 0, 1 or 1 + cluster size");
         hd->opt_persistent = value;
+    } else if (!strcmp(key, "potts_tma")) {
+        if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "potts_tma must be 0 or 1");
+        hd->opt_potts_tma = value;
     } else if (!strcmp(key, "tensor_cores")) {
         if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "tensor_cores must be 0 or 1");
         hd->opt_tensor_cores = value;
@@ -492,6 +495,7 @@ int64_t fem_get_info(const fem_handle *h, const char *key) {
     if (!strcmp(key, "tc_launches")) return hd->tc_launches;
     if (!strcmp(key, "persist_launches")) return hd->persist_launches;
     if (!strcmp(key, "persist_cluster")) return hd->persist_cluster;
+    if (!strcmp(key, "tma_launches")) return hd->tma_launches;
     if (!strcmp(key, "t_done")) return hd->t_done;
     if (!strcmp(key, "R")) return hd->R;
     if (!strcmp(key, "replica_block")) return hd->Rb;

@@ -229,8 +229,9 @@ __global__ void __launch_bounds__(kThreads, DISC ? 3 : POTTS_EXACT_MIN) potts_te
             for (int v = 0; v < VEC; ++v) {
                 T gp = (T)0;
                 if (ok) {
-                    if (DISC) gp = -(cf * f[v]) + lam_c * (Ss[v] - own[v]) + h[v] * sc.inv_beta;
-                    else gp = -f[v] + sc.two_lambda * (Ss[v] - P[v]) + h[v] * sc.inv_beta;
+                    // explicit fma: potts_tma_kernel must round exactly alike
+                    if (DISC) gp = fma(h[v], sc.inv_beta, fma(lam_c, Ss[v] - own[v], -(cf * f[v])));
+                    else gp = fma(h[v], sc.inv_beta, fma(sc.two_lambda, Ss[v] - P[v], -f[v]));
                 }
                 T gbar = P[v] * gp;
 #pragma unroll
@@ -262,7 +263,7 @@ __global__ void __launch_bounds__(kThreads, DISC ? 3 : POTTS_EXACT_MIN) potts_te
             T z = e;
 #pragma unroll
             for (int k = 0; k < kStages; ++k) z += shfl_any(z, partner[k]);
-            po.v[v] = e * frcp(z) - inv_q;
+            po.v[v] = fma(e, frcp(z), -inv_q);
             if (DISC) {
                 win[v] = winner(h[v], mx, ok);
                 po.v[v] = (win[v] == s ? (T)1 : (T)0) - inv_q;
@@ -331,6 +332,8 @@ static void launch_potts_v(Handle *hd, const PottsParams<T> &p, dim3 grid, bool 
     else launch_potts_t<T, QPAD, 1>(hd, p, grid, step);
 }
 
+bool launch_potts_tma(Handle *hd, const StepScalars &sc, int blk_begin, int blk_count);  // k_step_potts_tma.cu
+
 int potts_qpad(int q) {
     int qp = 2;
     while (qp < q) qp <<= 1;
@@ -393,6 +396,7 @@ void launch_potts(Handle *hd, const StepScalars &sc, bool wide, bool step, int b
         const size_t bytes = (size_t)hd->dp.q * hd->Rb * blk_count * sizeof(long long);
         cudaMemsetAsync(hd->colsum[sc.t % 3] + (int64_t)blk_begin * hd->dp.q * hd->Rb, 0, bytes, hd->stream);
     }
+    if (!wide && step && launch_potts_tma(hd, sc, blk_begin, blk_count)) return;  // TMA-staged fast path where it applies
     if (wide) launch_potts_typed<double>(hd, sc, step, blk_begin, blk_count);
     else launch_potts_typed<float>(hd, sc, step, blk_begin, blk_count);
 }

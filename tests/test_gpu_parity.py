@@ -303,3 +303,31 @@ def test_persistent_kernel_bit_identical_to_stepwise(fem, name, mode):
             assert np.array_equal(a[k], b[k]), (persistent, k)
         assert np.array_equal(a[3][0], b[3][0]) and np.array_equal(a[3][1], b[3][1])
         assert np.array_equal(a[4]["energy"], b[4]["energy"]) and a[4]["best_replica"] == b[4]["best_replica"]
+
+
+@pytest.mark.parametrize("case", ["q8_reg10_R16", "q8_reg10_R32_two_blocks", "q4_reg6_weighted_R32", "q32_reg16_R4", "q2_reg3_R64"])
+def test_potts_tma_bit_identical_to_team_kernel(fem, case):
+    """The TMA-staged Potts step (rows fetched one variable ahead into a shared-memory ring) against the register
+    path: same arithmetic, so fields, moments, energies must be bit-identical; the counter proves which one ran."""
+    q, d, R, rb, weighted = {"q8_reg10_R16": (8, 10, 16, 0, False), "q8_reg10_R32_two_blocks": (8, 10, 32, 16, False),
+                             "q4_reg6_weighted_R32": (4, 6, 32, 0, True), "q32_reg16_R4": (32, 16, 4, 0, False),
+                             "q2_reg3_R64": (2, 3, 64, 0, False)}[case]
+    inst = wl.random_regular(1201 if d % 2 == 0 else 1200, d, 2020 + q, wl.BMINCUT, q, lam=0.03)
+    if weighted:
+        w = np.random.default_rng(3).integers(1, 5, inst.nnz // 2).astype(np.float32)[edge_ids(inst)]
+        inst = wl.Instance(wl.BMINCUT, inst.n, q, inst.row_ptr, inst.col_idx, w, lam=0.03)
+    sch = fem.Schedule(beta=fem.linear_temperature_schedule(1.0, 0.05, 40), precise_steps=4)
+    out = {}
+    for tma in (1, 0):
+        eng = fem.Fem(inst, R)
+        eng.set_option("potts_tma", tma)
+        if rb:
+            eng.set_option("replica_block", rb)
+        eng.anneal(sch, R, seed=8, stop_after=17)
+        eng.anneal(sch, R, seed=8, stop_after=40)
+        out[tma] = (eng.get_fields(), eng.get_moments(), eng.result())
+        assert eng.info("tma_launches") == (36 * (R // rb if rb else 1) if tma else 0)   # 40 steps - 4 wide ones, per block
+        eng.close()
+    assert np.array_equal(out[1][0], out[0][0])
+    assert np.array_equal(out[1][1][0], out[0][1][0]) and np.array_equal(out[1][1][1], out[0][1][1])
+    assert np.array_equal(out[1][2]["energy"], out[0][2]["energy"])
