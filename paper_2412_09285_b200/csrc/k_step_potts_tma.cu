@@ -11,7 +11,8 @@
 // only then does the softmax / chain rule / optimiser work, which covers the fetch.  The bytes in flight live in
 // shared memory, not in registers: 64 registers per thread, four CTAs (32 warps, 32 slots of 6.5 KB) per SM.
 // Measured on cfg 2: 116 us (register path) -> 101 us; a two-stage ring at 2 CTAs per SM gave 117 us
-// (too few warps to cover the ALU latency), per-lane cp.async (LDGSTS) staging instead of bulk copies 105 us.  The column indices are read two variables ahead (one per lane, handed to the issuing lanes by a shuffle).
+// (too few warps to cover the ALU latency), per-lane cp.async (LDGSTS) staging instead of bulk copies 105 us, L2
+// cache hints on the bulk copies (evict-first own rows + evict-last neighbour rows 122 us, evict-first alone 101 us).  The column indices are read two variables ahead (one per lane, handed to the issuing lanes by a shuffle).
 //
 // The arithmetic is potts_team_kernel's, instruction for instruction (same device functions, same CSR-order sum),
 // so the two kernels are bit-identical (tests/test_gpu_parity.py::test_potts_tma_bit_identical).  Rows a1-a4 of
