@@ -254,6 +254,9 @@ def main():
         """The whole hot path on resident inputs; `ev` collects (start, end) events around the fp32 bulk."""
         flush.zero_()
         eng.reset()
+        if ev is not None:
+            z = torch.cuda.Event(enable_timing=True)
+            z.record()
         eng.anneal(sched, R, seed=seed, stop_after=K)          # init + wide phase
         if ev is not None:
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -262,8 +265,11 @@ def main():
         eng.anneal(sched, R, seed=seed, stop_after=N)          # launches of the fused fp32 step kernel (+1 narrowing)
         if ev is not None:
             b.record()
-            ev.append((a, b, eng.info("launches") - l0 - (1 if K > 0 else 0)))
         eng.readout()                                          # rounding + energies + argmin
+        if ev is not None:
+            c = torch.cuda.Event(enable_timing=True)
+            c.record()
+            ev.append((a, b, eng.info("launches") - l0 - (1 if K > 0 else 0), z, c))
 
     sampler = ClockSampler(local_rank) if rank == 0 else None   # started before warm-up: nvidia-smi takes a while to start
     for w in range(args.warmup):
@@ -283,8 +289,10 @@ def main():
     clocks = sampler.stop(wall_begin, wall_end) if sampler else None
     launches = eng.info("launches") - launches0
     res = eng.result()
-    bulk_ms = sum(a.elapsed_time(b) for a, b, _ in bulk_events)
-    bulk_launches = sum(c for _, _, c in bulk_events)
+    bulk_ms = sum(e[0].elapsed_time(e[1]) for e in bulk_events)
+    bulk_launches = sum(e[2] for e in bulk_events)
+    init_wide_ms = sum(e[3].elapsed_time(e[0]) for e in bulk_events) / max(len(bulk_events), 1)
+    readout_ms = sum(e[1].elapsed_time(e[4]) for e in bulk_events) / max(len(bulk_events), 1)
     # algorithmic bytes of one launch: the whole step's bytes spread over the launches that make up a step
     step_bytes = eng.info("step_bytes") * (N - K) * args.steps / max(bulk_launches, 1)
 
@@ -388,6 +396,9 @@ def main():
                     "d2h_bytes_per_step": d2h, "steps": e2e_steps},
             "gpu_launches": int(launches),
             "clocks": clocks,
+            "breakdown_ms_per_pass": {"init_and_wide_phase": init_wide_ms, "fp32_steps": bulk_ms / max(len(bulk_events), 1),
+                                      "readout": readout_ms, "note": "rank 0, CUDA events; the rest of ms_per_step is the L2 flush"},
+            **({"field_updates_per_s": value * inst.q} if inst.kind == wl.BMINCUT else {}),
             "result": {"best_energy": best_energy, "best_rank": best_owner, "mean_energy": float(np.mean(res["energy"]))},
         }
         if not args.no_cpu_baseline and world == 1:

@@ -147,7 +147,7 @@ static fem_status fail(Handle *hd, fem_status st, const char *msg) {
 }
 
 // Validate the symmetric CSR and report whether all weights are integral.
-static bool validate_graph(const fem_problem *pb, int64_t nnz, bool *integral, int *uniform_deg, std::string *err) {
+static bool validate_graph(const fem_problem *pb, int64_t nnz, bool *integral, int *uniform_deg, int *max_deg, std::string *err) {
     const int n = pb->n;
     *integral = true;
     int64_t d0 = pb->row_ptr[1] - pb->row_ptr[0];
@@ -176,6 +176,9 @@ static bool validate_graph(const fem_problem *pb, int64_t nnz, bool *integral, i
             if (pb->weight && pb->weight[it - pb->col_idx] != pb->weight[e]) return *err = "weights are not symmetric", false;
         }
     *uniform_deg = (uniform && d0 > 0 && d0 <= 64) ? (int)d0 : 0;
+    int64_t mx = 0;
+    for (int i = 0; i < n; ++i) mx = std::max<int64_t>(mx, pb->row_ptr[i + 1] - pb->row_ptr[i]);
+    *max_deg = (int)std::min<int64_t>(mx, 1 << 30);
     return true;
 }
 
@@ -374,7 +377,7 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
         hd->integral_weights = false;
         hd->structure_bytes = 4 * (int64_t)n * n;
     } else {
-        if (!validate_graph(pb, s.nnz, &hd->integral_weights, &dp.uniform_deg, &err)) {
+        if (!validate_graph(pb, s.nnz, &hd->integral_weights, &dp.uniform_deg, &dp.max_deg, &err)) {
             delete hd;
             return fail(nullptr, FEM_EINVAL, err.c_str());
         }

@@ -42,6 +42,7 @@ struct DevProblem {
     const int *col;      // [nnz]
     const float *w;      // [nnz] or nullptr (= +1)
     int uniform_deg;     // > 0 when every row has this many entries
+    int max_deg;         // longest row
     int64_t nnz;
     const float *J;  // dense Ising, n*n
     // Max-SAT, variable-centric: occurrences of variable i are occ_ptr[i]..occ_ptr[i+1]; occurrence o

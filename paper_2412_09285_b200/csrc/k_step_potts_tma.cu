@@ -1,4 +1,4 @@
-// Potts (balanced minimum cut) step with the memory side on the TMA: fp32, exact gradient, uniform degree <= 16,
+// Potts (balanced minimum cut) step with the memory side on the TMA: fp32, exact gradient, every degree <= 16,
 // one variable per warp (q * Rb / 4 == 32 lanes, q a power of two) -- BASELINE.json configs[2].
 //
 // Why: ncu on potts_team_kernel (profiles/r01_cfg2_step.md) shows nothing saturated -- DRAM 49%, issue ~50% -- with
@@ -36,7 +36,10 @@ struct PottsTmaParams {
     const long long *S_in;
     long long *S_out, *S_zero;
     double fx_scale, fx_inv;
-    int n, q, Rb, deg;
+    int n, q, Rb;
+    int deg;              // uniform degree, or 0: rows from row_ptr, at most max_deg entries each
+    int max_deg;          // rows of the slot reserved for neighbours
+    const int *row_ptr;
     unsigned row_len;     // q * Rb floats = 128 (one float4 per lane)
 };
 
@@ -80,7 +83,7 @@ __global__ void __launch_bounds__(kTmaWarps * 32, 4) potts_tma_kernel(const __gr
     __shared__ __align__(8) uint64_t full_bar[kTmaWarps];
     __shared__ unsigned long long cta_sum[32 * VEC];
     pdl_trigger();
-    const int n = p.n, deg = p.deg;
+    const int n = p.n;
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const int s = lane / lps, rl = lane - s * lps;
     int partner[kStages];
@@ -93,7 +96,7 @@ __global__ void __launch_bounds__(kTmaWarps * 32, 4) potts_tma_kernel(const __gr
     const float fx_scale_t = (float)p.fx_scale;
     const int warps_total = gridDim.x * kTmaWarps;
     const int warp_gid = blockIdx.x * kTmaWarps + wib;
-    const int rows = 3 + deg;
+    const int rows = 3 + p.max_deg;  // slot capacity
     const uint32_t row_bytes = 128 * sizeof(float);
     float *my_ring = ring + (size_t)wib * rows * 128;
     uint64_t *bar = &full_bar[wib];
@@ -121,25 +124,39 @@ __global__ void __launch_bounds__(kTmaWarps * 32, 4) potts_tma_kernel(const __gr
 
     // fetch of variable `i` into stage `st`: lane 0 posts the byte count, lanes 0..2 copy the h, m1, m2 rows,
     // lanes 3..3+deg-1 the neighbour rows (lane 3+k holds column index k after the shuffle)
-    auto issue = [&](int i, int col_lane) {
+    auto issue = [&](int i, int col_lane, int d) {
         const int c = __shfl_sync(0xffffffffu, col_lane, lane >= 3 ? lane - 3 : 0);
         float *dst = my_ring + (size_t)lane * 128;
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // the slot was read through the generic proxy
-        if (lane == 0) mbar_expect_tx(bar, (uint32_t)rows * row_bytes);
+        if (lane == 0) mbar_expect_tx(bar, (uint32_t)(3 + d) * row_bytes);
         __syncwarp();
         const int64_t own = blk + (int64_t)i * 128;
         if (lane == 0) bulk_g2s(dst, p.h + own, row_bytes, bar);
         else if (lane == 1) bulk_g2s(dst, p.m1 + own, row_bytes, bar);
         else if (lane == 2) bulk_g2s(dst, p.m2 + own, row_bytes, bar);
-        else if (lane < rows) bulk_g2s(dst, p.g_in + blk + (int64_t)(unsigned)c * 128, row_bytes, bar);
+        else if (lane < 3 + d) bulk_g2s(dst, p.g_in + blk + (int64_t)(unsigned)c * 128, row_bytes, bar);
     };
-    auto load_col = [&](int i) -> int { return (i < n && lane < deg) ? __ldg(p.col + (int64_t)i * deg + lane) : 0; };
+    // CSR row of variable i: first entry e0, degree d (warp-uniform), this lane's column index
+    auto load_row = [&](int i, int &e0, int &d) -> int {
+        e0 = 0;
+        d = 0;
+        if (i >= n) return 0;
+        if (p.deg > 0) {
+            e0 = i * p.deg;
+            d = p.deg;
+        } else {
+            e0 = __ldg(p.row_ptr + i);
+            d = __ldg(p.row_ptr + i + 1) - e0;
+        }
+        return lane < d ? __ldg(p.col + e0 + lane) : 0;
+    };
 
     int i = warp_gid;
-    int col_next = 0;
+    int e0 = 0, deg = 0, e0_next = 0, deg_next = 0, col_next = 0;
     if (i < n) {
-        issue(i, load_col(i));
-        col_next = load_col(i + warps_total);
+        const int c0 = load_row(i, e0, deg);
+        issue(i, c0, deg);
+        col_next = load_row(i + warps_total, e0_next, deg_next);
     }
     for (int t = 0; i < n; ++t, i += warps_total) {
         const int in = i + warps_total;
@@ -156,7 +173,7 @@ __global__ void __launch_bounds__(kTmaWarps * 32, 4) potts_tma_kernel(const __gr
             if (UNITW) {
                 f[0] += nb.x; f[1] += nb.y; f[2] += nb.z; f[3] += nb.w;  // == fma(1, D_j, f)
             } else {
-                const float ww = __ldg(p.w + (int64_t)i * deg + k);
+                const float ww = __ldg(p.w + e0 + k);
                 f[0] = fma(ww, nb.x, f[0]); f[1] = fma(ww, nb.y, f[1]); f[2] = fma(ww, nb.z, f[2]); f[3] = fma(ww, nb.w, f[3]);
             }
         }
@@ -172,9 +189,12 @@ __global__ void __launch_bounds__(kTmaWarps * 32, 4) potts_tma_kernel(const __gr
         }
         // the slot is in registers now: refill it with the warp's next variable while this one is computed
         __syncwarp();
+        const int deg_issue = deg_next;
+        e0 = e0_next;   // (the neighbour sum above is done with this variable's row)
+        deg = deg_next;
         if (in < n) {
-            issue(in, col_next);
-            col_next = load_col(in + warps_total);
+            issue(in, col_next, deg_issue);
+            col_next = load_row(in + warps_total, e0_next, deg_next);
         }
         // softmax of h(t) across the states
         float P[VEC];
@@ -236,10 +256,10 @@ __global__ void __launch_bounds__(kTmaWarps * 32, 4) potts_tma_kernel(const __gr
 
 // ---- host side ----
 bool potts_tma_applicable(const Handle *hd) {
-    const int q = hd->dp.q, Rb = hd->Rb, deg = hd->dp.uniform_deg;
+    const int q = hd->dp.q, Rb = hd->Rb, deg = hd->dp.max_deg;
     if (hd->opt_potts_tma == 0 || hd->gather_disc) return false;
     if (q < 2 || (q & (q - 1)) != 0 || Rb % 4 != 0 || q * (Rb / 4) != 32) return false;  // one variable = one warp of float4 lanes
-    return deg >= 1 && deg <= kTmaMaxDeg;
+    return deg >= 1 && deg <= kTmaMaxDeg && hd->dp.nnz < ((int64_t)1 << 31);
 }
 
 template <int QPAD, bool UNITW>
@@ -296,8 +316,10 @@ bool launch_potts_tma(Handle *hd, const StepScalars &sc, int blk_begin, int blk_
     p.q = q;
     p.Rb = Rb;
     p.deg = hd->dp.uniform_deg;
+    p.max_deg = hd->dp.max_deg;
+    p.row_ptr = hd->dp.row_ptr;
     p.row_len = 128;
-    const size_t smem = (size_t)kTmaWarps * (3 + p.deg) * 128 * sizeof(float);
+    const size_t smem = (size_t)kTmaWarps * (3 + p.max_deg) * 128 * sizeof(float);
     cudaError_t e;
     const bool unit = p.w == nullptr;
     switch (q) {

@@ -305,14 +305,21 @@ def test_persistent_kernel_bit_identical_to_stepwise(fem, name, mode):
         assert np.array_equal(a[4]["energy"], b[4]["energy"]) and a[4]["best_replica"] == b[4]["best_replica"]
 
 
-@pytest.mark.parametrize("case", ["q8_reg10_R16", "q8_reg10_R32_two_blocks", "q4_reg6_weighted_R32", "q32_reg16_R4", "q2_reg3_R64"])
+@pytest.mark.parametrize("case", ["q8_reg10_R16", "q8_reg10_R32_two_blocks", "q4_reg6_weighted_R32", "q32_reg16_R4", "q2_reg3_R64",
+                                  "q8_er_csr_R16", "q4_er_csr_weighted_R32"])
 def test_potts_tma_bit_identical_to_team_kernel(fem, case):
     """The TMA-staged Potts step (rows fetched one variable ahead into a shared-memory ring) against the register
     path: same arithmetic, so fields, moments, energies must be bit-identical; the counter proves which one ran."""
-    q, d, R, rb, weighted = {"q8_reg10_R16": (8, 10, 16, 0, False), "q8_reg10_R32_two_blocks": (8, 10, 32, 16, False),
+    q, d, R, rb, weighted = {"q8_er_csr_R16": (8, 0, 16, 0, False), "q4_er_csr_weighted_R32": (4, 0, 32, 0, True), "q8_reg10_R16": (8, 10, 16, 0, False), "q8_reg10_R32_two_blocks": (8, 10, 32, 16, False),
                              "q4_reg6_weighted_R32": (4, 6, 32, 0, True), "q32_reg16_R4": (32, 16, 4, 0, False),
                              "q2_reg3_R64": (2, 3, 64, 0, False)}[case]
-    inst = wl.random_regular(1201 if d % 2 == 0 else 1200, d, 2020 + q, wl.BMINCUT, q, lam=0.03)
+    if case.startswith(("q8_er", "q4_er")):                       # CSR rows of different lengths (0 .. 16), isolated nodes
+        q, R, rb, weighted = (8, 16, 0, False) if case.startswith("q8") else (4, 32, 0, True)
+        er = wl.erdos_renyi_maxcut(1203, 0.0045, 2040 + q, pm1=False)
+        assert 0 < np.diff(er.row_ptr).max() <= 16 and np.diff(er.row_ptr).min() == 0
+        inst = wl.Instance(wl.BMINCUT, er.n, q, er.row_ptr, er.col_idx, None, lam=0.03)
+    else:
+        inst = wl.random_regular(1201 if d % 2 == 0 else 1200, d, 2020 + q, wl.BMINCUT, q, lam=0.03)
     if weighted:
         w = np.random.default_rng(3).integers(1, 5, inst.nnz // 2).astype(np.float32)[edge_ids(inst)]
         inst = wl.Instance(wl.BMINCUT, inst.n, q, inst.row_ptr, inst.col_idx, w, lam=0.03)
