@@ -152,14 +152,22 @@ struct FinalizeParams {
     int *part;  // [R][q]
 };
 
+// One warp per replica: lane l adds chunks l, l+32, ... in index order, then a fixed butterfly adds the 32 lane sums
+// (a fixed order, so the fp64 sum is the same run to run; the integer sums do not depend on the order at all).
 __global__ void __launch_bounds__(kThreads) energy_finalize_kernel(const FinalizeParams p) {
-    const int a = blockIdx.x * kThreads + threadIdx.x;
-    if (a >= p.R) return;
+    const int a = blockIdx.x * (kThreads / 32) + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (a >= p.R) return;  // warp-uniform
     long long si = 0;
     double sd = 0.0;
-    for (int c = 0; c < p.nchunks; ++c) {
+    for (int c = lane; c < p.nchunks; c += 32) {
         si += p.part_i[(int64_t)c * p.R + a];
         sd += p.part_d[(int64_t)c * p.R + a];
+    }
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) {
+        si += __shfl_xor_sync(0xffffffffu, si, s);
+        sd += __shfl_xor_sync(0xffffffffu, sd, s);
     }
     if (p.integral && p.kind != FEM_ISING) sd = (double)si;
     long long ei = 0;
@@ -178,16 +186,20 @@ __global__ void __launch_bounds__(kThreads) energy_finalize_kernel(const Finaliz
         const double target = __ddiv_rn((double)p.n, (double)p.q);
         for (int k = 0; k < p.q; ++k) {
             int ck = 0;
-            for (int c = 0; c < p.nchunks; ++c) ck += p.part_cnt[((int64_t)c * p.q + k) * p.R + a];
-            p.part[(int64_t)a * p.q + k] = ck;
+            for (int c = lane; c < p.nchunks; c += 32) ck += p.part_cnt[((int64_t)c * p.q + k) * p.R + a];
+#pragma unroll
+            for (int s = 16; s > 0; s >>= 1) ck += __shfl_xor_sync(0xffffffffu, ck, s);
+            if (lane == 0) p.part[(int64_t)a * p.q + k] = ck;
             const double d = __dsub_rn((double)ck, target);
             pen = __dadd_rn(pen, __dmul_rn(d, d));
         }
         ei = si;
         er = __dadd_rn(sd, __dmul_rn(p.lambda, pen));
     }
-    p.e_int[a] = ei;
-    p.e_real[a] = er;
+    if (lane == 0) {
+        p.e_int[a] = ei;
+        p.e_real[a] = er;
+    }
 }
 
 // argmin_a E_a, lowest a on ties; then the winner's configuration.  One CTA.
@@ -283,7 +295,7 @@ static void run_energy(Handle *hd, int R, int Rb, double lambda) {
     f.e_int = hd->e_int;
     f.e_real = hd->e_real;
     f.part = hd->part;
-    energy_finalize_kernel<<<(unsigned)ceil_div(R, kThreads), kThreads, 0, hd->stream>>>(f);
+    energy_finalize_kernel<<<(unsigned)ceil_div(R, kThreads / 32), kThreads, 0, hd->stream>>>(f);
     hd->launches += 2;
 }
 
