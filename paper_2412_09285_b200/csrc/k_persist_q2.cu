@@ -52,6 +52,7 @@ struct PersistParams {
     T rsqrt_bc2[PersistChunk<T>::kSteps];
 };
 
+constexpr int kPersistUnroll = 8;     // ELL rows are padded to a multiple of this: warp-uniform, remainder-free gather loops
 constexpr int kPersistMaxUnits = 128;  // (items per thread) x (warps per CTA) <= 4 x 32
 
 // IPT variables per thread: variable i = c*chunk + k*blockDim.x + threadIdx.x.  ISING: dU/dp = -2 sum_j J_ij m_j.
@@ -61,8 +62,9 @@ __global__ void __launch_bounds__(1024, 1) persist_q2_kernel(const __grid_consta
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int unit_off[kPersistMaxUnits + 1];
     const int n = p.n;
-    T *gbuf = reinterpret_cast<T *>(smem_raw);                             // [2][n]
-    float *ws = reinterpret_cast<float *>(gbuf + 2 * (size_t)n);          // [ell_cap] when WEIGHTED
+    const int gn = n + 1;                                                  // slot n of each buffer stays 0: the ELL padding points at it
+    T *gbuf = reinterpret_cast<T *>(smem_raw);                             // [2][n + 1]
+    float *ws = reinterpret_cast<float *>(gbuf + 2 * (size_t)gn);         // [ell_cap] when WEIGHTED
     unsigned short *cs = reinterpret_cast<unsigned short *>(WEIGHTED ? (ws + p.ell_cap) : ws);  // [ell_cap]
 
     cg::cluster_group cluster = cg::this_cluster();
@@ -75,7 +77,7 @@ __global__ void __launch_bounds__(1024, 1) persist_q2_kernel(const __grid_consta
 
     // ---- state into registers, the whole gathered vector into this CTA's shared memory ----
     T h[IPT], m1[IPT], m2[IPT];
-    int e0[IPT], deg[IPT], off[IPT];
+    int e0[IPT], deg[IPT], off[IPT], pdeg[IPT];  // pdeg: the unit's longest row rounded up to kPersistUnroll (warp-uniform)
 #pragma unroll
     for (int k = 0; k < IPT; ++k) {
         const int i = v_begin + k * nt + tid;
@@ -89,11 +91,16 @@ __global__ void __launch_bounds__(1024, 1) persist_q2_kernel(const __grid_consta
         int mx = deg[k];
 #pragma unroll
         for (int s = 16; s > 0; s >>= 1) mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, s));
-        if (lane == 0) unit_off[k * nwarps + warp + 1] = mx * 32;
+        pdeg[k] = (mx + kPersistUnroll - 1) / kPersistUnroll * kPersistUnroll;
+        if (lane == 0) unit_off[k * nwarps + warp + 1] = pdeg[k] * 32;
     }
     for (int i = tid; i < n; i += nt)
         gbuf[i] = p.disc ? (T)(int)p.g8_in[base + (int64_t)i * p.Rb] : p.g_in[base + (int64_t)i * p.Rb];
-    if (tid == 0) unit_off[0] = 0;
+    if (tid == 0) {
+        unit_off[0] = 0;
+        gbuf[n] = (T)0;
+        gbuf[gn + n] = (T)0;
+    }
     __syncthreads();
     if (tid == 0)
         for (int u = 1; u <= IPT * nwarps; ++u) unit_off[u] += unit_off[u - 1];
@@ -102,9 +109,10 @@ __global__ void __launch_bounds__(1024, 1) persist_q2_kernel(const __grid_consta
 #pragma unroll
     for (int k = 0; k < IPT; ++k) {
         off[k] = unit_off[k * nwarps + warp] + lane;
-        for (int j = 0; j < deg[k]; ++j) {
-            cs[off[k] + j * 32] = (unsigned short)p.col[e0[k] + j];
-            if (WEIGHTED) ws[off[k] + j * 32] = p.w[e0[k] + j];
+        for (int j = 0; j < pdeg[k]; ++j) {  // rows shorter than the unit are padded with (column n, weight 0): adds +0
+            const bool real = j < deg[k];
+            cs[off[k] + j * 32] = real ? (unsigned short)p.col[e0[k] + j] : (unsigned short)n;
+            if (WEIGHTED) ws[off[k] + j * 32] = real ? p.w[e0[k] + j] : 0.0f;
         }
     }
     if (CS > 1) cluster.sync();  // every CTA of the cluster is running before anyone stores into its shared memory
@@ -127,8 +135,8 @@ __global__ void __launch_bounds__(1024, 1) persist_q2_kernel(const __grid_consta
     }
     int cur = 0;
     for (int t = 0; t < p.nsteps; ++t) {
-        const T *__restrict__ gi = gbuf + (size_t)cur * n;
-        T *go = gbuf + (size_t)(cur ^ 1) * n;
+        const T *__restrict__ gi = gbuf + (size_t)cur * gn;
+        T *go = gbuf + (size_t)(cur ^ 1) * gn;
         sc.inv_beta = p.inv_beta[t];
         sc.step_size = p.step_size[t];
         sc.rsqrt_bc2 = p.rsqrt_bc2[t];
@@ -141,11 +149,11 @@ __global__ void __launch_bounds__(1024, 1) persist_q2_kernel(const __grid_consta
                 const unsigned short *__restrict__ cp = cs + off[k];
                 if (WEIGHTED) {
                     const float *__restrict__ wp = ws + off[k];
-#pragma unroll 8
-                    for (int j = 0; j < deg[k]; ++j) dU = fma((T)wp[j * 32], gi[cp[j * 32]], dU);
+#pragma unroll kPersistUnroll
+                    for (int j = 0; j < pdeg[k]; ++j) dU = fma((T)wp[j * 32], gi[cp[j * 32]], dU);
                 } else {
-#pragma unroll 8
-                    for (int j = 0; j < deg[k]; ++j) dU += gi[cp[j * 32]];  // == fma(1, m_j, dU) of the stepwise kernel
+#pragma unroll kPersistUnroll
+                    for (int j = 0; j < pdeg[k]; ++j) dU += gi[cp[j * 32]];  // == fma(1, m_j, dU) of the stepwise kernel
                 }
                 if (ISING) dU = (T)-2 * dU;
                 const T g = q2_grad(dU, ci[k], h[k], sc);
@@ -173,8 +181,8 @@ __global__ void __launch_bounds__(1024, 1) persist_q2_kernel(const __grid_consta
             p.h[o] = h[k];
             p.m1[o] = m1[k];
             p.m2[o] = m2[k];
-            if (p.disc) p.g8_out[o] = (signed char)(int)gbuf[(size_t)cur * n + i];
-            else p.g_out[o] = gbuf[(size_t)cur * n + i];
+            if (p.disc) p.g8_out[o] = (signed char)(int)gbuf[(size_t)cur * gn + i];
+            else p.g_out[o] = gbuf[(size_t)cur * gn + i];
         }
     }
 }
@@ -215,7 +223,7 @@ void persist_prepare(Handle *hd, const int64_t *row_ptr) {
                         const int i = v_begin + k * g.threads + w0 + l;
                         if (i < v_end) mx = std::max<int64_t>(mx, row_ptr[i + 1] - row_ptr[i]);
                     }
-                    entries += 32 * mx;
+                    entries += 32 * ((mx + kPersistUnroll - 1) / kPersistUnroll * kPersistUnroll);
                 }
             worst = std::max(worst, entries);
         }
@@ -224,7 +232,7 @@ void persist_prepare(Handle *hd, const int64_t *row_ptr) {
 }
 
 static size_t persist_smem_bytes(const Handle *hd, int a, size_t elt) {
-    return 2 * (size_t)hd->dp.n * elt + (size_t)hd->persist_ell[a] * (hd->dp.w ? 6 : 2) + 16;
+    return 2 * ((size_t)hd->dp.n + 1) * elt + (size_t)hd->persist_ell[a] * (hd->dp.w ? 6 : 2) + 16;
 }
 
 // Cluster size index for R replicas: spread a replica over as many SMs as the device has to spare (R * CS <= SMs),
