@@ -264,6 +264,131 @@ __global__ void __launch_bounds__(256) dense_field_kernel(const float *__restric
         }
 }
 
+// The same product for the fp64 wide phase and the CUDA-core fallback, as a register-tiled GEMM: 128 x 128 tile per
+// CTA, k step 8, 16 x 16 threads with an 8 x 8 micro-tile each (64 accumulators), J converted on load.  The generic
+// 64 x 64 / 4 x 4 kernel above reached 8.5 TFLOP/s in fp64 on cfg 4b (4 ms per wide step, 12% of the whole pass).
+// Sums run over k in ascending order per output, as in dense_field_kernel (the order inside a k step is the same).
+template <typename T>
+__global__ void __launch_bounds__(256) dense_field_big_kernel(const float *__restrict__ J, const T *__restrict__ M,
+                                                              T *__restrict__ C, int n, int Rb) {
+    constexpr int BM = 128, BN = 128, BK = 8;
+    __shared__ __align__(16) T As[BK][BM];
+    __shared__ __align__(16) T Bs[BK][BN];
+    const int tx = threadIdx.x % 16, ty = threadIdx.x / 16;
+    const int row0 = blockIdx.y * BM, col0 = blockIdx.x * BN;
+    T acc[8][8];
+#pragma unroll
+    for (int x = 0; x < 8; ++x)
+#pragma unroll
+        for (int y = 0; y < 8; ++y) acc[x][y] = (T)0;
+    const int ar = threadIdx.x / 2, ak = (threadIdx.x % 2) * 4;   // A tile: row ar, k = ak .. ak+3
+    const int bk = threadIdx.x / 32, bc = (threadIdx.x % 32) * 4;  // B tile: row bk, columns bc .. bc+3
+    for (int k0 = 0; k0 < n; k0 += BK) {
+#pragma unroll
+        for (int z = 0; z < 4; ++z) {
+            const int gr = row0 + ar, gk = k0 + ak + z;
+            As[ak + z][ar] = (gr < n && gk < n) ? (T)J[(int64_t)gr * n + gk] : (T)0;
+            const int gkb = k0 + bk, gc = col0 + bc + z;
+            Bs[bk][bc + z] = (gkb < n && gc < Rb) ? M[(int64_t)gkb * Rb + gc] : (T)0;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < BK; ++k) {
+            T a[8], b[8];
+#pragma unroll
+            for (int x = 0; x < 8; ++x) a[x] = As[k][ty * 8 + x];
+#pragma unroll
+            for (int y = 0; y < 8; ++y) b[y] = Bs[k][tx * 8 + y];
+#pragma unroll
+            for (int x = 0; x < 8; ++x)
+#pragma unroll
+                for (int y = 0; y < 8; ++y) acc[x][y] = fma(a[x], b[y], acc[x][y]);
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int x = 0; x < 8; ++x)
+#pragma unroll
+        for (int y = 0; y < 8; ++y) {
+            const int gr = row0 + ty * 8 + x, gc = col0 + tx * 8 + y;
+            if (gr < n && gc < Rb) C[(int64_t)gr * Rb + gc] = acc[x][y];
+        }
+}
+
+// fp64 on the tensor cores: the vector FP64 pipe of this part tops out near 9 TFLOP/s (both CUDA-core kernels above
+// run the cfg 4b wide step in 3.9 ms), the DMMA path (mma.sync m8n8k4 f64) is the one rated ~37 TFLOP/s.
+// CTA tile 64 x 64, k step 16, 8 warps as 4 x 2, each warp 16 x 32 = 2 x 4 mma tiles; fragments straight from padded
+// shared memory (conflict-free per half-warp).  Used for the fp64 wide phase of dense couplings.
+__device__ __forceinline__ void dmma_8x8x4(double &c0, double &c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+__global__ void __launch_bounds__(256) dense_field_dmma_kernel(const float *__restrict__ J, const double *__restrict__ M,
+                                                               double *__restrict__ C, int n, int Rb) {
+    constexpr int BM = 64, BN = 64, BK = 16;
+    __shared__ double As[BM][BK + 4];
+    __shared__ double Bs[BK][BN + 4];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int wm = (warp >> 1) * 16, wn = (warp & 1) * 32;
+    const int row0 = blockIdx.y * BM, col0 = blockIdx.x * BN;
+    double acc[2][4][2];
+#pragma unroll
+    for (int x = 0; x < 2; ++x)
+#pragma unroll
+        for (int y = 0; y < 4; ++y) acc[x][y][0] = acc[x][y][1] = 0.0;
+    const int ar = threadIdx.x / 4, ak = (threadIdx.x % 4) * 4;    // A tile: row ar, k = ak .. ak+3
+    const int bk = threadIdx.x / 16, bc = (threadIdx.x % 16) * 4;  // B tile: row bk, columns bc .. bc+3
+    for (int k0 = 0; k0 < n; k0 += BK) {
+#pragma unroll
+        for (int z = 0; z < 4; ++z) {
+            const int gr = row0 + ar, gk = k0 + ak + z;
+            As[ar][ak + z] = (gr < n && gk < n) ? (double)J[(int64_t)gr * n + gk] : 0.0;
+            const int gkb = k0 + bk, gc = col0 + bc + z;
+            Bs[bk][bc + z] = (gkb < n && gc < Rb) ? M[(int64_t)gkb * Rb + gc] : 0.0;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int kk = 0; kk < BK; kk += 4) {
+            double a[2], b[4];
+#pragma unroll
+            for (int x = 0; x < 2; ++x) a[x] = As[wm + x * 8 + (lane >> 2)][kk + (lane & 3)];
+#pragma unroll
+            for (int y = 0; y < 4; ++y) b[y] = Bs[kk + (lane & 3)][wn + y * 8 + (lane >> 2)];
+#pragma unroll
+            for (int x = 0; x < 2; ++x)
+#pragma unroll
+                for (int y = 0; y < 4; ++y) dmma_8x8x4(acc[x][y][0], acc[x][y][1], a[x], b[y]);
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int x = 0; x < 2; ++x)
+#pragma unroll
+        for (int y = 0; y < 4; ++y) {
+            const int gr = row0 + wm + x * 8 + (lane >> 2), gc = col0 + wn + y * 8 + 2 * (lane & 3);
+            if (gr < n) {
+                if (gc < Rb) C[(int64_t)gr * Rb + gc] = acc[x][y][0];
+                if (gc + 1 < Rb) C[(int64_t)gr * Rb + gc + 1] = acc[x][y][1];
+            }
+        }
+}
+
+template <typename T>
+static void launch_dense_field(Handle *hd, const T *M, T *C, int n, int Rb) {
+    if (n >= 256 && Rb >= 64) {
+        if constexpr (std::is_same<T, double>::value) {
+            dim3 gb((unsigned)ceil_div(Rb, 64), (unsigned)ceil_div(n, 64));
+            dense_field_dmma_kernel<<<gb, 256, 0, hd->stream>>>(hd->dp.J, M, C, n, Rb);
+        } else {
+            dim3 gb((unsigned)ceil_div(Rb, 128), (unsigned)ceil_div(n, 128));
+            dense_field_big_kernel<T><<<gb, 256, 0, hd->stream>>>(hd->dp.J, M, C, n, Rb);
+        }
+    } else {
+        dim3 g((unsigned)ceil_div(Rb, 64), (unsigned)ceil_div(n, 64));
+        dense_field_kernel<T><<<g, 256, 0, hd->stream>>>(hd->dp.J, M, C, n, Rb);
+    }
+}
+
 template <typename T, int VEC, int MODE>
 static void launch_q2_deg(Handle *hd, const Q2Params<T> &p, dim3 grid) {
     if constexpr (MODE == MODE_SAT) {
@@ -329,7 +454,7 @@ static void launch_step_q2_t(Handle *hd, const StepScalars &sc, int blk_begin, i
         dim3 g((unsigned)ceil_div(Rb, 64), (unsigned)ceil_div(n, 64));
         for (int b = 0; b < blk_count; ++b) {
             const int64_t o = (int64_t)b * p.a.blk_stride;
-            dense_field_kernel<T><<<g, 256, 0, hd->stream>>>(hd->dp.J, p.a.g_in + o, S::field(hd) + base + o, n, Rb);
+            launch_dense_field<T>(hd, p.a.g_in + o, S::field(hd) + base + o, n, Rb);
             hd->launches++;
         }
     }
