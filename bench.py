@@ -216,7 +216,9 @@ def main():
         raise SystemExit("bench.py needs a CUDA device: the FEM path has no CPU fallback")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    if world > 1:
+    # under torchrun (even with one rank) the collectives of the N > 1 path are really run, over NCCL
+    use_dist = world > 1 or ("RANK" in os.environ and "MASTER_ADDR" in os.environ)
+    if use_dist:
         dist.init_process_group("nccl", device_id=dev)
 
     inst = cfg.make()
@@ -246,7 +248,7 @@ def main():
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > L2 (126 MB)
 
     def barrier():
-        if world > 1:
+        if use_dist:
             dist.barrier()
         torch.cuda.synchronize()
 
@@ -324,7 +326,7 @@ def main():
 
     # ---- max over ranks, best replica over ranks
     times = torch.tensor([elapsed_ms, e2e_s * 1e3, bulk_ms], dtype=torch.float64, device=dev)
-    if world > 1:
+    if use_dist:
         dist.all_reduce(times, op=dist.ReduceOp.MAX)
     # Eq.5 across ranks: 8 bytes per rank, then the owner's configuration
     best_energy, best_owner, _ = multigpu.best_over_ranks(float(res["energy"][res["best_replica"]]),
@@ -411,7 +413,7 @@ def main():
                                     "sample": f"{sN if use_omp else s1} annealing steps at full n={n}, R={R} of {cfg.name}",
                                     "single_thread_value": v1, "all_core_value": vN, "all_core_threads": cN}
         print(json.dumps(line))
-    if world > 1:
+    if use_dist:
         dist.destroy_process_group()
 
 

@@ -22,7 +22,7 @@ def best_over_ranks(best_energy: float, best_config: np.ndarray, device: torch.d
     Returns (energy, owner_rank, config) on every rank.  Traffic: 8 bytes per rank + n int32 from the owner."""
     world = dist.get_world_size() if dist.is_initialized() else 1
     cfg = torch.tensor(np.asarray(best_config, dtype=np.int32), device=device)  # a copy: the broadcast is in place
-    if world == 1:
+    if not dist.is_initialized():
         return float(best_energy), 0, cfg.cpu().numpy()
     mine = torch.tensor([best_energy], dtype=torch.float64, device=device)
     allv = [torch.zeros_like(mine) for _ in range(world)]
