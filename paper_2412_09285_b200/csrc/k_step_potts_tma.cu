@@ -41,6 +41,10 @@ struct PottsTmaParams {
     int max_deg;          // rows of the slot reserved for neighbours
     const int *row_ptr;
     unsigned row_len;     // q * Rb floats = 128 (one float4 per lane)
+    // manipulated gradients (DISC): neighbours enter as state ids, one byte per (variable, replica) (device_math.cuh)
+    const signed char *g8_in;
+    signed char *g8_out;
+    const double *rowsum;
 };
 
 constexpr int kTmaWarps = 8;          // warps per CTA
@@ -73,7 +77,7 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
                  : "memory");
 }
 
-template <int QPAD, bool UNITW>
+template <int QPAD, bool UNITW, bool DISC>
 __global__ void __launch_bounds__(kTmaWarps * 32, 4) potts_tma_kernel(const __grid_constant__ PottsTmaParams p) {
     constexpr int VEC = 4;
     using R = Row<float, VEC>;
@@ -128,19 +132,33 @@ __global__ void __launch_bounds__(kTmaWarps * 32, 4) potts_tma_kernel(const __gr
         const int c = __shfl_sync(0xffffffffu, col_lane, lane >= 3 ? lane - 3 : 0);
         float *dst = my_ring + (size_t)lane * 128;
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // the slot was read through the generic proxy
-        if (lane == 0) mbar_expect_tx(bar, (uint32_t)(3 + d) * row_bytes);
+        const uint32_t id_bytes = (uint32_t)p.Rb;  // DISC: one id row = Rb bytes (a multiple of 16 on this path)
+        if (lane == 0) mbar_expect_tx(bar, DISC ? 3 * row_bytes + (uint32_t)(d + 1) * id_bytes : (uint32_t)(3 + d) * row_bytes);
         __syncwarp();
         const int64_t own = blk + (int64_t)i * 128;
         if (lane == 0) bulk_g2s(dst, p.h + own, row_bytes, bar);
         else if (lane == 1) bulk_g2s(dst, p.m1 + own, row_bytes, bar);
         else if (lane == 2) bulk_g2s(dst, p.m2 + own, row_bytes, bar);
-        else if (lane < 3 + d) bulk_g2s(dst, p.g_in + blk + (int64_t)(unsigned)c * 128, row_bytes, bar);
+        else if (!DISC && lane < 3 + d) bulk_g2s(dst, p.g_in + blk + (int64_t)(unsigned)c * 128, row_bytes, bar);
+        else if (DISC && lane <= 3 + d) {
+            // id rows behind the three fp32 rows: neighbour k at byte 1536 + k*Rb, the variable's own ids after them
+            signed char *d8 = reinterpret_cast<signed char *>(my_ring + 3 * 128) + (size_t)(lane - 3) * id_bytes;
+            const int64_t var = lane < 3 + d ? (int64_t)(unsigned)c : (int64_t)i;
+            bulk_g2s(d8, p.g8_in + blk + var * p.Rb, id_bytes, bar);
+        }
     };
     // CSR row of variable i: first entry e0, degree d (warp-uniform), this lane's column index
+    float cf_n = 1.0f, lamc_n = sc.two_lambda, shift_n = 0.0f;  // DISC: c^f, lambda c^a, sum_j W_ij / q of the row loaded last
     auto load_row = [&](int i, int &e0, int &d) -> int {
         e0 = 0;
         d = 0;
         if (i >= n) return 0;
+        if (DISC) {  // S27, exactly as in potts_team_kernel
+            const double rs = __ldg(p.rowsum + i);
+            cf_n = rs > 0.0 ? (float)((double)p.q / rs) : 0.0f;
+            lamc_n = rs > 0.0 ? (float)(0.5 * (double)sc.two_lambda * ((double)p.q / sqrt(rs))) : 0.0f;
+            shift_n = (float)(rs / (double)p.q);
+        }
         if (p.deg > 0) {
             e0 = i * p.deg;
             d = p.deg;
@@ -153,10 +171,13 @@ __global__ void __launch_bounds__(kTmaWarps * 32, 4) potts_tma_kernel(const __gr
 
     int i = warp_gid;
     int e0 = 0, deg = 0, e0_next = 0, deg_next = 0, col_next = 0;
+    float cf = 1.0f, lam_c = sc.two_lambda, shift = 0.0f, cf_next = 1.0f, lamc_next = sc.two_lambda, shift_next = 0.0f;
     if (i < n) {
         const int c0 = load_row(i, e0, deg);
+        cf = cf_n; lam_c = lamc_n; shift = shift_n;
         issue(i, c0, deg);
         col_next = load_row(i + warps_total, e0_next, deg_next);
+        cf_next = cf_n; lamc_next = lamc_n; shift_next = shift_n;
     }
     for (int t = 0; i < n; ++t, i += warps_total) {
         const int in = i + warps_total;
@@ -168,7 +189,23 @@ __global__ void __launch_bounds__(kTmaWarps * 32, 4) potts_tma_kernel(const __gr
         float f[VEC];
 #pragma unroll
         for (int v = 0; v < VEC; ++v) f[v] = 0.0f;
-        for (int k = 0; k < deg; ++k) {
+        unsigned own_ids = 0;
+        if (DISC) {
+            // one-hot neighbours: f(s) = sum_j W_ij [id_j == s], centred by sum_j W_ij / q; this lane's 4 replicas are
+            // word rl of each Rb-byte id row
+            const unsigned *ids = reinterpret_cast<const unsigned *>(my_ring + 3 * 128) + rl;
+            const int words = p.Rb / 4;
+            for (int k = 0; k < deg; ++k) {
+                const unsigned w4 = ids[k * words];
+                const float ww = UNITW ? 1.0f : __ldg(p.w + e0 + k);
+#pragma unroll
+                for (int v = 0; v < VEC; ++v) f[v] += ((w4 >> (8 * v)) & 0xffu) == (unsigned)s ? ww : 0.0f;
+            }
+            own_ids = ids[deg * words];
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) f[v] -= shift;
+        }
+        for (int k = 0; k < (DISC ? 0 : deg); ++k) {
             const float4 nb = *reinterpret_cast<const float4 *>(stage + (3 + k) * 128);
             if (UNITW) {
                 f[0] += nb.x; f[1] += nb.y; f[2] += nb.z; f[3] += nb.w;  // == fma(1, D_j, f)
@@ -190,11 +227,14 @@ __global__ void __launch_bounds__(kTmaWarps * 32, 4) potts_tma_kernel(const __gr
         // the slot is in registers now: refill it with the warp's next variable while this one is computed
         __syncwarp();
         const int deg_issue = deg_next;
+        const float cf_i = cf, lamc_i = lam_c;  // this variable's factors; the rotation below is for the next one
         e0 = e0_next;   // (the neighbour sum above is done with this variable's row)
         deg = deg_next;
+        cf = cf_next; lam_c = lamc_next; shift = shift_next;
         if (in < n) {
             issue(in, col_next, deg_issue);
             col_next = load_row(in + warps_total, e0_next, deg_next);
+            cf_next = cf_n; lamc_next = lamc_n; shift_next = shift_n;
         }
         // softmax of h(t) across the states
         float P[VEC];
@@ -213,7 +253,13 @@ __global__ void __launch_bounds__(kTmaWarps * 32, 4) potts_tma_kernel(const __gr
         const bool use_m1 = sc.uses_m1(), use_m2 = sc.uses_m2();
 #pragma unroll
         for (int v = 0; v < VEC; ++v) {
-            const float gp = fma(h[v], sc.inv_beta, fma(sc.two_lambda, Ss[v] - P[v], -f[v]));
+            float gp;
+            if (DISC) {
+                const float own = ((((own_ids >> (8 * v)) & 0xffu) == (unsigned)s) ? 1.0f : 0.0f) - inv_q;
+                gp = fma(h[v], sc.inv_beta, fma(lamc_i, Ss[v] - own, -(cf_i * f[v])));
+            } else {
+                gp = fma(h[v], sc.inv_beta, fma(sc.two_lambda, Ss[v] - P[v], -f[v]));
+            }
             float gbar = P[v] * gp;
 #pragma unroll
             for (int k = 0; k < kStages; ++k) gbar += __shfl_sync(0xffffffffu, gbar, partner[k]);
@@ -226,6 +272,7 @@ __global__ void __launch_bounds__(kTmaWarps * 32, 4) potts_tma_kernel(const __gr
         if (use_m2) m2.st_stream(p.m2 + off);
         // centred marginals of the new fields -> g_out, and their column sums
         R po;
+        int win[VEC] = {0, 0, 0, 0};
 #pragma unroll
         for (int v = 0; v < VEC; ++v) {
             float mx = h[v];
@@ -236,9 +283,20 @@ __global__ void __launch_bounds__(kTmaWarps * 32, 4) potts_tma_kernel(const __gr
 #pragma unroll
             for (int k = 0; k < kStages; ++k) z += __shfl_sync(0xffffffffu, z, partner[k]);
             po.v[v] = fma(e, frcp(z), -inv_q);
+            if (DISC) {  // centred one-hot of the new fields: lowest state among the maxima (rounding rule R3)
+                int cand = h[v] == mx ? s : 1 << 30;
+#pragma unroll
+                for (int k = 0; k < kStages; ++k) cand = min(cand, __shfl_sync(0xffffffffu, cand, partner[k]));
+                win[v] = cand;
+                po.v[v] = (cand == s ? 1.0f : 0.0f) - inv_q;
+            }
             colacc[v] += __float2ll_rn(po.v[v] * fx_scale_t);
         }
-        po.st(p.g_out + off);
+        if (DISC) {
+            if (s == 0) st_bytes<VEC>(p.g8_out + blk + (int64_t)i * p.Rb + (unsigned)rl * VEC, win);
+        } else {
+            po.st(p.g_out + off);
+        }
     }
 
     // column sums: exact integer adds -- lanes -> CTA (shared atomics) -> grid (global atomics)
@@ -257,21 +315,22 @@ __global__ void __launch_bounds__(kTmaWarps * 32, 4) potts_tma_kernel(const __gr
 // ---- host side ----
 bool potts_tma_applicable(const Handle *hd) {
     const int q = hd->dp.q, Rb = hd->Rb, deg = hd->dp.max_deg;
-    if (hd->opt_potts_tma == 0 || hd->gather_disc) return false;
+    if (hd->opt_potts_tma == 0) return false;
+    if (hd->gather_disc && Rb % 16 != 0) return false;  // id rows travel as bulk copies of Rb bytes (q <= 8)
     if (q < 2 || (q & (q - 1)) != 0 || Rb % 4 != 0 || q * (Rb / 4) != 32) return false;  // one variable = one warp of float4 lanes
     return deg >= 1 && deg <= kTmaMaxDeg && hd->dp.nnz < ((int64_t)1 << 31);
 }
 
-template <int QPAD, bool UNITW>
+template <int QPAD, bool UNITW, bool DISC>
 static cudaError_t launch_tma_one(Handle *hd, const PottsTmaParams &p, int blk_count, size_t smem) {
     static std::map<size_t, int> resident_of;  // CTAs resident at once, per ring size (the degree sets it)
     int &resident = resident_of[smem];
     if (resident == 0) {
         const size_t smem_max = (size_t)kTmaWarps * (3 + kTmaMaxDeg) * 128 * sizeof(float);
-        cudaError_t e = cudaFuncSetAttribute(potts_tma_kernel<QPAD, UNITW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
+        cudaError_t e = cudaFuncSetAttribute(potts_tma_kernel<QPAD, UNITW, DISC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
         if (e != cudaSuccess) return e;
         int occ = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, potts_tma_kernel<QPAD, UNITW>, kTmaWarps * 32, smem) != cudaSuccess ||
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, potts_tma_kernel<QPAD, UNITW, DISC>, kTmaWarps * 32, smem) != cudaSuccess ||
             occ < 1)
             occ = 1;
         resident = occ * hd->sm_count;
@@ -287,7 +346,7 @@ static cudaError_t launch_tma_one(Handle *hd, const PottsTmaParams &p, int blk_c
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, potts_tma_kernel<QPAD, UNITW>, p);
+    return cudaLaunchKernelEx(&cfg, potts_tma_kernel<QPAD, UNITW, DISC>, p);
 }
 
 // One fp32 exact-gradient Potts step of replica blocks [blk_begin, blk_begin + blk_count); false = not applicable.
@@ -320,14 +379,22 @@ bool launch_potts_tma(Handle *hd, const StepScalars &sc, int blk_begin, int blk_
     p.row_ptr = hd->dp.row_ptr;
     p.row_len = 128;
     const size_t smem = (size_t)kTmaWarps * (3 + p.max_deg) * 128 * sizeof(float);
+    p.g8_in = reinterpret_cast<const signed char *>(hd->g[hd->cur]) + base;
+    p.g8_out = reinterpret_cast<signed char *>(hd->g[hd->cur ^ 1]) + base;
+    p.rowsum = hd->rowsum;
     cudaError_t e;
-    const bool unit = p.w == nullptr;
+    const bool unit = p.w == nullptr, disc = hd->gather_disc;
+    auto go = [&](auto qtag) -> cudaError_t {
+        constexpr int Q = decltype(qtag)::value;
+        if (disc) return unit ? launch_tma_one<Q, true, true>(hd, p, blk_count, smem) : launch_tma_one<Q, false, true>(hd, p, blk_count, smem);
+        return unit ? launch_tma_one<Q, true, false>(hd, p, blk_count, smem) : launch_tma_one<Q, false, false>(hd, p, blk_count, smem);
+    };
     switch (q) {
-        case 2: e = unit ? launch_tma_one<2, true>(hd, p, blk_count, smem) : launch_tma_one<2, false>(hd, p, blk_count, smem); break;
-        case 4: e = unit ? launch_tma_one<4, true>(hd, p, blk_count, smem) : launch_tma_one<4, false>(hd, p, blk_count, smem); break;
-        case 8: e = unit ? launch_tma_one<8, true>(hd, p, blk_count, smem) : launch_tma_one<8, false>(hd, p, blk_count, smem); break;
-        case 16: e = unit ? launch_tma_one<16, true>(hd, p, blk_count, smem) : launch_tma_one<16, false>(hd, p, blk_count, smem); break;
-        default: e = unit ? launch_tma_one<32, true>(hd, p, blk_count, smem) : launch_tma_one<32, false>(hd, p, blk_count, smem); break;
+        case 2: e = go(std::integral_constant<int, 2>{}); break;
+        case 4: e = go(std::integral_constant<int, 4>{}); break;
+        case 8: e = go(std::integral_constant<int, 8>{}); break;
+        case 16: e = go(std::integral_constant<int, 16>{}); break;
+        default: e = go(std::integral_constant<int, 32>{}); break;
     }
     if (e != cudaSuccess) {
         (void)cudaGetLastError();

@@ -307,7 +307,8 @@ def test_persistent_kernel_bit_identical_to_stepwise(fem, name, mode):
 
 @pytest.mark.parametrize("case", ["q8_reg10_R16", "q8_reg10_R32_two_blocks", "q4_reg6_weighted_R32", "q32_reg16_R4", "q2_reg3_R64",
                                   "q8_er_csr_R16", "q4_er_csr_weighted_R32"])
-def test_potts_tma_bit_identical_to_team_kernel(fem, case):
+@pytest.mark.parametrize("manipulated", [False, True])
+def test_potts_tma_bit_identical_to_team_kernel(fem, case, manipulated):
     """The TMA-staged Potts step (rows fetched one variable ahead into a shared-memory ring) against the register
     path: same arithmetic, so fields, moments, energies must be bit-identical; the counter proves which one ran."""
     q, d, R, rb, weighted = {"q8_er_csr_R16": (8, 0, 16, 0, False), "q4_er_csr_weighted_R32": (4, 0, 32, 0, True), "q8_reg10_R16": (8, 10, 16, 0, False), "q8_reg10_R32_two_blocks": (8, 10, 32, 16, False),
@@ -323,7 +324,9 @@ def test_potts_tma_bit_identical_to_team_kernel(fem, case):
     if weighted:
         w = np.random.default_rng(3).integers(1, 5, inst.nnz // 2).astype(np.float32)[edge_ids(inst)]
         inst = wl.Instance(wl.BMINCUT, inst.n, q, inst.row_ptr, inst.col_idx, w, lam=0.03)
-    sch = fem.Schedule(beta=fem.linear_temperature_schedule(1.0, 0.05, 40), precise_steps=4)
+    sch = fem.Schedule(beta=fem.linear_temperature_schedule(1.0, 0.05, 40), precise_steps=4, manipulated=manipulated,
+                       gamma_grad=0.9, **(dict(optimizer=1, lr=0.03, alpha=0.9, momentum=0.5) if manipulated else {}))
+    applies = not manipulated or q <= 8              # manipulated: the id rows must be whole 16-byte bulk copies
     out = {}
     for tma in (1, 0):
         eng = fem.Fem(inst, R)
@@ -333,7 +336,7 @@ def test_potts_tma_bit_identical_to_team_kernel(fem, case):
         eng.anneal(sch, R, seed=8, stop_after=17)
         eng.anneal(sch, R, seed=8, stop_after=40)
         out[tma] = (eng.get_fields(), eng.get_moments(), eng.result())
-        assert eng.info("tma_launches") == (36 * (R // rb if rb else 1) if tma else 0)   # 40 steps - 4 wide ones, per block
+        assert eng.info("tma_launches") == (36 * (R // rb if rb else 1) if tma and applies else 0)   # 40 steps - 4 wide, per block
         eng.close()
     assert np.array_equal(out[1][0], out[0][0])
     assert np.array_equal(out[1][1][0], out[0][1][0]) and np.array_equal(out[1][1][1], out[0][1][1])
