@@ -274,6 +274,10 @@ def main():
             ev.append((a, b, eng.info("launches") - l0 - (1 if K > 0 else 0), z, c))
 
     sampler = ClockSampler(local_rank) if rank == 0 else None   # started before warm-up: nvidia-smi takes a while to start
+    if sampler is not None and sampler.p is not None:           # ... so wait for its first line (short workloads: cfg 0)
+        t_wait = time.time()
+        while os.path.getsize(sampler.f.name) == 0 and time.time() - t_wait < 5.0:
+            time.sleep(0.02)
     for w in range(args.warmup):
         one_pass(multigpu.replica_seed(1000 + w, rank))
     barrier()
