@@ -353,6 +353,11 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
         dp.lits = reinterpret_cast<int *>(at(L.lits));
         hd->integral_weights = true;
         hd->structure_bytes = 4 * ((int64_t)n + 1) + 4 * (int64_t)s.nocc * kst;
+        {   // sliced-ELL sizes of the replica-persistent kernel, from the occurrence counts
+            hd->dp = dp;
+            std::vector<int64_t> optr(h_occ_ptr.begin(), h_occ_ptr.end());
+            persist_prepare(hd, optr.data());
+        }
     } else if (s.dense) {
         const int n = pb->n;
         for (int i = 0; i < n; ++i) {

@@ -1,4 +1,5 @@
-// Replica-persistent annealing kernel for SMALL sparse two-state problems (MaxCut / sparse Ising, n <= 4096).
+// Replica-persistent annealing kernel for SMALL two-state problems (MaxCut / sparse Ising / Max-SAT with clauses of at
+// most 5 literals; at most 4096 variables per CTA of the cluster).
 //
 // The stepwise kernel (k_step_q2.cu) is launch- and latency-bound when n*R is a few tens of thousands of
 // fields (BASELINE.json configs[0]: n = 800, R = 32: one launch per annealing step, 11 us each, 1% of HBM).
@@ -46,6 +47,7 @@ struct PersistParams {
     signed char *g8_out;
     T eps, b1, b2, omb1, omb2, wd, gamma;
     int opt, disc;
+    int kst;             // Max-SAT: ints per occurrence in `col` (k_max - 1 rounded up to a power of two)
     int first_step;      // index in this chunk of the anneal's step 0 (SGD momentum buffer starts there), or -1
     T inv_beta[PersistChunk<T>::kSteps];
     T step_size[PersistChunk<T>::kSteps];
@@ -56,7 +58,10 @@ constexpr int kPersistUnroll = 8;     // ELL rows are padded to a multiple of th
 constexpr int kPersistMaxUnits = 128;  // (items per thread) x (warps per CTA) <= 4 x 32
 
 // IPT variables per thread: variable i = c*chunk + k*blockDim.x + threadIdx.x.  ISING: dU/dp = -2 sum_j J_ij m_j.
-template <typename T, int IPT, bool ISING, bool WEIGHTED>
+// SATK > 0: Max-SAT -- `row_ptr` / `col` are the variable -> occurrence table (fem_internal.cuh), SATK = k_max - 1 packed
+// entries (var << 1 | negated) per occurrence, own sign in bit 31 of entry 0; the ELL keeps SATK 16-bit arrays and a sign
+// byte per slot; slot n of the gathered vector is the constant 1 that pads short clauses.
+template <typename T, int IPT, bool ISING, bool WEIGHTED, int SATK>
 __global__ void __launch_bounds__(1024, 1) persist_q2_kernel(const __grid_constant__ PersistParams<T> p) {
     namespace cg = cooperative_groups;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -65,7 +70,8 @@ __global__ void __launch_bounds__(1024, 1) persist_q2_kernel(const __grid_consta
     const int gn = n + 1;                                                  // slot n of each buffer stays 0: the ELL padding points at it
     T *gbuf = reinterpret_cast<T *>(smem_raw);                             // [2][n + 1]
     float *ws = reinterpret_cast<float *>(gbuf + 2 * (size_t)gn);         // [ell_cap] when WEIGHTED
-    unsigned short *cs = reinterpret_cast<unsigned short *>(WEIGHTED ? (ws + p.ell_cap) : ws);  // [ell_cap]
+    unsigned short *cs = reinterpret_cast<unsigned short *>(WEIGHTED ? (ws + p.ell_cap) : ws);  // [ell_cap] ([SATK][ell_cap])
+    unsigned char *sgn = reinterpret_cast<unsigned char *>(cs + (size_t)(SATK > 0 ? SATK : 1) * p.ell_cap);  // SAT: [ell_cap]
 
     cg::cluster_group cluster = cg::this_cluster();
     const unsigned CS = cluster.num_blocks();
@@ -98,8 +104,8 @@ __global__ void __launch_bounds__(1024, 1) persist_q2_kernel(const __grid_consta
         gbuf[i] = p.disc ? (T)(int)p.g8_in[base + (int64_t)i * p.Rb] : p.g_in[base + (int64_t)i * p.Rb];
     if (tid == 0) {
         unit_off[0] = 0;
-        gbuf[n] = (T)0;
-        gbuf[gn + n] = (T)0;
+        gbuf[n] = SATK > 0 ? (T)1 : (T)0;
+        gbuf[gn + n] = SATK > 0 ? (T)1 : (T)0;
     }
     __syncthreads();
     if (tid == 0)
@@ -111,6 +117,16 @@ __global__ void __launch_bounds__(1024, 1) persist_q2_kernel(const __grid_consta
         off[k] = unit_off[k * nwarps + warp] + lane;
         for (int j = 0; j < pdeg[k]; ++j) {  // rows shorter than the unit are padded with (column n, weight 0): adds +0
             const bool real = j < deg[k];
+            if (SATK > 0) {
+                // padding occurrence: first factor 0.5 - 0.5 * 1 = 0, the others 1: contributes +-0
+#pragma unroll
+                for (int x = 0; x < (SATK > 0 ? SATK : 1); ++x) {
+                    const unsigned pk = real ? (unsigned)p.col[(int64_t)(e0[k] + j) * p.kst + x] : (((unsigned)n << 1) | (x == 0 ? 0u : 1u));
+                    cs[(size_t)x * p.ell_cap + off[k] + j * 32] = (unsigned short)(pk & 0xffffu);
+                    if (x == 0) sgn[off[k] + j * 32] = (unsigned char)(pk >> 31);
+                }
+                continue;
+            }
             cs[off[k] + j * 32] = real ? (unsigned short)p.col[e0[k] + j] : (unsigned short)n;
             if (WEIGHTED) ws[off[k] + j * 32] = real ? p.w[e0[k] + j] : 0.0f;
         }
@@ -147,7 +163,21 @@ __global__ void __launch_bounds__(1024, 1) persist_q2_kernel(const __grid_consta
             if (i < v_end) {
                 T dU = (T)0;
                 const unsigned short *__restrict__ cp = cs + off[k];
-                if (WEIGHTED) {
+                if (SATK > 0) {
+                    // dU/dp_i = sum_{m ni i} s_mi prod_{k != i} u_mk (S28), occurrences in table order
+                    const unsigned char *__restrict__ sp = sgn + off[k];
+#pragma unroll 4
+                    for (int j = 0; j < pdeg[k]; ++j) {
+                        T prod = (T)1;
+#pragma unroll
+                        for (int x = 0; x < (SATK > 0 ? SATK : 1); ++x) {
+                            const unsigned e = cp[(size_t)x * p.ell_cap + j * 32];
+                            const T sg = (e & 1u) ? (T)0.5 : (T)-0.5;
+                            prod *= fma(sg, gi[e >> 1], (T)0.5);
+                        }
+                        dU += sp[j * 32] ? -prod : prod;
+                    }
+                } else if (WEIGHTED) {
                     const float *__restrict__ wp = ws + off[k];
 #pragma unroll kPersistUnroll
                     for (int j = 0; j < pdeg[k]; ++j) dU = fma((T)wp[j * 32], gi[cp[j * 32]], dU);
@@ -232,14 +262,18 @@ void persist_prepare(Handle *hd, const int64_t *row_ptr) {
 }
 
 static size_t persist_smem_bytes(const Handle *hd, int a, size_t elt) {
-    return 2 * ((size_t)hd->dp.n + 1) * elt + (size_t)hd->persist_ell[a] * (hd->dp.w ? 6 : 2) + 16;
+    const size_t per_slot = hd->dp.kind == FEM_MAXSAT ? 2 * (size_t)hd->dp.kstride + 1 : (hd->dp.w ? 6 : 2);
+    return 2 * ((size_t)hd->dp.n + 1) * elt + (size_t)hd->persist_ell[a] * per_slot + 16;
 }
 
 // Cluster size index for R replicas: spread a replica over as many SMs as the device has to spare (R * CS <= SMs),
 // at least 64 variables per CTA, and the CTA's ELL + two copies of the gathered vector (fp64) must fit.
 static int persist_choose(const Handle *hd, int R) {
     if (hd->opt_persistent == 0) return -1;
-    if (!(hd->dp.kind == FEM_MAXCUT || (hd->dp.kind == FEM_ISING && !hd->dp.J))) return -1;
+    const bool graph = hd->dp.kind == FEM_MAXCUT || (hd->dp.kind == FEM_ISING && !hd->dp.J);
+    // Max-SAT: clause length <= 5 (one kernel per k_max - 1 = 1..4), packed entries (var << 1 | negated) in 16 bits
+    const bool sat = hd->dp.kind == FEM_MAXSAT && hd->dp.kstride >= 1 && hd->dp.kstride <= 4 && hd->dp.n <= 32767;
+    if (!graph && !sat) return -1;
     int best = -1;
     for (int a = 0; a < 4; ++a) {
         if (hd->persist_ell[a] < 0 || persist_smem_bytes(hd, a, sizeof(double)) > kSmemCap) continue;
@@ -251,6 +285,10 @@ static int persist_choose(const Handle *hd, int R) {
         const int sms = kClusterSizes[a] == 1 ? hd->sm_count : hd->sm_count - hd->sm_count % (2 * kClusterSizes[a]);
         if ((int64_t)R * kClusterSizes[a] <= sms && ceil_div(hd->dp.n, kClusterSizes[a]) >= 64) best = a;
     }
+    // one CTA (cluster) per replica runs in waves over the SMs: beyond ~3 waves the stepwise kernel, which spreads every
+    // step over the whole device, is faster (Max-SAT n = 300, m = 2600: R = 148 -> 2.0 vs 7.1 ms per 500-step anneal,
+    // R = 400 -> 6.0 vs 7.8, R = 800 -> 11.8 vs 10.3)
+    if (best >= 0 && (int64_t)R * kClusterSizes[best] > 3 * (int64_t)hd->sm_count) return -1;
     return best;
 }
 
@@ -276,8 +314,16 @@ static cudaError_t persist_launch_ipt(Handle *hd, const PersistParams<T> &p, int
         return cudaLaunchKernelEx(&cfg, kernel, p);
     };
     const bool ising = hd->dp.kind == FEM_ISING, weighted = hd->dp.w != nullptr;
-    if (ising) return weighted ? launch(persist_q2_kernel<T, IPT, true, true>) : launch(persist_q2_kernel<T, IPT, true, false>);
-    return weighted ? launch(persist_q2_kernel<T, IPT, false, true>) : launch(persist_q2_kernel<T, IPT, false, false>);
+    if (hd->dp.kind == FEM_MAXSAT) {
+        switch (hd->dp.kstride) {
+            case 1: return launch(persist_q2_kernel<T, IPT, false, false, 1>);
+            case 2: return launch(persist_q2_kernel<T, IPT, false, false, 2>);
+            case 3: return launch(persist_q2_kernel<T, IPT, false, false, 3>);
+            default: return launch(persist_q2_kernel<T, IPT, false, false, 4>);
+        }
+    }
+    if (ising) return weighted ? launch(persist_q2_kernel<T, IPT, true, true, 0>) : launch(persist_q2_kernel<T, IPT, true, false, 0>);
+    return weighted ? launch(persist_q2_kernel<T, IPT, false, true, 0>) : launch(persist_q2_kernel<T, IPT, false, false, 0>);
 }
 
 // Runs steps [t_begin, t_end) of the schedule for all replicas; `scalars(t)` gives the per-step scalars.
@@ -299,9 +345,12 @@ static cudaError_t persist_run_t(Handle *hd, int t_begin, int t_end, F &&scalars
         p.g_in = S::g(hd, hd->cur);
         const int cur_after = hd->cur ^ ((tb - ta) & 1);
         p.g_out = S::g(hd, cur_after);
-        p.row_ptr = hd->dp.row_ptr;
-        p.col = hd->dp.col;
-        p.w = hd->dp.w;
+        const bool sat = hd->dp.kind == FEM_MAXSAT;
+        p.row_ptr = sat ? hd->dp.occ_ptr : hd->dp.row_ptr;
+        p.col = sat ? hd->dp.occ : hd->dp.col;
+        p.w = sat ? nullptr : hd->dp.w;
+        p.kst = 1;
+        while (p.kst < hd->dp.kstride) p.kst <<= 1;
         p.n = hd->dp.n;
         p.Rb = hd->Rb;
         p.blk_stride = hd->rows * hd->Rb;

@@ -159,7 +159,7 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
                     // probability the literal is false: 1-p = (1-m)/2 (positive literal), p = (1+m)/2 (negated)
                     const T sg = (pk[b][x] & 1u) ? (T)0.5 : (T)-0.5;
 #pragma unroll
-                    for (int v = 0; v < VEC; ++v) prod[v] *= (T)0.5 + sg * mr[b][x].v[v];
+                    for (int v = 0; v < VEC; ++v) prod[v] *= fma(sg, mr[b][x].v[v], (T)0.5);  // as in persist_q2_kernel
                 }
                 const bool positive = (pk[b][0] >> 31) != 0u;  // bit 31 of entry 0: own literal is positive
                 if (o + b < o1) {

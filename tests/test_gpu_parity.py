@@ -267,6 +267,9 @@ def _persist_cases():
         "ising_sparse": lambda: get("ising_sparse"),                                 # real weights, Ising sign
         "maxcut_er_n1500": lambda: (wl.erdos_renyi_maxcut(1500, 0.01, 2012, pm1=True), 12),   # 2 variables per thread
         "maxcut_torus_61x50": lambda: (wl.torus_maxcut(61, 2013, W=50), 20),          # 3050 nodes: 4 variables per thread
+        "maxsat_k4_n300": lambda: (wl.random_ksat(300, 2600, 4, 2014), 24),            # the paper's MaxSAT-2016 sizes (:179)
+        "maxsat_k3_odd_R": lambda: get("maxsat_k3_odd_R"),
+        "maxsat_k2_n1500": lambda: (wl.random_ksat(1500, 4000, 2, 2015), 10),          # 2 variables per thread
     }
 
 
