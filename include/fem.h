@@ -156,8 +156,8 @@ fem_status fem_energy_of(fem_handle *h, const int32_t *cfg /* [count][n] */, int
  * Results do not depend on either (replicas are independent).  Dense ISING only: "tensor_cores"
  * (1 = tcgen05 3xTF32 step, the default where it applies: n % 4 == 0 and R % 32 == 0; 0 = CUDA-core
  * GEMM) and "tc_tile_n" (replica columns per tensor-core tile: 0 = default, 32/64/128/256).
- * "persistent" (small sparse MAXCUT / ISING problems: 1 = replica-persistent cluster kernel where the problem
- * fits, the default; 0 = one launch per step; 1 + CS = force clusters of CS = 1, 2, 4 or 8 CTAs per replica) and
+ * "persistent" (small sparse MAXCUT / ISING / MAXSAT problems with few enough replicas to run in at most three
+ * waves of clusters: 1 = replica-persistent cluster kernel where the problem fits, the default; 0 = one launch per step; 1 + CS = force clusters of CS = 1, 2, 4 or 8 CTAs per replica) and
  * "potts_tma" (BMINCUT: 1 = rows staged by bulk asynchronous copies where the shape allows, the default; 0 =
  * register path).  Neither changes a single bit of the results.  Unknown key: FEM_EINVAL. */
 fem_status fem_set_option(fem_handle *h, const char *key, int64_t value);
