@@ -362,15 +362,21 @@ def main():
             # binding resource is warp-instruction issue (shared-memory gathers): per annealing step and replica,
             # 3 instructions per CSR entry (index LDS, value LDS, FADD) + ~45 per field (entropy gradient, Adam, tanh),
             # per warp of 32 fields.  Peak = 148 SMs x 4 schedulers x clocks.max.sm.
-            nnz = eng.info("nnz")
-            winst = (3.0 * nnz + 45.0 * n) / 32.0 * R * (N - K) * args.steps
+            if inst.kind == wl.MAXSAT:   # per occurrence: (k-1) x (index LDS, value LDS, FFMA, FMUL) + sign LDS, select, FADD
+                ks = int(np.diff(inst.clause_ptr).max()) - 1
+                nnz = int(inst.lits.size)
+                per_entry = 4.0 * ks + 3.0
+            else:
+                nnz = eng.info("nnz")
+                per_entry = 3.0
+            winst = (per_entry * nnz + 45.0 * n) / 32.0 * R * (N - K) * args.steps
             achieved = winst / (bulk_ms * 1e-3) / 1e9
             alu_peak = 148 * 4 * 1.965
             roofline = {"bound": "alu", "kernel": "persist_q2_kernel<float> (one CTA per replica, all steps in one launch)",
                         "achieved": achieved, "peak": alu_peak, "unit": "Gwarp-inst/s", "frac": achieved / alu_peak,
                         "traffic": load_traffic(args.workload),
-                        "peak_source": "148 SMs x 4 issue slots x 1.965 GHz (B200_PROFILING.md nominal clocks); only R of "
-                                       "148 SMs can be occupied (one CTA per replica)",
+                        "peak_source": "148 SMs x 4 issue slots x 1.965 GHz (B200_PROFILING.md nominal clocks); only R x cluster "
+                                       "size of the 148 SMs can be occupied (one cluster per replica)",
                         "kernel_us": kernel_us, "us_per_anneal_step": bulk_ms * 1e3 / ((N - K) * args.steps),
                         "kernel_share_of_step": bulk_ms / elapsed_ms}
         else:

@@ -203,5 +203,9 @@ CONFIGS = {
     "cfg3": Config("cfg3 Max-4-SAT n=20000 m=200000 R=128 N=2000", lambda: random_ksat(20000, 200000, 4, 1003), 128, 2000),
     "cfg4a": Config("cfg4a MaxCut 3-regular n=1000000 W=+-1 R=32 N=1000",
                     lambda: random_regular(1000000, 3, 1004, MAXCUT, pm1=True), 32, 1000),
+    # not a BASELINE.json config: the size of the paper's own MaxSAT-2016 instances (N 70-300, M 700-2600,
+    # 50-800 replicas, 50-500 steps; mean 0.074 s per instance on the paper's GPU), for the replica-persistent Max-SAT kernel
+    "sat2016": Config("sat2016 Max-4-SAT n=300 m=2600 R=128 N=500 (MaxSAT-2016-sized stand-in)",
+                      lambda: random_ksat(300, 2600, 4, 1006), 128, 500),
     "cfg4b": Config("cfg4b SK dense n=4096 J~N(0,1/n) R=1024 N=1000", lambda: sk_dense(4096, 1005), 1024, 1000),
 }
