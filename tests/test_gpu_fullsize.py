@@ -12,7 +12,7 @@ from test_oracle_gradient import as_problem
 pytestmark = pytest.mark.gpu
 
 # config -> replicas the oracle follows for 50 steps
-SUBSET = {"cfg0": 32, "cfg1": 4, "cfg2": 2, "cfg3": 4, "cfg4a": 2, "cfg4b": 2}
+SUBSET = {"cfg0": 32, "cfg1": 4, "cfg2": 2, "cfg3": 4, "cfg4a": 2, "cfg4b": 2, "sat2016": 128}
 
 
 @pytest.fixture(scope="module")
@@ -31,7 +31,7 @@ def instance(name):
     return _cache[name]
 
 
-@pytest.mark.parametrize("name", ["cfg0", "cfg1", "cfg2", "cfg3", "cfg4a", "cfg4b"])
+@pytest.mark.parametrize("name", ["cfg0", "cfg1", "cfg2", "cfg3", "cfg4a", "cfg4b", "sat2016"])
 def test_marginals_after_50_steps_full_size(fem, name):
     c = wl.CONFIGS[name]
     inst = instance(name)
@@ -57,7 +57,7 @@ def test_marginals_after_50_steps_full_size(fem, name):
     eng.close()
 
 
-@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3", "cfg4a", "cfg4b"])
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3", "cfg4a", "cfg4b", "sat2016"])
 def test_full_anneal_readout_properties(fem, name):
     """Properties that hold at any size: the reported energies are the oracle's energies of the reported
     configurations (bit-exact for the integer kinds), the rounding rule, the argmin and its tie-break."""
