@@ -167,14 +167,19 @@ static bool validate_graph(const fem_problem *pb, int64_t nnz, bool *integral, i
             if (w != std::nearbyint(w) || std::fabs(w) > 1e6f) *integral = false;
         }
     }
-    for (int i = 0; i < n; ++i)
-        for (int64_t e = pb->row_ptr[i]; e < pb->row_ptr[i + 1]; ++e) {
-            const int j = pb->col_idx[e];
-            const int32_t *lo = pb->col_idx + pb->row_ptr[j], *hi = pb->col_idx + pb->row_ptr[j + 1];
-            const int32_t *it = std::lower_bound(lo, hi, i);
-            if (it == hi || *it != i) return *err = "CSR is not symmetric", false;
-            if (pb->weight && pb->weight[it - pb->col_idx] != pb->weight[e]) return *err = "weights are not symmetric", false;
-        }
+    // symmetry in O(nnz): sweeping the rows i in ascending order, the entries (j, i) of any row j come up in ascending i,
+    // i.e. in the order row j stores them (columns are strictly ascending), so one cursor per row suffices
+    {
+        std::vector<int64_t> cursor(pb->row_ptr, pb->row_ptr + n);
+        for (int i = 0; i < n; ++i)
+            for (int64_t e = pb->row_ptr[i]; e < pb->row_ptr[i + 1]; ++e) {
+                const int j = pb->col_idx[e];
+                const int64_t c = cursor[j];
+                if (c >= pb->row_ptr[j + 1] || pb->col_idx[c] != i) return *err = "CSR is not symmetric", false;
+                if (pb->weight && pb->weight[c] != pb->weight[e]) return *err = "weights are not symmetric", false;
+                cursor[j] = c + 1;
+            }
+    }
     *uniform_deg = (uniform && d0 > 0 && d0 <= 64) ? (int)d0 : 0;
     int64_t mx = 0;
     for (int i = 0; i < n; ++i) mx = std::max<int64_t>(mx, pb->row_ptr[i + 1] - pb->row_ptr[i]);
