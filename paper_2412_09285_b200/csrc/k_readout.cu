@@ -141,6 +141,29 @@ __global__ void __launch_bounds__(kThreads) energy_dense_kernel(const ReadoutPar
     p.part_d[(int64_t)chunk * p.R + a] = acc;
 }
 
+// Dense Ising on the fp64 tensor-core GEMM: S = +-1 spins as doubles, F = J * S (launch_dense_field_f64), then
+// E_a = -1/2 sum_i S_ia F_ia (J symmetric with zero diagonal: sum_i s_i (J s)_i = 2 sum_{i<j} J_ij s_i s_j).
+__global__ void __launch_bounds__(kThreads) spins_f64_kernel(const int8_t *cfg, double *S, int n, int R, int Rb, int64_t cstride) {
+    const int64_t idx = (int64_t)blockIdx.x * kThreads + threadIdx.x;
+    if (idx >= (int64_t)n * R) return;
+    const int i = (int)(idx / R), a = (int)(idx - (int64_t)i * R);
+    S[idx] = (double)(2 * cfg[cfg_off(a, i, Rb, cstride)] - 1);
+}
+
+__global__ void __launch_bounds__(kThreads) energy_dense_reduce_kernel(const double *S, const double *F, int n, int R, int nchunks,
+                                                                       long long *part_i, double *part_d) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int a = blockIdx.y * 32 + lane;
+    const int chunk = blockIdx.x * 8 + warp;
+    if (a >= R) return;
+    double acc = 0.0;
+    for (int i = chunk; i < n; i += nchunks) acc += S[(int64_t)i * R + a] * F[(int64_t)i * R + a];
+    part_i[(int64_t)chunk * R + a] = 0;
+    part_d[(int64_t)chunk * R + a] = -0.5 * acc;
+}
+
+void launch_dense_field_f64(Handle *hd, const double *M, double *C, int n, int R);  // k_step_q2.cu
+
 struct FinalizeParams {
     int kind, n, q, R, nchunks, integral;
     double lambda;
@@ -273,7 +296,15 @@ static void run_energy(Handle *hd, int R, int Rb, double lambda) {
     dim3 grid((unsigned)nblocks, (unsigned)ceil_div(R, 32));
     if (dp.kind == FEM_MAXSAT)
         energy_sat_kernel<<<grid, kThreads, 0, hd->stream>>>(p);
-    else if (dp.kind == FEM_ISING && dp.J)
+    else if (dp.kind == FEM_ISING && dp.J && dp.n >= 256 && R >= 64) {
+        // scratch: the J*m buffer of the dense step and the gather array the next step overwrites (both n x R doubles)
+        double *S = hd->gW[hd->cur ^ 1], *F = reinterpret_cast<double *>(hd->field);
+        const int64_t tot = (int64_t)dp.n * R;
+        spins_f64_kernel<<<(unsigned)ceil_div(tot, kThreads), kThreads, 0, hd->stream>>>(hd->cfg, S, dp.n, R, Rb, p.cstride);
+        launch_dense_field_f64(hd, S, F, dp.n, R);
+        energy_dense_reduce_kernel<<<grid, kThreads, 0, hd->stream>>>(S, F, dp.n, R, p.nchunks, p.part_i, p.part_d);
+        hd->launches += 2;
+    } else if (dp.kind == FEM_ISING && dp.J)
         energy_dense_kernel<<<grid, kThreads, 0, hd->stream>>>(p);
     else if (dp.kind == FEM_ISING)
         energy_graph_kernel<FEM_ISING><<<grid, kThreads, 0, hd->stream>>>(p);

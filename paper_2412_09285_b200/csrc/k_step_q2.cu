@@ -389,6 +389,9 @@ static void launch_dense_field(Handle *hd, const T *M, T *C, int n, int Rb) {
     }
 }
 
+// C = J * M in fp64 for the dense readout (k_readout.cu): the DMMA kernel where the shape allows
+void launch_dense_field_f64(Handle *hd, const double *M, double *C, int n, int R) { launch_dense_field<double>(hd, M, C, n, R); }
+
 template <typename T, int VEC, int MODE>
 static void launch_q2_deg(Handle *hd, const Q2Params<T> &p, dim3 grid) {
     if constexpr (MODE == MODE_SAT) {
