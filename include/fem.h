@@ -11,8 +11,17 @@
  *
  * Conventions
  *   - All pointers in fem_problem / fem_schedule and all result pointers are HOST pointers.
- *     fem_create validates the problem on the host and uploads the device formats it builds.
- *     The only DEVICE pointer in this ABI is `workspace` (caller-owned, e.g. a torch tensor).
+ *     fem_create validates the problem on the host (symmetry, self loops, repeated variables: the
+ *     checks need the host copy) and uploads the device formats it builds (CSR / padded occurrence
+ *     table / split dense couplings).  The only DEVICE pointer in this ABI is `workspace`
+ *     (caller-owned, e.g. a torch tensor).  DESIGN.md section 3 (R15) records this reading.
+ *   - Coupling convention (R1): the exact gradient is that of U_MF = <E>, every edge counted
+ *     ONCE (Eq.6/Eq.9): dU/dp_i = sum_j W_ij m_j for MAXCUT, -sum_j W_ij P_j(s) for
+ *     BMINCUT.  The paper's listing and S21/S24/S26 count ordered pairs (a factor 2 on the coupling
+ *     term), so hyper-parameters quoted for the listing correspond to HALF the
+ *     temperature here (beta_here = 2 beta_listing for the coupling/entropy balance; for BMINCUT also
+ *     lambda_here = 2 lambda_listing).  The manipulated gradients (S25/S27/S30) carry no such factor
+ *     and are implemented term for term.
  *   - The library allocates no device memory: all state lives in the caller's workspace, which
  *     must stay alive and untouched until fem_destroy.  Host-side bookkeeping is freed by
  *     fem_destroy.
@@ -76,6 +85,8 @@ typedef struct {
 /* Annealing schedule and optimiser.  Step t = 0..steps-1 uses beta[t]
  * (inverse temperature) and Adam step count t+1. */
 typedef struct {
+    uint32_t struct_bytes; /* sizeof(fem_schedule) as the CALLER compiled it; fem_anneal returns FEM_EINVAL on any other
+                            * value, so a caller built against another ABI version is never read out of bounds */
     int32_t steps;
     const double *beta;   /* HOST [steps], > 0 */
     const double *lambda; /* HOST [steps] per-step balance weight, or NULL */
@@ -100,6 +111,14 @@ typedef struct {
 
 typedef enum { FEM_ADAM = 0, FEM_RMSPROP = 1, FEM_SGD = 2 } fem_optimizer;
 
+/* The two annealing schedules of the paper, t = 0..N-1, written to HOST beta_out[N]:
+ *   inverse-proportional (linear in temperature): T(t) = T_max + (T_min - T_max) t/(N-1), beta(t) = 1/T(t)
+ *   exponential: beta(t) = exp((ln beta_max - ln beta_min) t/(N-1) + ln beta_min)
+ * so that beta(0) = beta_min = 1/T_max and beta(N-1) = beta_max = 1/T_min; N = 1 gives beta(0).
+ * FEM_EINVAL: N < 1, NULL output, non-positive or non-finite endpoints.  Pure host arithmetic in double. */
+fem_status fem_schedule_inverse_proportional(double T_max, double T_min, int32_t N, double *beta_out);
+fem_status fem_schedule_exponential(double beta_min, double beta_max, int32_t N, double *beta_out);
+
 /* Bytes of device workspace fem_create needs for this problem with up to R_cap replicas
  * (0 on invalid arguments).  Pure host arithmetic. */
 size_t fem_workspace_bytes(const fem_problem *problem, int32_t R_cap);
@@ -115,7 +134,8 @@ fem_status fem_create(const fem_problem *problem, int32_t R_cap, void *workspace
  * already run since the last reset.  When t_done == 0 the Adam moments are zeroed and, unless fields
  * were injected with fem_set_fields, the fields are drawn from `seed` with the counter-based
  * generator of DESIGN.md section 3 (R4).  Asynchronous.  FEM_EINVAL: R < 1 or > R_cap, R differs
- * from the R of the steps already run, stop_after outside [t_done, steps], beta[t] <= 0.
+ * from the R of the steps already run, stop_after outside [t_done, steps], beta[t] <= 0, struct_bytes !=
+ * sizeof(fem_schedule), or optimizer / manipulated differ from the ones the trajectory was started with (t_done > 0).
  * One launch of the fused step kernel per step and replica block (one iteration
  * of the listing's loop). */
 fem_status fem_anneal(fem_handle *h, const fem_schedule *schedule, int32_t R, uint64_t seed, int32_t stop_after);

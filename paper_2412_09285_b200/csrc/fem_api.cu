@@ -241,7 +241,28 @@ using namespace fem;
 
 extern "C" {
 
-int32_t fem_abi_version(void) { return 2; }
+int32_t fem_abi_version(void) { return 3; }
+
+// a5: the two schedules, in double on the host.  beta(0) = beta_min, beta(N-1) = beta_max.
+fem_status fem_schedule_inverse_proportional(double T_max, double T_min, int32_t N, double *beta_out) {
+    if (N < 1 || !beta_out || !(T_max > 0) || !(T_min > 0) || !std::isfinite(T_max) || !std::isfinite(T_min)) return FEM_EINVAL;
+    for (int32_t t = 0; t < N; ++t) {
+        const double T = N > 1 ? T_max + (T_min - T_max) * (double)t / (double)(N - 1) : T_max;  // linear in temperature
+        beta_out[t] = 1.0 / T;
+    }
+    return FEM_OK;
+}
+
+fem_status fem_schedule_exponential(double beta_min, double beta_max, int32_t N, double *beta_out) {
+    if (N < 1 || !beta_out || !(beta_min > 0) || !(beta_max > 0) || !std::isfinite(beta_min) || !std::isfinite(beta_max))
+        return FEM_EINVAL;
+    const double l0 = std::log(beta_min), l1 = std::log(beta_max);
+    for (int32_t t = 0; t < N; ++t) {
+        const double x = N > 1 ? (double)t / (double)(N - 1) : 0.0;
+        beta_out[t] = std::exp((l1 - l0) * x + l0);
+    }
+    return FEM_OK;
+}
 
 const char *fem_last_error(const fem_handle *h) {
     return h ? reinterpret_cast<const Handle *>(h)->err.c_str() : g_create_error.c_str();
@@ -593,6 +614,7 @@ fem_status fem_get_marginals(fem_handle *h, float *marginals) {
 fem_status fem_anneal(fem_handle *h, const fem_schedule *sch, int32_t R, uint64_t seed, int32_t stop_after) {
     Handle *hd = reinterpret_cast<Handle *>(h);
     if (!hd || !sch) return FEM_EINVAL;
+    if (sch->struct_bytes != sizeof(fem_schedule)) return fail(hd, FEM_EINVAL, "fem_schedule.struct_bytes != sizeof(fem_schedule): caller built against another ABI version");
     if (R < 1 || R > hd->R_cap) return fail(hd, FEM_EINVAL, "R must be in 1..R_cap");
     if (sch->steps < 0 || (sch->steps > 0 && !sch->beta)) return fail(hd, FEM_EINVAL, "schedule needs beta[steps]");
     if (stop_after < hd->t_done || stop_after > sch->steps) return fail(hd, FEM_EINVAL, "stop_after must be in [t_done, steps]");
@@ -608,11 +630,16 @@ fem_status fem_anneal(fem_handle *h, const fem_schedule *sch, int32_t R, uint64_
     if (sch->manipulated != 0 && sch->manipulated != 1) return fail(hd, FEM_EINVAL, "manipulated must be 0 or 1");
     if (sch->manipulated && (!(sch->gamma_grad > 0) || !std::isfinite(sch->gamma_grad)))
         return fail(hd, FEM_EINVAL, "gamma_grad must be finite and > 0");
+    // the moment arrays and the gather buffers mean different things under another optimiser / gradient mode
+    if (hd->t_done > 0 && (sch->optimizer != hd->traj_optimizer || sch->manipulated != hd->traj_manipulated))
+        return fail(hd, FEM_EINVAL, "optimizer / manipulated cannot change inside a trajectory (fem_reset first)");
     for (int t = hd->t_done; t < stop_after; ++t)
         if (!(sch->beta[t] > 0) || !std::isfinite(sch->beta[t])) return fail(hd, FEM_EINVAL, "beta[t] must be finite and > 0");
 
     const int K = std::max(0, sch->precise_steps);
     if (hd->t_done == 0) {
+        hd->traj_optimizer = sch->optimizer;
+        hd->traj_manipulated = sch->manipulated;
         if (!hd->injected) {
             configure_R(hd, R);
             launch_init_fields(hd, seed, sch->init_scale);

@@ -11,7 +11,10 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <map>
+#include <set>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "../../include/fem.h"
@@ -82,7 +85,7 @@ struct Handle {
     // dense Ising on the tensor cores (k_dense_tc.cu): low parts of J and of the transposed gather buffers
     float *Jlo = nullptr, *glo[2] = {nullptr, nullptr};
     alignas(64) unsigned char tc_maps[6 * 128];  // CUtensorMap x6: J, Jlo, GT[0], GTlo[0], GT[1], GTlo[1]
-    int tc_maps_R = -1;
+    int tc_maps_R = -1, tc_maps_bn = -1;     // the maps bake in R (rows of GT) and the tile height bn
     bool tc_ready = false;                   // g[cur]/glo[cur] hold GT / GT_lo of the current fields
     double *rowsum = nullptr;  // graph kinds: sum_j |W_ij| per node (manipulated gradients: c_i, c^f_i, c^a_i)
     int bytes_per_field = 24;  // algorithmic HBM bytes per field per step: read + write of h and of the moments in use
@@ -100,6 +103,11 @@ struct Handle {
     int *best = nullptr;  // [0] = best replica, [1..n] = its configuration
     int cur = 0;          // g[cur] holds the gathered quantity of the current fields
     int t_done = 0;
+    int traj_optimizer = 0, traj_manipulated = 0;  // fixed at the first step of a trajectory
+    // per-handle (hence per-device) caches of the launch helpers: kernels whose shared-memory attribute is set,
+    // and resident-CTA counts from the occupancy calculator, keyed by kernel function (and shared-memory size)
+    std::set<const void *> attr_done;
+    std::map<std::pair<const void *, size_t>, int> resident_ctas;
     bool injected = false, readout_valid = false, gather_valid = false;
     int64_t opt_replica_block = 0, opt_steps_per_block = 0, opt_tensor_cores = 1, opt_tc_tile_n = 0;
     // small sparse two-state problems: replica-persistent kernel (k_persist_q2.cu).  0 = off, 1 = automatic cluster

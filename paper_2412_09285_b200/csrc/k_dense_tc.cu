@@ -329,12 +329,12 @@ int tc_tile_n(int n, int Rb, int forced) {  // 0 = tensor-core path not applicab
 template <int BN>
 static bool launch_tc(Handle *hd, const TcParams &p, const CUtensorMap *maps) {
     using S = TcShape<BN>;
-    static bool attr_set = false;
-    if (!attr_set) {
+    const void *fn = reinterpret_cast<const void *>(&dense_tc_step_kernel<BN>);
+    if (!hd->attr_done.count(fn)) {  // per handle, i.e. per device and context
         if (cudaFuncSetAttribute(dense_tc_step_kernel<BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::kSmem) !=
             cudaSuccess)
             return false;
-        attr_set = true;
+        hd->attr_done.insert(fn);
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)ceil_div(p.n, TC_BM), (unsigned)(p.Rb / BN));
@@ -361,13 +361,14 @@ bool launch_step_dense_tc(Handle *hd, const StepScalars &sc) {
     const int n = hd->dp.n, Rb = hd->Rb;
     const int bn = tc_tile_n(n, Rb, (int)hd->opt_tc_tile_n);
     if (bn == 0 || hd->R != Rb || !hd->Jlo || !hd->opt_tensor_cores) return false;
-    if (hd->tc_maps_R != hd->R) {  // tensor maps depend on R (rows of GT) -- rebuild when it changes
+    if (hd->tc_maps_R != hd->R || hd->tc_maps_bn != bn) {  // the maps bake in R (rows of GT) and the box height bn
         CUtensorMap *m = reinterpret_cast<CUtensorMap *>(hd->tc_maps);
         bool ok = make_map(&m[0], hd->dp.J, n, n, TC_BM) && make_map(&m[1], hd->Jlo, n, n, TC_BM);
         for (int k = 0; k < 2 && ok; ++k)
             ok = make_map(&m[2 + 2 * k], hd->g[k], hd->R, n, bn) && make_map(&m[3 + 2 * k], hd->glo[k], hd->R, n, bn);
         if (!ok) return false;
         hd->tc_maps_R = hd->R;
+        hd->tc_maps_bn = bn;
     }
     if (!hd->tc_ready) {
         dim3 grid((unsigned)ceil_div(n, 32), (unsigned)ceil_div(Rb, 32));
@@ -396,6 +397,10 @@ bool launch_step_dense_tc(Handle *hd, const StepScalars &sc) {
     if (ok) {
         hd->launches++;
         hd->tc_launches++;
+    } else {
+        (void)cudaGetLastError();
+        // g[cur] was overwritten with the TRANSPOSED layout above: the CUDA-core path must rebuild it from h
+        // (launch_step_q2_t does so when it sees tc_ready)
     }
     return ok;
 }

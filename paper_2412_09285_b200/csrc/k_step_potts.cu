@@ -44,11 +44,9 @@ __device__ __forceinline__ double shfl_any(double v, int src) { return __shfl_sy
 
 constexpr int kGatherChunk = 5;  // neighbour rows in flight per lane
 
-#ifndef POTTS_EXACT_MIN
-#define POTTS_EXACT_MIN 4
-#endif
+constexpr int kTeamMinCtas = 4;  // CTAs per SM the exact-gradient kernel is compiled for (measured optimum)
 template <typename T, int QPAD, int VEC, bool STEP, bool DISC, bool UNITW>
-__global__ void __launch_bounds__(kThreads, DISC ? 3 : POTTS_EXACT_MIN) potts_team_kernel(const PottsParams<T> p) {
+__global__ void __launch_bounds__(kThreads, DISC ? 3 : kTeamMinCtas) potts_team_kernel(const PottsParams<T> p) {
     using R = Row<T, VEC>;
     constexpr int kStages = QPAD == 32 ? 5 : QPAD == 16 ? 4 : QPAD == 8 ? 3 : QPAD == 4 ? 2 : 1;
     __shared__ unsigned long long cta_sum[32 * VEC];
@@ -296,8 +294,8 @@ __global__ void __launch_bounds__(kThreads, DISC ? 3 : POTTS_EXACT_MIN) potts_te
 // grid-stride kernel: never more CTAs than are resident at once (occupancy x SMs), so no second wave
 template <typename T, int QPAD, int VEC, bool STEP, bool DISC, bool UNITW>
 static void launch_potts_w(Handle *hd, const PottsParams<T> &p, dim3 grid) {
-    static std::map<int, int> resident;  // per device SM count: CTAs resident at once for THIS instantiation
-    int &r = resident[hd->sm_count];
+    // CTAs resident at once for THIS instantiation, cached per handle (= per device and context)
+    int &r = hd->resident_ctas[{reinterpret_cast<const void *>(&potts_team_kernel<T, QPAD, VEC, STEP, DISC, UNITW>), 0}];
     if (r == 0) {
         int occ = 0;
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, potts_team_kernel<T, QPAD, VEC, STEP, DISC, UNITW>, kThreads,

@@ -323,8 +323,9 @@ bool potts_tma_applicable(const Handle *hd) {
 
 template <int QPAD, bool UNITW, bool DISC>
 static cudaError_t launch_tma_one(Handle *hd, const PottsTmaParams &p, int blk_count, size_t smem) {
-    static std::map<size_t, int> resident_of;  // CTAs resident at once, per ring size (the degree sets it)
-    int &resident = resident_of[smem];
+    // CTAs resident at once, per ring size (the degree sets it), cached per handle (= per device and context)
+    const void *fn = reinterpret_cast<const void *>(&potts_tma_kernel<QPAD, UNITW, DISC>);
+    int &resident = hd->resident_ctas[{fn, smem}];
     if (resident == 0) {
         const size_t smem_max = (size_t)kTmaWarps * (3 + kTmaMaxDeg) * 128 * sizeof(float);
         cudaError_t e = cudaFuncSetAttribute(potts_tma_kernel<QPAD, UNITW, DISC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);

@@ -426,6 +426,7 @@ static void launch_q2_mode(Handle *hd, const Q2Params<T> &p, dim3 grid, int mode
 }
 
 bool launch_step_dense_tc(Handle *hd, const StepScalars &sc);  // k_dense_tc.cu
+void launch_prepare_q2(Handle *hd, bool wide);
 
 template <typename T>
 static void launch_step_q2_t(Handle *hd, const StepScalars &sc, int blk_begin, int blk_count) {
@@ -433,6 +434,12 @@ static void launch_step_q2_t(Handle *hd, const StepScalars &sc, int blk_begin, i
     if (std::is_same<T, float>::value && hd->dp.kind == FEM_ISING && hd->dp.J && blk_begin == 0 && blk_count == 1 && hd->plain_adam &&
         launch_step_dense_tc(hd, sc))
         return;  // dense couplings: tcgen05 GEMM with the update fused in its epilogue
+    if (std::is_same<T, float>::value && hd->tc_ready) {
+        // a tensor-core step (or its preparation) left g[cur] in the TRANSPOSED layout GT[a][i]; this path reads
+        // g[cur] as [i][Rb].  Rebuild it from the fields before gathering from it.
+        hd->tc_ready = false;
+        launch_prepare_q2(hd, false);
+    }
     const int Rb = hd->Rb;
     const int64_t base = (int64_t)blk_begin * hd->rows * Rb;
     Q2Params<T> p;

@@ -25,6 +25,7 @@ EXPORTS = [
     "fem_abi_version", "fem_workspace_bytes", "fem_create", "fem_anneal", "fem_reset", "fem_readout", "fem_result",
     "fem_set_fields", "fem_get_fields", "fem_get_moments", "fem_get_marginals", "fem_get_configs", "fem_energy_of",
     "fem_set_option", "fem_get_info", "fem_last_error", "fem_destroy",
+    "fem_schedule_inverse_proportional", "fem_schedule_exponential",
 ]
 
 
@@ -44,7 +45,7 @@ class CProblem(C.Structure):
 
 class CSchedule(C.Structure):
     _fields_ = [
-        ("steps", C.c_int32), ("beta", C.c_void_p), ("lambda_", C.c_void_p),
+        ("struct_bytes", C.c_uint32), ("steps", C.c_int32), ("beta", C.c_void_p), ("lambda_", C.c_void_p),
         ("lr", C.c_double), ("beta1", C.c_double), ("beta2", C.c_double), ("eps", C.c_double),
         ("weight_decay", C.c_double), ("init_scale", C.c_double), ("precise_steps", C.c_int32),
         ("optimizer", C.c_int32), ("alpha", C.c_double), ("momentum", C.c_double), ("dampening", C.c_double),
@@ -88,6 +89,8 @@ def load_library():
     lib.fem_last_error.restype = C.c_char_p
     lib.fem_last_error.argtypes = [C.c_void_p]
     lib.fem_destroy.argtypes = [C.c_void_p]
+    lib.fem_schedule_inverse_proportional.argtypes = [C.c_double, C.c_double, C.c_int32, C.c_void_p]
+    lib.fem_schedule_exponential.argtypes = [C.c_double, C.c_double, C.c_int32, C.c_void_p]
     _lib = lib
     return lib
 
@@ -119,22 +122,27 @@ class Schedule:
         self.beta = np.ascontiguousarray(self.beta, dtype=np.float64)
         if self.lam is not None:
             self.lam = np.ascontiguousarray(self.lam, dtype=np.float64)
-        return CSchedule(int(self.beta.size), _ptr(self.beta), _ptr(self.lam), self.lr, self.beta1, self.beta2, self.eps,
+        return CSchedule(C.sizeof(CSchedule), int(self.beta.size), _ptr(self.beta), _ptr(self.lam), self.lr, self.beta1, self.beta2, self.eps,
                          self.weight_decay, self.init_scale, self.precise_steps, int(self.optimizer), self.alpha,
                          self.momentum, self.dampening, 1 if self.manipulated else 0, self.gamma_grad)
 
 
+def _schedule(fn_name: str, a: float, b: float, steps: int) -> np.ndarray:
+    out = np.empty(int(steps), dtype=np.float64)
+    st = getattr(load_library(), fn_name)(float(a), float(b), int(steps), _ptr(out))
+    if st != FEM_OK:
+        raise FemError(st, f"{fn_name}({a}, {b}, {steps})")
+    return out
+
+
 def linear_temperature_schedule(T_max: float, T_min: float, steps: int) -> np.ndarray:
-    """Inverse-proportional schedule: T linear from T_max to T_min; returns beta[t] = 1/T(t)."""
-    t = np.arange(steps, dtype=np.float64)
-    T = T_max + (T_min - T_max) * t / max(steps - 1, 1)
-    return 1.0 / T
+    """fem_schedule_inverse_proportional: T linear from T_max to T_min; returns beta[t] = 1/T(t)."""
+    return _schedule("fem_schedule_inverse_proportional", T_max, T_min, steps)
 
 
 def exponential_schedule(beta_min: float, beta_max: float, steps: int) -> np.ndarray:
-    """Exponential schedule."""
-    t = np.arange(steps, dtype=np.float64) / max(steps - 1, 1)
-    return np.exp((np.log(beta_max) - np.log(beta_min)) * t + np.log(beta_min))
+    """fem_schedule_exponential (PAPER.md:270-274)."""
+    return _schedule("fem_schedule_exponential", beta_min, beta_max, steps)
 
 
 class Fem:

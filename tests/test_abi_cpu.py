@@ -27,11 +27,11 @@ def declared_symbols():
 
 def test_every_declared_symbol_is_exported(lib):
     names = declared_symbols()
-    assert len(names) >= 17
+    assert len(names) >= 19
     for name in names:
         assert hasattr(lib, name), name
     assert sorted(fem.EXPORTS) == names
-    assert lib.fem_abi_version() == 2
+    assert lib.fem_abi_version() == 3
 
 
 def cproblem(inst, keep):
@@ -126,3 +126,29 @@ def test_schedule_helpers_match_the_paper_endpoints():
     assert b[0] == 1.0 and abs(b[-1] - 100.0) < 1e-9 and np.all(np.diff(b) > 0)
     e = fem.exponential_schedule(0.02, 750.0, 100)
     assert abs(e[0] - 0.02) < 1e-15 and abs(e[-1] - 750.0) < 1e-9
+
+
+def test_schedules_behind_the_abi_equal_the_oracles(lib):
+    """a5 lives behind the C ABI (fem_schedule_*): same arithmetic order as the paper's formulas, so
+    the arrays are bit-identical to the oracle's; N = 1 gives beta(0); bad arguments are rejected."""
+    from oracle import fem_oracle as fo
+    for N in (1, 2, 7, 500, 2000):
+        assert np.array_equal(fem.linear_temperature_schedule(1.0, 0.01, N), fo.schedule_inverse_proportional(1.0, 0.01, N))
+        assert np.array_equal(fem.linear_temperature_schedule(2.5, 0.3, N), fo.schedule_inverse_proportional(2.5, 0.3, N))
+        a, b = fem.exponential_schedule(0.02, 750.0, N), fo.schedule_exponential(0.02, 750.0, N)
+        ulp = np.abs(a.view(np.int64) - b.view(np.int64))
+        assert ulp.max() <= 1, ulp.max()                  # exp / log come from two different libm builds at most 1 ulp apart
+    out = np.empty(4)
+    ptr = out.ctypes.data_as(C.c_void_p)
+    assert lib.fem_schedule_inverse_proportional(1.0, 0.01, 0, ptr) == fem.FEM_EINVAL
+    assert lib.fem_schedule_inverse_proportional(1.0, -0.01, 4, ptr) == fem.FEM_EINVAL
+    assert lib.fem_schedule_inverse_proportional(1.0, 0.01, 4, None) == fem.FEM_EINVAL
+    assert lib.fem_schedule_exponential(0.0, 5.0, 4, ptr) == fem.FEM_EINVAL
+    assert lib.fem_schedule_exponential(0.1, float("inf"), 4, ptr) == fem.FEM_EINVAL
+    with pytest.raises(fem.FemError):
+        fem.exponential_schedule(-1.0, 5.0, 10)
+
+
+def test_schedule_struct_carries_its_size():
+    sch = fem.Schedule(beta=np.ones(3)).c()
+    assert sch.struct_bytes == C.sizeof(fem.CSchedule) and sch.steps == 3

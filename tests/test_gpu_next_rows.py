@@ -150,6 +150,71 @@ def test_manipulated_full_anneal_quality_cfg0(fem):
     eng.close()
 
 
+@pytest.mark.parametrize("manipulated", [False, True])
+@pytest.mark.parametrize("name", ["bmincut_q8_reg10", "bmincut_q5_weighted", "bmincut_q3_reg6_odd_R"])
+def test_lambda_ramp(fem, name, manipulated):
+    """The balance weight incremented linearly from 0 to lambda_max over the N steps (Table S3 :842)
+    through fem_schedule.lambda[]: wide phase over 50 steps against the oracle's anneal(lam_t), then the fp32 kernels
+    (TMA-staged and register Potts paths) for the rest of the ramp; the readout uses the LAST step's lambda."""
+    inst, R = get(name)
+    N = 120
+    beta = fem.exponential_schedule(0.5, 30.0, N)
+    lam = np.linspace(0.0, 0.2, N)
+    h0 = fo.init_fields(4, R, inst.n, inst.fields_per_var).astype(np.float32)
+    pb = as_problem(inst)
+    opt = fo.Optimizer(kind=fo.ADAM, lr=0.05)
+    st = fo.anneal_ex(fo.State(pb, h0.astype(np.float64)), beta, opt, 123.0, lam_t=lam, t_end=50,
+                      manipulated=manipulated, gamma=0.9)
+    for K, tol in ((50, WIDE_TOL), (8, MARGINAL_TOL)):
+        if K == 8 and manipulated:
+            continue                     # one-hot decisions inside fp32 steps: covered step by step below
+        eng = fem.Fem(inst, R)
+        eng.set_fields(h0)
+        eng.anneal(fem.Schedule(beta=beta, lam=lam, lr=0.05, precise_steps=K, manipulated=manipulated, gamma_grad=0.9), R,
+                   stop_after=50)
+        P = eng.get_marginals().astype(np.float64)
+        err = np.max(np.abs(P - fo.marginals(pb, st.h).reshape(P.shape)))
+        assert err < tol, (K, err)
+        eng.close()
+    # fp32 kernels one step at a time along the ramp, from the GPU's own state
+    sch = fem.Schedule(beta=beta, lam=lam, lr=0.05, precise_steps=4, manipulated=manipulated, gamma_grad=0.9)
+    eng = fem.Fem(inst, R)
+    eng.set_fields(h0)
+    eng.anneal(sch, R, stop_after=60)
+    for t in range(60, 64):
+        h = eng.get_fields()
+        m1, m2 = eng.get_moments()
+        s2 = fo.State(pb, h.astype(np.float64))
+        s2.m1, s2.m2, s2.t = m1.astype(np.float64).reshape(s2.h.shape), m2.astype(np.float64).reshape(s2.h.shape), t
+        fo.anneal_ex(s2, beta, opt, 123.0, lam_t=lam, t_end=t + 1, manipulated=manipulated, gamma=0.9)
+        eng.anneal(sch, R, stop_after=t + 1)
+        h1 = eng.get_fields().astype(np.float64)
+        assert np.all(np.abs(h1 - s2.h.reshape(h1.shape)) <= 2e-5 * np.maximum(1.0, np.abs(h1))), t
+    # the whole ramp; energies reported with lambda_max (the last step's value)
+    eng.anneal(sch, R)
+    res = eng.result()
+    cfg = eng.get_configs()
+    e_int, e_real, part = fo.energies(pb, cfg, float(lam[-1]))
+    assert np.array_equal(res["energy_int"], e_int) and np.array_equal(res["energy"], e_real)
+    assert np.array_equal(res["part_sizes"], part)
+    eng.close()
+
+
+def test_optimiser_cannot_change_inside_a_trajectory(fem):
+    inst, R = get("maxcut_torus_30x34")
+    beta = fem.linear_temperature_schedule(1.0, 0.01, 20)
+    eng = fem.Fem(inst, R)
+    eng.anneal(fem.Schedule(beta=beta), R, stop_after=10)
+    with pytest.raises(fem.FemError):
+        eng.anneal(fem.Schedule(beta=beta, optimizer=2, lr=0.5), R)
+    with pytest.raises(fem.FemError):
+        eng.anneal(fem.Schedule(beta=beta, manipulated=True), R)
+    eng.anneal(fem.Schedule(beta=beta), R)           # the same optimiser continues
+    eng.reset()
+    eng.anneal(fem.Schedule(beta=beta, optimizer=2, lr=0.5), R)   # a new trajectory may use another
+    eng.close()
+
+
 def test_bad_optimiser_arguments_are_rejected(fem):
     inst, R = get("maxcut_torus_30x34")
     beta = fem.linear_temperature_schedule(1.0, 0.01, 10)

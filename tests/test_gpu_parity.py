@@ -260,6 +260,47 @@ def test_dense_tensor_core_path_is_taken_and_agrees_with_cuda_cores(fem):
     assert np.max(np.abs(out[1] - out[0])) < MARGINAL_TOL
 
 
+@pytest.mark.parametrize("bn", [32, 64, 128, 256])
+def test_dense_tensor_core_every_tile_size(fem, bn):
+    """Each replica-tile width of the tcgen05 step (tc_tile_n) against the oracle, and two tile sizes one after the
+    other on ONE handle (the tensor maps bake in the box height: they are rebuilt when it changes)."""
+    inst = wl.sk_dense(328, 2011)
+    R = 256                                                        # divisible by every tile width
+    beta = fem.linear_temperature_schedule(1.0, 0.01, 500)
+    h0 = fo.init_fields(5, R, inst.n, 1).astype(np.float32)
+    pb, st = oracle_run(inst, h0[:24], beta, 30, inst.lam)         # the oracle follows 24 of the replicas
+    P_ref = fo.marginals(pb, st.h).reshape(24, inst.n)
+    eng = fem.Fem(inst, R)
+    for tile in (bn, 64 if bn != 64 else 128):
+        eng.reset()
+        eng.set_option("tc_tile_n", tile)
+        eng.set_fields(h0)
+        eng.anneal(fem.Schedule(beta=beta, precise_steps=8), R, stop_after=30)
+        P = eng.get_marginals().astype(np.float64)[:24]
+        assert np.max(np.abs(P - P_ref)) < MARGINAL_TOL, tile
+    assert eng.info("tc_launches") == 44
+    eng.close()
+
+
+def test_dense_tensor_core_phase_resumes_anywhere(fem):
+    """Resume points inside the tensor-core phase with the parity hooks called in between (the hooks use the spare
+    gather buffer as scratch; the transposed gather layout of this phase must survive them)."""
+    inst, R = get("ising_dense_sk_tc")
+    beta = fem.linear_temperature_schedule(1.0, 0.01, 500)
+    h0 = fo.init_fields(5, R, inst.n, 1).astype(np.float32)
+    pb, st = oracle_run(inst, h0, beta, 30, inst.lam)
+    eng = fem.Fem(inst, R)
+    eng.set_fields(h0)
+    sch = fem.Schedule(beta=beta, precise_steps=8)
+    for stop in (12, 13, 21, 30):                                  # resume points inside the tensor-core phase
+        eng.anneal(sch, R, stop_after=stop)
+        eng.get_marginals()
+    P = eng.get_marginals().astype(np.float64)
+    assert np.max(np.abs(P - fo.marginals(pb, st.h).reshape(P.shape))) < MARGINAL_TOL
+    assert eng.info("tc_launches") == 22
+    eng.close()
+
+
 def _persist_cases():
     return {
         "cfg0_maxcut_er800": lambda: get("cfg0_maxcut_er800"),                       # unit weights, 1 variable per thread

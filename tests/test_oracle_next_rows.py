@@ -199,3 +199,92 @@ def test_manipulated_anneal_reaches_brute_force_optimum(kind):
         e = fo.energies(pb, fo.round_configs(pb, st.h))[1]
         hits += int(round(-e.min()) == round(_brute_force_maxcut(inst)))
     assert hits >= 7, hits
+
+
+# --------------------------------------------------- Potts manipulated gradient on a weighted, irregular graph
+def _general_form_potts(inst, h, beta, lam, gamma, global_rowsum=False):
+    """S27 + S20 written over explicit states with a DENSE weight matrix:
+    ghat^p = -c^f (W e) + lambda c^a [1 (1^T e) - e] + (1/beta)[ln P + 1],  c^f_i = q / sum_j W_ij,
+    c^a_i = q / sqrt(sum_j W_ij) per NODE;  g^h = gamma P (ghat^p - <ghat^p>_P)."""
+    n, q = inst.n, inst.q
+    W = np.zeros((n, n))
+    rows = np.repeat(np.arange(n), np.diff(inst.row_ptr))
+    W[rows, inst.col_idx] = np.ones(inst.nnz) if inst.weight is None else inst.weight.astype(np.float64)
+    assert np.array_equal(W, W.T)
+    H = h.reshape(n, q)
+    P = np.exp(H - H.max(1, keepdims=True))
+    P /= P.sum(1, keepdims=True)
+    e = np.zeros((n, q))
+    e[np.arange(n), np.argmax(H, axis=1)] = 1.0        # numpy's argmax returns the lowest index among ties (R3)
+    rs = W.sum(1)
+    ok = rs > 0
+    if global_rowsum:                                  # (deliberately wrong variant, used to show the pin has teeth)
+        rs = np.where(ok, rs[ok].mean(), 0.0)
+    cf = np.where(ok, q / np.where(ok, rs, 1.0), 0.0)
+    ca = np.where(ok, q / np.sqrt(np.where(ok, rs, 1.0)), 0.0)
+    ghat = -cf[:, None] * (W @ e) + lam * ca[:, None] * (e.sum(0)[None, :] - e) + (np.log(P) + 1.0) / beta
+    return (gamma * P * (ghat - (P * ghat).sum(1, keepdims=True))).ravel()
+
+
+def _weighted_irregular_potts(n, q, seed, lam):
+    """Erdos-Renyi graph (irregular degrees, maybe an isolated node) with real positive weights of very different sizes."""
+    rng = np.random.default_rng(seed)
+    iu, ju = np.triu_indices(n, k=1)
+    keep = rng.random(iu.size) < 0.3
+    keep[iu == n - 1] = False
+    keep[ju == n - 1] = False                          # node n-1 isolated: c^f = c^a = 0
+    u, v = iu[keep], ju[keep]
+    w = (rng.random(u.size) * 3.0 + 0.05) * 10.0 ** rng.integers(-1, 2, size=u.size)
+    row_ptr, col, weight = wl.csr_from_edges(n, u, v, w)
+    return wl.Instance(wl.BMINCUT, n, q, row_ptr, col, weight, lam=lam)
+
+
+@pytest.mark.parametrize("q,beta,gamma", [(3, 0.7, 1.0), (5, 2.5, 0.6), (8, 11.0, 2.0)])
+def test_potts_manipulated_gradient_on_a_weighted_irregular_graph_is_s27_with_per_node_factors(q, beta, gamma):
+    inst = _weighted_irregular_potts(13, q, 40 + q, lam=0.37)
+    deg = np.diff(inst.row_ptr)
+    assert deg.min() == 0 and len(set(deg.tolist())) > 3            # irregular, with an isolated node
+    rs = np.bincount(np.repeat(np.arange(inst.n), deg), weights=inst.weight.astype(np.float64), minlength=inst.n)
+    assert rs[rs > 0].max() / rs[rs > 0].min() > 3.0                 # per-node factors differ a lot
+    rng = np.random.default_rng(41)
+    h = rng.normal(size=(inst.n, q)) * 1.2
+    h[2, 1] = h[2, 3 % q] = h[2].max() + 0.5                          # a tie among the maxima: lowest state wins
+    g = fo.grad_h_manipulated(as_problem(inst), h.ravel(), beta, inst.lam, gamma)
+    ref = _general_form_potts(inst, h.ravel(), beta, inst.lam, gamma)
+    assert np.max(np.abs(g - ref)) <= 1e-13 * max(1.0, np.max(np.abs(ref)))
+    # a mistake this pin is there to catch -- one global row sum instead of one per node -- is far outside the tolerance
+    wrong = _general_form_potts(inst, h.ravel(), beta, inst.lam, gamma, global_rowsum=True)
+    assert np.max(np.abs(wrong - ref)) > 1e-3 * np.max(np.abs(ref))
+
+
+# -------------------------------------------------------------------------------------- per-step lambda (the ramp)
+@pytest.mark.parametrize("manipulated", [False, True])
+def test_anneal_with_a_lambda_ramp_is_step_by_step_grad_with_that_steps_lambda(manipulated):
+    """PAPER.md:828, Table S3 :842: lambda is incremented linearly from 0 to lambda_max over the N steps.  anneal(lam_t)
+    must equal: for t, g = grad(h, beta[t], lam_t[t]); Adam(t + 1) -- composed here from the separately pinned pieces."""
+    inst = _weighted_irregular_potts(12, 4, 77, lam=123.0)            # inst.lam must be IGNORED when lam_t is given
+    pb = as_problem(inst)
+    N, R = 30, 3
+    beta = fo.schedule_exponential(0.3, 20.0, N)
+    lam_t = np.linspace(0.0, 0.2, N)
+    h0 = fo.init_fields(5, R, inst.n, inst.q)
+    adam = fo.Adam(lr=0.05, weight_decay=0.01)
+    if manipulated:
+        st = fo.anneal_ex(fo.State(pb, h0), beta, fo.Optimizer(kind=fo.ADAM, lr=0.05, weight_decay=0.01), inst.lam,
+                          lam_t=lam_t, manipulated=True, gamma=0.9)
+    else:
+        st = fo.anneal(fo.State(pb, h0), beta, adam, inst.lam, lam_t=lam_t)
+    h = h0.reshape(R, -1).copy()
+    m1, m2 = np.zeros_like(h), np.zeros_like(h)
+    for t in range(N):
+        for a in range(R):
+            g = (fo.grad_h_manipulated(pb, h[a], beta[t], lam_t[t], 0.9) if manipulated
+                 else fo.grad_h(pb, h[a], beta[t], lam_t[t]))
+            fo.adam_update(adam, t + 1, h[a], m1[a], m2[a], g)
+    assert np.array_equal(st.h.reshape(R, -1), h)
+    # and the ramp matters: the constant-lambda anneal ends elsewhere
+    other = fo.anneal(fo.State(pb, h0), beta, adam, 0.2)
+    assert np.max(np.abs(other.h - st.h)) > 1e-3
+    # lambda_t[t] = lambda for all t is the constant-lambda anneal, bit for bit
+    same = fo.anneal(fo.State(pb, h0), beta, adam, 999.0, lam_t=np.full(N, 0.2))
+    assert np.array_equal(same.h, other.h)
