@@ -513,6 +513,9 @@ fem_status fem_set_option(fem_handle *h, const char *key, int64_t value) {
     } else if (!strcmp(key, "potts_tma")) {
         if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "potts_tma must be 0 or 1");
         hd->opt_potts_tma = value;
+    } else if (!strcmp(key, "potts_lane")) {
+        if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "potts_lane must be 0 or 1");
+        hd->opt_potts_lane = value;
     } else if (!strcmp(key, "tensor_cores")) {
         if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "tensor_cores must be 0 or 1");
         hd->opt_tensor_cores = value;
@@ -530,6 +533,7 @@ int64_t fem_get_info(const fem_handle *h, const char *key) {
     if (!strcmp(key, "persist_launches")) return hd->persist_launches;
     if (!strcmp(key, "persist_cluster")) return hd->persist_cluster;
     if (!strcmp(key, "tma_launches")) return hd->tma_launches;
+    if (!strcmp(key, "lane_launches")) return hd->lane_launches;
     if (!strcmp(key, "t_done")) return hd->t_done;
     if (!strcmp(key, "R")) return hd->R;
     if (!strcmp(key, "replica_block")) return hd->Rb;
