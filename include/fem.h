@@ -179,11 +179,12 @@ fem_status fem_energy_of(fem_handle *h, const int32_t *cfg /* [count][n] */, int
  * "persistent" (small sparse MAXCUT / ISING / MAXSAT problems with few enough replicas to run in at most three
  * waves of clusters: 1 = replica-persistent cluster kernel where the problem fits, the default; 0 = one launch per step; 1 + CS = force clusters of CS = 1, 2, 4 or 8 CTAs per replica) and
  * "potts_tma" (BMINCUT: 1 = rows staged by bulk asynchronous copies where the shape allows, the default; 0 =
- * register path).  Neither changes a single bit of the results.  Unknown key: FEM_EINVAL. */
+ * register path) and "potts_lane" (BMINCUT, q <= 8, replica blocks of 8 / 16 / 32: 1 = the lane-per-replica kernel, k_step_potts_lane.cu;
+ * 0 = the default).  None of them changes a single bit of the results.  Unknown key: FEM_EINVAL. */
 fem_status fem_set_option(fem_handle *h, const char *key, int64_t value);
 /* Introspection for benchmarks: "launches" (kernels enqueued so far), "tc_launches" (of which tcgen05
  * dense steps), "persist_launches", "persist_cluster" (CTAs per replica of the persistent kernel),
- * "tma_launches" (TMA-staged Potts steps), "t_done", "R", "replica_block", "nnz", "uniform_degree",
+ * "tma_launches" (TMA-staged Potts steps), "lane_launches" (lane-per-replica Potts steps), "t_done", "R", "replica_block", "nnz", "uniform_degree",
  * "integral_weights", "step_bytes" (algorithmic HBM bytes of one fused step of the last schedule's optimiser,
  * DESIGN.md section 6).  Unknown key: -1. */
 int64_t fem_get_info(const fem_handle *h, const char *key);

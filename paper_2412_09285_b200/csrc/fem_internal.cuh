@@ -116,7 +116,8 @@ struct Handle {
     int64_t persist_launches = 0, persist_cluster = 0;
     int64_t opt_potts_tma = 1;    // Potts step with TMA-staged rows (k_step_potts_tma.cu) where it applies
     int64_t tma_launches = 0;
-    int64_t opt_potts_lane = 1;   // Potts step with a lane per replica (k_step_potts_lane.cu) where it applies
+    int64_t opt_potts_lane = 0;   // Potts step with a lane per replica (k_step_potts_lane.cu): measured slower than the
+                                  // TMA-staged team kernel on cfg 2, so off unless asked for
     int64_t lane_launches = 0;
     int64_t persist_ell[4] = {-1, -1, -1, -1};  // sliced-ELL entries per CTA for cluster sizes 1, 2, 4, 8
     int sm_count = 148;
