@@ -189,6 +189,12 @@ fem_status fem_set_option(fem_handle *h, const char *key, int64_t value);
  * DESIGN.md section 6).  Unknown key: -1. */
 int64_t fem_get_info(const fem_handle *h, const char *key);
 
+/* Measurement helper (not on the hot path): L2 -> SM read rate of the current device in GB/s.  `buffer` is a DEVICE
+ * pointer (16-byte aligned) to `bytes` (1 MiB .. 96 MiB, a multiple of 16; it is overwritten with zeros), read `repeats`
+ * times from all SMs with 16-byte loads that bypass L1, timed with CUDA events on `cuda_stream`; synchronous.  bench.py
+ * compares the L2-resident Max-SAT step (cfg 3) with this roof.  FEM_EINVAL on bad arguments, FEM_ECUDA without a device. */
+fem_status fem_probe_l2_read(void *buffer, size_t bytes, int32_t repeats, void *cuda_stream, double *gigabytes_per_second);
+
 const char *fem_last_error(const fem_handle *h); /* h may be NULL: last create-time error */
 void fem_destroy(fem_handle *h);
 int32_t fem_abi_version(void);

@@ -25,7 +25,7 @@ EXPORTS = [
     "fem_abi_version", "fem_workspace_bytes", "fem_create", "fem_anneal", "fem_reset", "fem_readout", "fem_result",
     "fem_set_fields", "fem_get_fields", "fem_get_moments", "fem_get_marginals", "fem_get_configs", "fem_energy_of",
     "fem_set_option", "fem_get_info", "fem_last_error", "fem_destroy",
-    "fem_schedule_inverse_proportional", "fem_schedule_exponential",
+    "fem_schedule_inverse_proportional", "fem_schedule_exponential", "fem_probe_l2_read",
 ]
 
 
@@ -91,6 +91,7 @@ def load_library():
     lib.fem_destroy.argtypes = [C.c_void_p]
     lib.fem_schedule_inverse_proportional.argtypes = [C.c_double, C.c_double, C.c_int32, C.c_void_p]
     lib.fem_schedule_exponential.argtypes = [C.c_double, C.c_double, C.c_int32, C.c_void_p]
+    lib.fem_probe_l2_read.argtypes = [C.c_void_p, C.c_size_t, C.c_int32, C.c_void_p, C.POINTER(C.c_double)]
     _lib = lib
     return lib
 
@@ -277,6 +278,20 @@ class Fem:
 
     def info(self, key: str) -> int:
         return int(self._lib.fem_get_info(self._h, key.encode()))
+
+
+def probe_l2_read(device: str = "cuda:0", mib: int = 32, repeats: int = 200) -> float:
+    """fem_probe_l2_read on a torch-owned buffer: the L2 -> SM read rate in GB/s (measurement helper)."""
+    import torch
+    lib = load_library()
+    with torch.cuda.device(torch.device(device)):
+        buf = torch.empty(mib << 20, dtype=torch.uint8, device=device)
+        out = C.c_double(0.0)
+        st = lib.fem_probe_l2_read(C.c_void_p(buf.data_ptr()), C.c_size_t(buf.numel()), repeats,
+                                   C.c_void_p(torch.cuda.current_stream().cuda_stream), C.byref(out))
+    if st != FEM_OK:
+        raise FemError(st, "fem_probe_l2_read")
+    return float(out.value)
 
 
 def schedule_for(cfg: wl.Config, precise_steps: int = 8) -> Schedule:

@@ -22,12 +22,12 @@ def lib():
 def declared_symbols():
     text = open(os.path.join(ROOT, "include", "fem.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(fem_[a-z_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(fem_[a-z0-9_]+)\s*\(", text)))
 
 
 def test_every_declared_symbol_is_exported(lib):
     names = declared_symbols()
-    assert len(names) >= 19
+    assert len(names) >= 20
     for name in names:
         assert hasattr(lib, name), name
     assert sorted(fem.EXPORTS) == names
