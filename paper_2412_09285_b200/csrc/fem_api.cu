@@ -490,6 +490,7 @@ fem_status fem_reset(fem_handle *h) {
     hd->readout_valid = false;
     hd->wide_live = false;
     hd->tc_ready = false;
+    hd->gather_h = hd->gather_h_want = false;
     return FEM_OK;
 }
 
@@ -513,6 +514,9 @@ fem_status fem_set_option(fem_handle *h, const char *key, int64_t value) {
     } else if (!strcmp(key, "potts_tma")) {
         if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "potts_tma must be 0 or 1");
         hd->opt_potts_tma = value;
+    } else if (!strcmp(key, "gather_fields")) {
+        if (value < -1 || value > 1) return fail(hd, FEM_EINVAL, "gather_fields must be -1, 0 or 1");
+        hd->opt_gather_fields = value;
     } else if (!strcmp(key, "potts_lane")) {
         if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "potts_lane must be 0 or 1");
         hd->opt_potts_lane = value;
@@ -534,6 +538,7 @@ int64_t fem_get_info(const fem_handle *h, const char *key) {
     if (!strcmp(key, "persist_cluster")) return hd->persist_cluster;
     if (!strcmp(key, "tma_launches")) return hd->tma_launches;
     if (!strcmp(key, "lane_launches")) return hd->lane_launches;
+    if (!strcmp(key, "gather_fields")) return hd->gather_h || hd->gather_h_want ? 1 : 0;
     if (!strcmp(key, "t_done")) return hd->t_done;
     if (!strcmp(key, "R")) return hd->R;
     if (!strcmp(key, "replica_block")) return hd->Rb;
@@ -546,7 +551,7 @@ int64_t fem_get_info(const fem_handle *h, const char *key) {
         // (8 B per moment array the optimiser of the last fem_anneal does not keep less: SGD has no second moment,
         // RMSprop / SGD without momentum no first)
         const int64_t fields = (int64_t)hd->dp.n * hd->dp.F * hd->R;
-        return hd->bytes_per_field * fields + hd->structure_bytes;
+        return hd->bytes_per_field * fields + hd->structure_bytes;  // (the same 24 B per field in gather-the-fields mode)
     }
     return -1;
 }
@@ -567,6 +572,7 @@ fem_status fem_set_fields(fem_handle *h, int32_t R, const float *fields) {
     hd->readout_valid = false;
     hd->wide_live = false;
     hd->tc_ready = false;
+    hd->gather_h = hd->gather_h_want = false;  // the injected fields are in hd->h
     return FEM_OK;
 }
 
@@ -584,7 +590,7 @@ static fem_status fetch_state(Handle *hd, const float *src, const double *srcW, 
 fem_status fem_get_fields(fem_handle *h, float *fields) {
     Handle *hd = reinterpret_cast<Handle *>(h);
     if (!hd || !fields) return FEM_EINVAL;
-    return fetch_state(hd, hd->h, hd->hW, fields);
+    return fetch_state(hd, hd->fields(), hd->hW, fields);
 }
 
 fem_status fem_get_moments(fem_handle *h, float *m1, float *m2) {
@@ -597,7 +603,7 @@ fem_status fem_get_moments(fem_handle *h, float *m1, float *m2) {
 }
 
 static void ensure_gather(Handle *hd) {
-    if (hd->gather_valid) return;
+    if (hd->gather_valid || (hd->gather_h && !hd->wide_live)) return;  // (gather_h: the fp32 steps gather from the fields themselves)
     StepScalars sc{};
     sc.t = hd->t_done;
     if (hd->dp.kind == FEM_BMINCUT) launch_potts(hd, sc, hd->wide_live, /*step=*/false, 0, hd->R / hd->Rb);
@@ -609,10 +615,11 @@ fem_status fem_get_marginals(fem_handle *h, float *marginals) {
     Handle *hd = reinterpret_cast<Handle *>(h);
     if (!hd || !marginals) return FEM_EINVAL;
     if (hd->R < 1) return fail(hd, FEM_ESTATE, "no fields yet");
-    // the fp32 g[cur ^ 1] is scratch here: the next step (or the narrowing) overwrites it anyway
-    if (hd->dp.kind == FEM_BMINCUT) launch_potts_softmax(hd, hd->g[hd->cur ^ 1]);
-    else launch_sigmoid(hd, hd->g[hd->cur ^ 1]);
-    return fetch_state(hd, hd->g[hd->cur ^ 1], nullptr, marginals);
+    // the fp32 scratch array (g[cur ^ 1]) is free here: the next step (or the narrowing) overwrites it anyway
+    float *scratch = hd->scratch();
+    if (hd->dp.kind == FEM_BMINCUT) launch_potts_softmax(hd, scratch);
+    else launch_sigmoid(hd, scratch);
+    return fetch_state(hd, scratch, nullptr, marginals);
 }
 
 fem_status fem_anneal(fem_handle *h, const fem_schedule *sch, int32_t R, uint64_t seed, int32_t stop_after) {
@@ -657,12 +664,23 @@ fem_status fem_anneal(fem_handle *h, const fem_schedule *sch, int32_t R, uint64_
         }
         hd->gather_valid = false;
         hd->tc_ready = false;
+        hd->gather_h = hd->gather_h_want = false;
     }
     const int nb = hd->R / hd->Rb;
     // one-hot neighbours only where the paper manipulates the gradient (graph kinds with a CSR)
     const bool disc = sch->manipulated && hd->rowsum != nullptr;
     if (hd->gather_valid && hd->gather_disc != disc) hd->gather_valid = false;
     hd->gather_disc = disc;
+    if (hd->t_done == 0) {
+        // gather-the-fields mode (fixed for the trajectory): sparse two-state graph kinds, exact gradient, regular degree 3
+        // or 4 (three or four extra tanh per field), the stepwise fp32 kernel.  Automatic choice: only when the state is
+        // streamed from HBM (one replica block, too large for L2), where the 4 B per field of the gather array count.
+        const bool shape_ok = (hd->dp.kind == FEM_MAXCUT || (hd->dp.kind == FEM_ISING && !hd->dp.J)) && !disc &&
+                              (hd->dp.uniform_deg == 3 || hd->dp.uniform_deg == 4) && hd->Rb % 4 == 0 && !persist_eligible(hd);
+        const bool streamed = nb == 1 && 20.0 * (double)hd->dp.n * hd->R > 0.45 * (double)hd->l2_bytes;
+        hd->gather_h_want = shape_ok && (hd->opt_gather_fields == 1 || (hd->opt_gather_fields < 0 && streamed));
+        hd->gather_h = false;
+    }
     hd->plain_adam = sch->optimizer == FEM_ADAM && !sch->manipulated;
     hd->bytes_per_field = 8 + (sch->optimizer == FEM_ADAM || sch->momentum > 0 ? 8 : 0) + (sch->optimizer != FEM_SGD ? 8 : 0);
     auto scalars = [&](int t) {
@@ -715,6 +733,17 @@ fem_status fem_anneal(fem_handle *h, const fem_schedule *sch, int32_t R, uint64_
         launch_narrow(hd, false);
         hd->wide_live = false;
         hd->tc_ready = false;
+    }
+    if (hd->gather_h_want && !hd->gather_h && !hd->wide_live && t < stop_after) {
+        // The first fp32 step of a trajectory takes the default path: its gather array is the accurately rounded one
+        // (narrowed from the fp64 wide phase, or made from the fields with the double-precision tanh), and the early
+        // dynamics amplifies that rounding.  From its output on, the gather array is exactly
+        // mag_of(h) in fp32 -- what the gather-the-fields steps recompute -- so the mode switches without changing a bit.
+        one_step(t, 0, nb);
+        hd->cur ^= 1;
+        ++t;
+        hd->gather_h = true;
+        hd->hpar = hd->cur;  // the fields are in hd->h
     }
     if (persist && t < stop_after) {  // small sparse two-state problem: one CTA per replica, all steps in one launch
         if (!cuda_ok(hd, persist_run(hd, false, t, stop_after, scalars_thunk, &scalars), "persistent launch")) return FEM_ECUDA;

@@ -101,6 +101,17 @@ struct Handle {
     double *e_real = nullptr;
     int *part = nullptr;
     int *best = nullptr;  // [0] = best replica, [1..n] = its configuration
+    // "gather the fields" mode of the sparse two-state step (k_step_q2.cu): neighbours are gathered
+    // from the fp32 FIELD array and m_j = tanh(h_j / 2) is recomputed per neighbour, so no separate gather array is
+    // written (4 B per field per step less).  The step is synchronous, so the fields ping-pong between the arrays
+    // h and g[0]: the current ones are in fields() = (cur ^ hpar) & 1 ? g[0] : h; g[1] is the hooks' scratch.
+    bool gather_h = false;       // active: the fp32 fields ping-pong, steps gather from them
+    bool gather_h_want = false;  // decided at the first step of a trajectory; becomes active after the first fp32 step
+    int hpar = 0;
+    int64_t opt_gather_fields = -1;  // -1 = automatic (degree <= 4, state streamed from HBM), 0 = never, 1 = wherever it applies
+    float *fields() const { return gather_h && ((cur ^ hpar) & 1) ? g[0] : h; }
+    float *fields_other() const { return gather_h && ((cur ^ hpar) & 1) ? h : g[0]; }
+    float *scratch() const { return gather_h ? g[1] : g[cur ^ 1]; }  // free fp32 array of state size (hooks)
     int cur = 0;          // g[cur] holds the gathered quantity of the current fields
     int t_done = 0;
     int traj_optimizer = 0, traj_manipulated = 0;  // fixed at the first step of a trajectory
@@ -153,7 +164,7 @@ namespace fem {
 // typed views of the live state arrays
 template <typename T> struct StateOf;
 template <> struct StateOf<float> {
-    static float *h(Handle *d) { return d->h; }
+    static float *h(Handle *d) { return d->fields(); }
     static float *m1(Handle *d) { return d->m1; }
     static float *m2(Handle *d) { return d->m2; }
     static float *g(Handle *d, int k) { return d->g[k]; }

@@ -185,7 +185,7 @@ void launch_sigmoid(Handle *hd, float *out) {
     if (hd->wide_live)
         sigmoid_kernel<double><<<grid, kThreads, 0, hd->stream>>>(hd->hW, out, per, nb, hd->rows * hd->Rb);
     else
-        sigmoid_kernel<float><<<grid, kThreads, 0, hd->stream>>>(hd->h, out, per, nb, hd->rows * hd->Rb);
+        sigmoid_kernel<float><<<grid, kThreads, 0, hd->stream>>>(hd->fields(), out, per, nb, hd->rows * hd->Rb);
     hd->launches++;
 }
 

@@ -338,7 +338,7 @@ void launch_readout(Handle *hd, double lambda) {
         round_kernel<double><<<rgrid, kThreads, 0, hd->stream>>>(hd->hW, hd->cfg, dp.n, dp.F, hd->R, hd->Rb,
                                                                  hd->rows * hd->Rb);
     else
-        round_kernel<float><<<rgrid, kThreads, 0, hd->stream>>>(hd->h, hd->cfg, dp.n, dp.F, hd->R, hd->Rb,
+        round_kernel<float><<<rgrid, kThreads, 0, hd->stream>>>(hd->fields(), hd->cfg, dp.n, dp.F, hd->R, hd->Rb,
                                                                 hd->rows * hd->Rb);
     hd->launches++;
     run_energy(hd, hd->R, hd->Rb, lambda);

@@ -18,6 +18,7 @@ struct Q2Params {
     DevProblem dp;
     Sc<T> sc;
     const T *field;     // dense Ising: precomputed J*m, same layout as h
+    T *h_out;           // gather-the-fields mode (GH): the new fields go to the other field array
     const double *rowsum;  // sum_j |W_ij| per node (manipulated gradients), or nullptr
     const signed char *g8_in;  // manipulated gradients: sgn(m) as bytes (device_math.cuh), same offsets as g_in
     signed char *g8_out;
@@ -28,8 +29,12 @@ struct Q2Params {
 
 enum { MODE_MAXCUT = 0, MODE_ISING = 1, MODE_SAT = 3, MODE_FIELD = 4 };
 
-template <typename T, int VEC, int MODE, int DEG>
-__global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) {
+// GH ("gather the fields", fp32 MaxCut / sparse Ising, regular degree 3 or 4): neighbours are gathered from the FIELD
+// array (p.a.g_in == p.a.h) and m_j = tanh(h_j / 2) is recomputed per neighbour with the very function the owner
+// would have used, so the results are bit-identical while no gather array is written: 24 B of HBM traffic per field
+// and step instead of 28, for DEG more exp / rcp per field (cfg 4a is DRAM-bound: profiles/r02_cfg4a_step.md).
+template <typename T, int VEC, int MODE, int DEG, bool GH = false>
+__global__ void __launch_bounds__(kThreads, GH ? 8 : 1) step_q2_kernel(const Q2Params<T> p) {
     using R = Row<T, VEC>;
     pdl_trigger();
     const unsigned idx = blockIdx.x * kThreads + threadIdx.x;
@@ -58,7 +63,12 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
             for (int v = 0; v < VEC; ++v) r.v[v] = (T)b[v];
             return r;
         }
-        return R::ld(row_of(j));
+        R r = R::ld(row_of(j));
+        if (GH) {
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) r.v[v] = mag_of(r.v[v]);
+        }
+        return r;
     };
 
     // static structure first (legal before pdl_wait), then everything the previous step wrote
@@ -74,7 +84,8 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
     pdl_wait();
     const Sc<T> &sc = p.sc;
     const bool use_m1 = sc.uses_m1(), use_m2 = sc.uses_m2();  // uniform: SGD keeps no second moment (8 B per field less)
-    const R h4 = R::ld_stream(p.a.h + off);
+    // (GH: the own row is one of the rows the neighbours gather -- keep it in L2 like them)
+    const R h4 = GH ? R::ld(p.a.h + off) : R::ld_stream(p.a.h + off);
     R m1 = {}, m2 = {};
     if (use_m1) m1 = R::ld_stream(p.a.m1 + off);
     if (use_m2) m2 = R::ld_stream(p.a.m2 + off);
@@ -185,9 +196,11 @@ __global__ void __launch_bounds__(kThreads) step_q2_kernel(const Q2Params<T> p) 
         hn.v[v] = opt_update(h, g, m1.v[v], m2.v[v], sc);
         gn.v[v] = disc ? sign_of(hn.v[v]) : mag_of(hn.v[v]);
     }
-    hn.st_stream(p.a.h + off);
+    if (GH) hn.st(p.h_out + off);
+    else hn.st_stream(p.a.h + off);
     if (use_m1) m1.st_stream(p.a.m1 + off);
     if (use_m2) m2.st_stream(p.a.m2 + off);
+    if (GH) return;
     if (disc) {
         int b[VEC];
 #pragma unroll
@@ -406,6 +419,13 @@ static void launch_q2_deg(Handle *hd, const Q2Params<T> &p, dim3 grid) {
         }
     } else {
         const int d = (MODE == MODE_MAXCUT || MODE == MODE_ISING) ? hd->dp.uniform_deg : 0;
+        if constexpr (std::is_same<T, float>::value && VEC == 4 && (MODE == MODE_MAXCUT || MODE == MODE_ISING)) {
+            if (hd->gather_h && p.h_out) {
+                if (d == 3) launch_pdl(step_q2_kernel<T, VEC, MODE, 3, true>, grid, dim3(kThreads), hd->stream, p);
+                else launch_pdl(step_q2_kernel<T, VEC, MODE, 4, true>, grid, dim3(kThreads), hd->stream, p);
+                return;
+            }
+        }
         if (d == 3)
             launch_pdl(step_q2_kernel<T, VEC, MODE, 3>, grid, dim3(kThreads), hd->stream, p);
         else if (d == 4)
@@ -453,6 +473,11 @@ static void launch_step_q2_t(Handle *hd, const StepScalars &sc, int blk_begin, i
     p.dp = hd->dp;
     p.sc = Sc<T>(sc);
     p.field = nullptr;
+    p.h_out = nullptr;
+    if (std::is_same<T, float>::value && hd->gather_h) {  // fields ping-pong between h and g[0]; gathers read the input fields
+        p.a.g_in = reinterpret_cast<const T *>(hd->fields()) + base;
+        p.h_out = reinterpret_cast<T *>(hd->fields_other()) + base;
+    }
     p.rowsum = hd->rowsum;
     p.g8_in = reinterpret_cast<const signed char *>(hd->g[hd->cur]) + base;   // byte offsets = element offsets
     p.g8_out = reinterpret_cast<signed char *>(hd->g[hd->cur ^ 1]) + base;
