@@ -66,6 +66,8 @@ typedef struct {
     int32_t m;
     const int64_t *clause_ptr;
     const int32_t *lits;
+    /* BMINCUT only, optional: node weights V_i > 0 of the balance term (S33-S35); NULL = all 1 */
+    const double *node_weight;
 } femo_problem;
 
 typedef struct {
@@ -136,6 +138,7 @@ double femo_entropy(const femo_problem *pb, const double *h) {
 }
 
 static double wgt(const femo_problem *pb, int64_t e) { return pb->weight ? pb->weight[e] : 1.0; }
+static double nodew(const femo_problem *pb, int i) { return pb->node_weight ? pb->node_weight[i] : 1.0; }
 
 /* ------------------------------------------------------------------------------------------
  * Mean-field internal energy U_MF(P), one replica (reading R1: every edge once).
@@ -144,6 +147,9 @@ static double wgt(const femo_problem *pb, int64_t e) { return pb->weight ? pb->w
  *   bMinCut (S11; balance() PAPER.md:536):
  *           U = sum_E W_ij sum_s P_i(s)[1 - P_j(s)] + lambda sum_s [(sum_i P_i(s))^2 - sum_i P_i(s)^2]
  *               + lambda (n - n^2/q)                                  (constant of reading R2)
+ *           with node weights V_i (S33): P_i(s) -> V_i P_i(s) in both sums of the balance term, and
+ *           the constant becomes lambda (sum_i V_i^2 - (sum_i V_i)^2 / q), so that one-hot marginals still give
+ *           exactly cut + lambda sum_k (sum_{i in k} V_i - sum_i V_i / q)^2
  *   MaxSAT  (S16):  U = sum_m prod_{i in dm} [1 - P_i(W_mi)]
  * ---------------------------------------------------------------------------------------- */
 double femo_internal_energy(const femo_problem *pb, const double *h, double lambda) {
@@ -186,12 +192,18 @@ double femo_internal_energy(const femo_problem *pb, const double *h, double lamb
         for (int s = 0; s < q; ++s) {
             double col = 0.0, sq = 0.0;
             for (int i = 0; i < n; ++i) {
-                col += P[(size_t)i * q + s];
-                sq += P[(size_t)i * q + s] * P[(size_t)i * q + s];
+                double vp = nodew(pb, i) * P[(size_t)i * q + s];
+                col += vp;
+                sq += vp * vp;
             }
             U += lambda * (col * col - sq);
         }
-        U += lambda * ((double)n - (double)n * (double)n / (double)q);
+        double v1 = 0.0, v2 = 0.0;
+        for (int i = 0; i < n; ++i) {
+            v1 += nodew(pb, i);
+            v2 += nodew(pb, i) * nodew(pb, i);
+        }
+        U += lambda * (v2 - v1 * v1 / (double)q);
     } else { /* MAXSAT */
         for (int c = 0; c < pb->m; ++c) {
             double prod = 1.0;
@@ -218,6 +230,7 @@ double femo_free_energy(const femo_problem *pb, const double *h, double beta, do
  *
  * Potts kind: g^p_i(s) from S26 in the edge-once reading,
  *     g^p_i(s) = -sum_j W_ij P_j(s) + 2 lambda [S_s - P_i(s)] + (1/beta)[ln P_i(s) + 1],
+ *   with node weights (S34): 2 lambda V_i [sum_j V_j P_j(s) - V_i P_i(s)] for the balance part,
  * then the chain rule S20:
  *     g^h_i(s) = P_i(s) [ g^p_i(s) - sum_s' P_i(s') g^p_i(s') ].
  * Two-state kinds: S29 with c_i = 1 and P_j in place of e_j,
@@ -236,16 +249,17 @@ void femo_grad_h(const femo_problem *pb, const double *h, double beta, double la
         double *gp = (double *)malloc(sizeof(double) * (size_t)q);
         femo_marginals(pb, h, P);
         for (int i = 0; i < n; ++i)
-            for (int s = 0; s < q; ++s) col[s] += P[(size_t)i * q + s];
+            for (int s = 0; s < q; ++s) col[s] += nodew(pb, i) * P[(size_t)i * q + s];
         for (int i = 0; i < n; ++i) {
             const double *hi = h + (size_t)i * q;
             const double *Pi = P + (size_t)i * q;
             double lse = logsumexp(hi, q);
+            double Vi = nodew(pb, i);
             for (int s = 0; s < q; ++s) {
                 double f = 0.0;
                 for (int64_t e = pb->row_ptr[i]; e < pb->row_ptr[i + 1]; ++e)
                     f += wgt(pb, e) * P[(size_t)pb->col_idx[e] * q + s];
-                gp[s] = -f + 2.0 * lambda * (col[s] - Pi[s]) + (hi[s] - lse + 1.0) / beta;
+                gp[s] = -f + 2.0 * lambda * Vi * (col[s] - Vi * Pi[s]) + (hi[s] - lse + 1.0) / beta;
             }
             double gbar = 0.0;
             for (int s = 0; s < q; ++s) gbar += Pi[s] * gp[s];
@@ -325,6 +339,7 @@ void femo_adam(const femo_adam_cfg *cfg, int32_t t, int64_t count, double *h, do
  * Potts kind, S27 taken literally (coefficient lambda, not 2 lambda, on the balance term):
  *     ghat^p_i(s) = -c^f_i sum_j W_ij e_j(s) + lambda c^a_i [ sum_j e_j(s) - e_i(s) ] + (1/beta)[ln P_i(s) + 1]
  *     c^f_i = q / sum_j W_ij,  c^a_i = q / sqrt(sum_j W_ij)
+ *   with node weights (S35): lambda c^a_i V_i [ sum_j V_j e_j(s) - V_i e_i(s) ] for the balance part,
  *   then S20:  g^h_i(s) = gamma P_i(s) [ ghat^p_i(s) - sum_s' P_i(s') ghat^p_i(s') ].
  *   e_j = one-hot of argmax_s h_j(s), ties -> lowest state (the rounding rule R3).
  * Max-SAT: the paper makes no modification: exact gradient times gamma.
@@ -350,7 +365,7 @@ void femo_grad_h_manipulated(const femo_problem *pb, const double *h, double bet
             for (int s = 1; s < q; ++s)
                 if (h[(size_t)i * q + s] > h[(size_t)i * q + best]) best = s;
             hot[i] = best;
-            cnt[best] += 1.0;
+            cnt[best] += nodew(pb, i);
         }
         for (int i = 0; i < n; ++i) {
             const double *hi = h + (size_t)i * q;
@@ -365,7 +380,8 @@ void femo_grad_h_manipulated(const femo_problem *pb, const double *h, double bet
                 for (int64_t e = pb->row_ptr[i]; e < pb->row_ptr[i + 1]; ++e)
                     if (hot[pb->col_idx[e]] == s) f += wgt(pb, e);
                 double ei = (hot[i] == s) ? 1.0 : 0.0;
-                gp[s] = -cf * f + lambda * ca * (cnt[s] - ei) + (hi[s] - lse + 1.0) / beta;
+                double Vi = nodew(pb, i);
+                gp[s] = -cf * f + lambda * ca * Vi * (cnt[s] - Vi * ei) + (hi[s] - lse + 1.0) / beta;
             }
             double gbar = 0.0;
             for (int s = 0; s < q; ++s) gbar += Pi[s] * gp[s];
@@ -566,6 +582,7 @@ void femo_round(const femo_problem *pb, int32_t R, const double *h, int32_t *cfg
  *   MaxCut : cut = sum_{(i,j) in E, s_i != s_j} W_ij ; E = -cut            (Eq.6)
  *   bMinCut: cut as above; n_k = #{i : s_i = k};
  *            energy = cut + lambda * sum_k (n_k - n/q)^2  (k ascending)     (Eq.7, R2)
+ *            with node weights (integral, S33 PAPER.md:892): n_k = sum_{i : s_i = k} V_i and n = sum_i V_i
  *   MaxSAT : unsat = #{m : every literal of m is false}                     (Eq.8)
  *   Ising  : E = -sum_{i<j} W_ij s_i s_j, s = 2 cfg - 1, row-major order
  * e_int is the integer energy (weights rounded to nearest; meaningful when they are integral),
@@ -592,10 +609,14 @@ void femo_energy(const femo_problem *pb, const int32_t *cfg, double lambda, int6
         } else {
             int q = pb->q;
             int32_t *cnt = (int32_t *)calloc((size_t)q, sizeof(int32_t));
-            for (int i = 0; i < n; ++i) cnt[cfg[i]] += 1;
+            int64_t total = 0;
+            for (int i = 0; i < n; ++i) {
+                cnt[cfg[i]] += (int32_t)llround(nodew(pb, i));
+                total += llround(nodew(pb, i));
+            }
             double pen = 0.0;
             for (int k = 0; k < q; ++k) {
-                double d = (double)cnt[k] - (double)n / (double)q;
+                double d = (double)cnt[k] - (double)total / (double)q;
                 pen = pen + d * d;
             }
             ei = cut_i;

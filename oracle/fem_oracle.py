@@ -41,6 +41,7 @@ class _Problem(C.Structure):
         ("row_ptr", C.c_void_p), ("col_idx", C.c_void_p), ("weight", C.c_void_p),
         ("dense_J", C.c_void_p),
         ("m", C.c_int32), ("clause_ptr", C.c_void_p), ("lits", C.c_void_p),
+        ("node_weight", C.c_void_p),
     ]
 
 
@@ -89,6 +90,7 @@ class Problem:
     m: int = 0
     clause_ptr: Optional[np.ndarray] = None  # int64 [m+1]
     lits: Optional[np.ndarray] = None        # int32, signed 1-based
+    node_weight: Optional[np.ndarray] = None  # float64 [n], BMINCUT balance weights V_i (S33-S35) or None (= all 1)
     _keep: list = field(default_factory=list, repr=False)
 
     def __post_init__(self):
@@ -100,6 +102,7 @@ class Problem:
         self.dense_J = cast(self.dense_J, np.float64)
         self.clause_ptr = cast(self.clause_ptr, np.int64)
         self.lits = cast(self.lits, np.int32)
+        self.node_weight = cast(self.node_weight, np.float64)
 
     @property
     def fields_per_var(self) -> int:
@@ -107,7 +110,7 @@ class Problem:
 
     def c(self) -> _Problem:
         return _Problem(self.kind, self.n, self.q, _p(self.row_ptr), _p(self.col_idx), _p(self.weight),
-                        _p(self.dense_J), self.m, _p(self.clause_ptr), _p(self.lits))
+                        _p(self.dense_J), self.m, _p(self.clause_ptr), _p(self.lits), _p(self.node_weight))
 
 
 @dataclass

@@ -33,6 +33,7 @@ class Instance:
     lam: float = 0.0                         # bMinCut balance weight
     name: str = ""
     meta: dict = field(default_factory=dict)
+    node_weight: Optional[np.ndarray] = None  # float32 [n], bMinCut balance weights V_i (integral, > 0) or None (= all 1)
 
     @property
     def fields_per_var(self) -> int:

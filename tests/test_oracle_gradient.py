@@ -15,7 +15,8 @@ from paper_2412_09285_b200 import workloads as wl
 
 def as_problem(inst: wl.Instance) -> fo.Problem:
     return fo.Problem(kind=inst.kind, n=inst.n, q=inst.q, row_ptr=inst.row_ptr, col_idx=inst.col_idx,
-                      weight=inst.weight, dense_J=inst.dense_J, m=inst.m, clause_ptr=inst.clause_ptr, lits=inst.lits)
+                      weight=inst.weight, dense_J=inst.dense_J, m=inst.m, clause_ptr=inst.clause_ptr, lits=inst.lits,
+                      node_weight=inst.node_weight)
 
 
 def small_graph(n, p, seed, pm1=True, real=False):
@@ -48,6 +49,9 @@ def cases():
     b2 = small_graph(7, 0.7, 16, real=True)
     b2.weight = np.abs(b2.weight)
     out.append(("bmincut_q5_w", wl.Instance(wl.BMINCUT, b2.n, 5, b2.row_ptr, b2.col_idx, b2.weight), 0.11))
+    vb = wl.Instance(wl.BMINCUT, b2.n, 4, b2.row_ptr, b2.col_idx, b2.weight,
+                     node_weight=np.array([3, 1, 7, 2, 1, 5, 4], dtype=np.float32))   # node-weighted balance term (S33-S34)
+    out.append(("bmincut_q4_node_weights", vb, 0.23))
     out.append(("maxsat_k3", wl.random_ksat(9, 30, 3, 17), 0.0))
     out.append(("maxsat_k4", wl.random_ksat(10, 40, 4, 18), 0.0))
     return out
