@@ -267,7 +267,7 @@ def run_workload(args, name, steps, warmup, ctx, with_e2e=True):
     readout_ms = sum(e[1].elapsed_time(e[4]) for e in bulk_events) / max(len(bulk_events), 1)
     # algorithmic bytes of one launch: the whole step's bytes spread over the launches that make up a step
     step_bytes = eng.info("step_bytes") * (N - K) * steps / max(bulk_launches, 1)
-    info = {k: eng.info(k) for k in ("tc_launches", "persist_launches", "tma_launches", "lane_launches", "replica_block", "nnz")}
+    info = {k: eng.info(k) for k in ("tc_launches", "persist_launches", "tma_launches", "lane_launches", "si_launches", "replica_block", "nnz")}
     eng.close()
 
     # ---- e2e through the public API from host buffers (pinned), host<->device copies inside the timed region
@@ -359,7 +359,9 @@ def run_workload(args, name, steps, warmup, ctx, with_e2e=True):
                             "rows gathered more than once by an SM can be served by its L1, so `achieved` (algorithmic gather bytes) is an upper bound on the L2 traffic"}
     else:
         achieved = step_bytes / (kernel_us * 1e-6) / 1e9
-        kname = (("potts_lane_kernel (a lane owns a replica; fused softmax + gather + balance + chain rule + optimiser)"
+        kname = (("potts_si_kernel (state-innermost replica blocks: a lane owns the q states of a (variable, replica) cell; fused "
+                  "softmax + gather + balance + chain rule + optimiser)" if info["si_launches"] > 0 else
+                  "potts_lane_kernel (a lane owns a replica; fused softmax + gather + balance + chain rule + optimiser)"
                   if info["lane_launches"] > 0 else
                   "potts_tma_kernel (rows staged by cp.async.bulk one variable ahead; fused softmax + gather + balance + "
                   "chain rule + optimiser)" if info["tma_launches"] > 0 else
@@ -371,6 +373,23 @@ def run_workload(args, name, steps, warmup, ctx, with_e2e=True):
                     "traffic": load_traffic(name), "peak_source": peak_src,
                     "algorithmic_bytes_per_launch": step_bytes, "kernel_us": kernel_us,
                     "kernel_share_of_step": share}
+        if inst.kind == wl.BMINCUT:
+            # what binds the Potts step: every neighbour row comes out of L2 (4 B per field and neighbour),
+            # so the SM <-> L2 traffic per field is 12 B own rows + 4 deg B gathers + 16 B stores, and the streamed arrays pass
+            # through L2 a second time on their way from / to DRAM.  The gather rate of this device out of a working set of
+            # the block's footprint (five fp32 arrays of the block) is measured live beside the 32 MiB figure.
+            deg_mean = float(info["nnz"]) / n
+            l2_side = (12.0 + 4.0 * deg_mean + 16.0) * n * inst.q * info["replica_block"]
+            foot_mib = int(min(1024, max(1, round(20.0 * n * inst.q * info["replica_block"] / 2 ** 20))))
+            seg = int(min(512, max(64, 16 * info["replica_block"])))
+            roofline["l2_side_bytes_per_launch"] = l2_side
+            roofline["l2_side_gbs"] = l2_side / (kernel_us * 1e-6) / 1e9
+            roofline["l2_gather_probe_gbs"] = {"32MiB": fem.probe_l2_gather(f"cuda:{local_rank}", 32, seg),
+                                               f"{foot_mib}MiB (block footprint)": fem.probe_l2_gather(f"cuda:{local_rank}", foot_mib, seg),
+                                               "row_bytes": seg}
+            roofline["note"] = ("the step moves (12 + 4 deg + 16) B per field between SMs and L2 against 24 B of compulsory HBM traffic; "
+                                "with a block footprint beyond one die's half of the L2 the measured SM <-> L2 rate, not HBM, is what "
+                                "binds (l2_gather_probe_gbs: pure random-row reads, footprint-sized vs 32 MiB working set)")
         if info["replica_block"] < R and 20.0 * n * inst.fields_per_var * info["replica_block"] < 0.5 * 126e6:
             roofline["note"] = ("replica block L2-resident for the whole anneal: `achieved` is the ALGORITHMIC-byte rate "
                                 "(24 B per field per step / time) served out of L2, not DRAM utilisation; it is compared with "

@@ -178,13 +178,15 @@ fem_status fem_energy_of(fem_handle *h, const int32_t *cfg /* [count][n] */, int
  * GEMM) and "tc_tile_n" (replica columns per tensor-core tile: 0 = default, 32/64/128/256).
  * "persistent" (small sparse MAXCUT / ISING / MAXSAT problems with few enough replicas to run in at most three
  * waves of clusters: 1 = replica-persistent cluster kernel where the problem fits, the default; 0 = one launch per step; 1 + CS = force clusters of CS = 1, 2, 4 or 8 CTAs per replica) and
+ * "potts_si" (BMINCUT, q = 4 or 8, replica blocks of 4 / 8 / 16 / 32 with n a multiple of 32 / block: 1 = fp32 steps on
+ * state-innermost replica blocks, k_step_potts_si.cu, the default; 0 = off),
  * "potts_tma" (BMINCUT: 1 = rows staged by bulk asynchronous copies where the shape allows, the default; 0 =
  * register path) and "potts_lane" (BMINCUT, q <= 8, replica blocks of 8 / 16 / 32: 1 = the lane-per-replica kernel, k_step_potts_lane.cu;
  * 0 = the default).  None of them changes a single bit of the results.  Unknown key: FEM_EINVAL. */
 fem_status fem_set_option(fem_handle *h, const char *key, int64_t value);
 /* Introspection for benchmarks: "launches" (kernels enqueued so far), "tc_launches" (of which tcgen05
  * dense steps), "persist_launches", "persist_cluster" (CTAs per replica of the persistent kernel),
- * "tma_launches" (TMA-staged Potts steps), "lane_launches" (lane-per-replica Potts steps), "t_done", "R", "replica_block", "nnz", "uniform_degree",
+ * "tma_launches" (TMA-staged Potts steps), "lane_launches" (lane-per-replica Potts steps), "si_launches" (state-innermost Potts steps), "t_done", "R", "replica_block", "nnz", "uniform_degree",
  * "integral_weights", "step_bytes" (algorithmic HBM bytes of one fused step of the last schedule's optimiser,
  * DESIGN.md section 6).  Unknown key: -1. */
 int64_t fem_get_info(const fem_handle *h, const char *key);
@@ -194,6 +196,14 @@ int64_t fem_get_info(const fem_handle *h, const char *key);
  * times from all SMs with 16-byte loads that bypass L1, timed with CUDA events on `cuda_stream`; synchronous.  bench.py
  * compares the L2-resident Max-SAT step (cfg 3) with this roof.  FEM_EINVAL on bad arguments, FEM_ECUDA without a device. */
 fem_status fem_probe_l2_read(void *buffer, size_t bytes, int32_t repeats, void *cuda_stream, double *gigabytes_per_second);
+
+/* Measurement helper (not on the hot path): rate in GB/s at which all SMs gather pseudo-random rows of `row_bytes` (64, 128,
+ * 256 or 512) out of a DEVICE buffer of `bytes` (1 MiB .. 1 GiB, a multiple of 512; overwritten with zeros), 8 independent
+ * rows in flight per warp, `repeats` iterations per warp -- the access pattern of the neighbour gathers (a2).  With the
+ * buffer size as the parameter it shows where the two-die L2 stops serving a working set at full rate (DESIGN.md section 6:
+ * bench.py reports it at 32 MiB and at the footprint of cfg 2's replica block).  Synchronous; FEM_EINVAL / FEM_ECUDA as above. */
+fem_status fem_probe_l2_gather(void *buffer, size_t bytes, int32_t row_bytes, int32_t repeats, void *cuda_stream,
+                               double *gigabytes_per_second);
 
 const char *fem_last_error(const fem_handle *h); /* h may be NULL: last create-time error */
 void fem_destroy(fem_handle *h);

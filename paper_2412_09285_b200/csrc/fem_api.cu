@@ -16,6 +16,8 @@ void launch_prepare_q2(Handle *hd, bool wide);
 void launch_potts(Handle *hd, const StepScalars &sc, bool wide, bool step, int blk_begin, int blk_count);
 void launch_sigmoid(Handle *hd, float *out);
 bool potts_block_ok(int q, int Rb);
+bool potts_si_applicable(const Handle *hd);                  // k_step_potts_si.cu
+void launch_potts_si_relayout(Handle *hd, bool to_si);
 void launch_potts_softmax(Handle *hd, float *out);
 void launch_tc_split(Handle *hd);
 bool persist_eligible(const Handle *hd);
@@ -199,14 +201,17 @@ static void configure_R(Handle *hd, int R) {
         // a block must fit the team mapping of the Potts kernel (one variable's lanes inside a warp); among the
         // divisors of R that do, take the requested one, else the largest that is L2-resident, else the smallest
         const int q = hd->dp.q;
-        // gathers_fit: the two gather buffers (8 B per field) of the block fit in L2 even though the streamed
-        // arrays do not -- neighbour rows are then served from L2 while h, m1, m2 stream through (evict-first)
+        // gathers_fit: the two gather buffers (8 B per field) of the block fit in 45% of L2 even though the streamed
+        // arrays do not -- neighbour rows are then served from L2 while h, m1, m2 stream through (evict-first).  The L2
+        // of this part is two halves of 63 MB, one per die: measured (profiles/r02_cfg2_step.md),
+        // blocks whose gather buffers take more than about one half lose their gather hits (cfg 2: Rb = 16 moves 530 MB
+        // of DRAM traffic per launch for 307 MB algorithmic, Rb = 8 moves 204 MB for 154 MB)
         int largest = 1, resident = 0, gathers_fit = 0, smallest_vec = 0;
         for (int d = 1; d <= R; ++d) {
             if (R % d || !potts_block_ok(q, d)) continue;
             largest = d;
             if (per_replica * d <= budget && d % 4 == 0 && (double)hd->dp.n * hd->dp.F * d >= 1.0e6) resident = d;
-            if (8.0 * (double)hd->dp.n * hd->dp.F * d <= 0.85 * (double)hd->l2_bytes) gathers_fit = d;
+            if (8.0 * (double)hd->dp.n * hd->dp.F * d <= 0.45 * (double)hd->l2_bytes) gathers_fit = d;
             if (!smallest_vec && d % 2 == 0) smallest_vec = d;
         }
         if (hd->opt_replica_block > 0 && hd->opt_replica_block <= R && R % hd->opt_replica_block == 0 &&
@@ -520,6 +525,9 @@ fem_status fem_set_option(fem_handle *h, const char *key, int64_t value) {
     } else if (!strcmp(key, "potts_lane")) {
         if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "potts_lane must be 0 or 1");
         hd->opt_potts_lane = value;
+    } else if (!strcmp(key, "potts_si")) {
+        if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "potts_si must be 0 or 1");
+        hd->opt_potts_si = value;
     } else if (!strcmp(key, "tensor_cores")) {
         if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "tensor_cores must be 0 or 1");
         hd->opt_tensor_cores = value;
@@ -538,6 +546,7 @@ int64_t fem_get_info(const fem_handle *h, const char *key) {
     if (!strcmp(key, "persist_cluster")) return hd->persist_cluster;
     if (!strcmp(key, "tma_launches")) return hd->tma_launches;
     if (!strcmp(key, "lane_launches")) return hd->lane_launches;
+    if (!strcmp(key, "si_launches")) return hd->si_launches;
     if (!strcmp(key, "gather_fields")) return hd->gather_h || hd->gather_h_want ? 1 : 0;
     if (!strcmp(key, "t_done")) return hd->t_done;
     if (!strcmp(key, "R")) return hd->R;
@@ -745,6 +754,13 @@ fem_status fem_anneal(fem_handle *h, const fem_schedule *sch, int32_t R, uint64_
         hd->gather_h = true;
         hd->hpar = hd->cur;  // the fields are in hd->h
     }
+    // Potts, q = 4 / 8: the fp32 steps of this call run on state-innermost replica blocks (k_step_potts_si.cu); the
+    // arrays are permuted in place here and back below, so nothing outside this call sees the other layout
+    const bool si = hd->dp.kind == FEM_BMINCUT && !hd->wide_live && t < stop_after && potts_si_applicable(hd);
+    if (si) {
+        launch_potts_si_relayout(hd, true);
+        hd->si_live = true;
+    }
     if (persist && t < stop_after) {  // small sparse two-state problem: one CTA per replica, all steps in one launch
         if (!cuda_ok(hd, persist_run(hd, false, t, stop_after, scalars_thunk, &scalars), "persistent launch")) return FEM_ECUDA;
         t = stop_after;
@@ -768,6 +784,10 @@ fem_status fem_anneal(fem_handle *h, const fem_schedule *sch, int32_t R, uint64_
             }
             hd->cur = cur0 ^ ((tb - ta) & 1);
         }
+    }
+    if (si) {
+        launch_potts_si_relayout(hd, false);
+        hd->si_live = false;
     }
     if (stop_after > t0) {
         hd->lambda_last = sch->lambda ? sch->lambda[stop_after - 1] : hd->pb.lambda;

@@ -130,6 +130,11 @@ struct Handle {
     int64_t opt_potts_lane = 0;   // Potts step with a lane per replica (k_step_potts_lane.cu): measured slower than the
                                   // TMA-staged team kernel on cfg 2, so off unless asked for
     int64_t lane_launches = 0;
+    // Potts step on state-innermost replica blocks (k_step_potts_si.cu): q = 4 / 8, blocks of 4 / 8 / 16 / 32.  The fp32
+    // arrays are re-laid out in place for the fp32 steps of one fem_anneal call (si_live) and back before it returns.
+    int64_t opt_potts_si = 1;
+    int64_t si_launches = 0;
+    bool si_live = false;
     int64_t persist_ell[4] = {-1, -1, -1, -1};  // sliced-ELL entries per CTA for cluster sizes 1, 2, 4, 8
     int sm_count = 148;
     int64_t launches = 0;

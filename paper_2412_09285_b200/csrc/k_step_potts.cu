@@ -332,6 +332,7 @@ static void launch_potts_v(Handle *hd, const PottsParams<T> &p, dim3 grid, bool 
 
 bool launch_potts_tma(Handle *hd, const StepScalars &sc, int blk_begin, int blk_count);  // k_step_potts_tma.cu
 bool launch_potts_lane(Handle *hd, const StepScalars &sc, int blk_begin, int blk_count);  // k_step_potts_lane.cu
+bool launch_potts_si(Handle *hd, const StepScalars &sc, int blk_begin, int blk_count);    // k_step_potts_si.cu
 
 int potts_qpad(int q) {
     int qp = 2;
@@ -394,6 +395,10 @@ void launch_potts(Handle *hd, const StepScalars &sc, bool wide, bool step, int b
     if (!step) {
         const size_t bytes = (size_t)hd->dp.q * hd->Rb * blk_count * sizeof(long long);
         cudaMemsetAsync(hd->colsum[sc.t % 3] + (int64_t)blk_begin * hd->dp.q * hd->Rb, 0, bytes, hd->stream);
+    }
+    if (hd->si_live) {  // the fp32 arrays are in the state-innermost layout: only this kernel reads it (fem_anneal)
+        (void)launch_potts_si(hd, sc, blk_begin, blk_count);  // a failed launch surfaces through cudaGetLastError
+        return;
     }
     if (!wide && step && launch_potts_lane(hd, sc, blk_begin, blk_count)) return;  // lane-per-replica fast path (q <= 8)
     if (!wide && step && launch_potts_tma(hd, sc, blk_begin, blk_count)) return;  // TMA-staged fast path where it applies

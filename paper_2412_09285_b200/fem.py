@@ -25,7 +25,7 @@ EXPORTS = [
     "fem_abi_version", "fem_workspace_bytes", "fem_create", "fem_anneal", "fem_reset", "fem_readout", "fem_result",
     "fem_set_fields", "fem_get_fields", "fem_get_moments", "fem_get_marginals", "fem_get_configs", "fem_energy_of",
     "fem_set_option", "fem_get_info", "fem_last_error", "fem_destroy",
-    "fem_schedule_inverse_proportional", "fem_schedule_exponential", "fem_probe_l2_read",
+    "fem_schedule_inverse_proportional", "fem_schedule_exponential", "fem_probe_l2_read", "fem_probe_l2_gather",
 ]
 
 
@@ -92,6 +92,7 @@ def load_library():
     lib.fem_schedule_inverse_proportional.argtypes = [C.c_double, C.c_double, C.c_int32, C.c_void_p]
     lib.fem_schedule_exponential.argtypes = [C.c_double, C.c_double, C.c_int32, C.c_void_p]
     lib.fem_probe_l2_read.argtypes = [C.c_void_p, C.c_size_t, C.c_int32, C.c_void_p, C.POINTER(C.c_double)]
+    lib.fem_probe_l2_gather.argtypes = [C.c_void_p, C.c_size_t, C.c_int32, C.c_int32, C.c_void_p, C.POINTER(C.c_double)]
     _lib = lib
     return lib
 
@@ -291,6 +292,20 @@ def probe_l2_read(device: str = "cuda:0", mib: int = 32, repeats: int = 200) -> 
                                    C.c_void_p(torch.cuda.current_stream().cuda_stream), C.byref(out))
     if st != FEM_OK:
         raise FemError(st, "fem_probe_l2_read")
+    return float(out.value)
+
+
+def probe_l2_gather(device: str = "cuda:0", mib: int = 32, row_bytes: int = 128, repeats: int = 300) -> float:
+    """fem_probe_l2_gather on a torch-owned buffer: the rate in GB/s of random-row gathers out of a `mib` MiB working set."""
+    import torch
+    lib = load_library()
+    with torch.cuda.device(torch.device(device)):
+        buf = torch.empty(mib << 20, dtype=torch.uint8, device=device)
+        out = C.c_double(0.0)
+        st = lib.fem_probe_l2_gather(C.c_void_p(buf.data_ptr()), C.c_size_t(buf.numel()), int(row_bytes), int(repeats),
+                                     C.c_void_p(torch.cuda.current_stream().cuda_stream), C.byref(out))
+    if st != FEM_OK:
+        raise FemError(st, "fem_probe_l2_gather")
     return float(out.value)
 
 

@@ -375,6 +375,7 @@ def test_potts_tma_bit_identical_to_team_kernel(fem, case, manipulated):
     for tma in (1, 0):
         eng = fem.Fem(inst, R)
         eng.set_option("potts_lane", 0)              # (the lane-per-replica kernel would take the q <= 8 exact cases)
+        eng.set_option("potts_si", 0)                # (and the state-innermost kernel the q = 4 / 8 ones)
         eng.set_option("potts_tma", tma)
         if rb:
             eng.set_option("replica_block", rb)
@@ -427,6 +428,7 @@ def test_potts_lane_bit_identical_to_team_kernel(fem, case, opt):
     for lane in (1, 0):
         eng = fem.Fem(inst, R)
         eng.set_option("potts_lane", lane)
+        eng.set_option("potts_si", 0)
         eng.set_option("potts_tma", 0)
         if rb:
             eng.set_option("replica_block", rb)
@@ -483,3 +485,65 @@ def test_gather_fields_mode_is_bit_identical(fem, name, opt):
         assert np.array_equal(a[4][0], b[4][0]) and np.array_equal(a[4][1], b[4][1]), key
         assert np.array_equal(a[5]["energy"], b[5]["energy"]) and a[5]["best_replica"] == b[5]["best_replica"], key
         assert np.array_equal(a[6], b[6]), key
+
+
+SI_CASES = {
+    # name: (q, degree (0 = Erdos-Renyi CSR with rows of 0..16 entries), n, R, replica_block, weighted)
+    "q8_reg10_R16_rb8": (8, 10, 1200, 16, 8, False),           # cfg 2's shape: 4 variables per 32-cell group
+    "q8_reg10_R32_rb16": (8, 10, 1200, 32, 16, False),         # 2 variables per group, two blocks
+    "q8_reg10_R8_rb4": (8, 10, 1200, 8, 4, False),             # 8 variables per group
+    "q8_reg3_R16_auto": (8, 3, 1200, 16, 0, False),
+    "q4_reg6_weighted_R32": (4, 6, 1201, 32, 32, True),        # one variable per group, odd n
+    "q4_reg4_R16_rb8": (4, 4, 1204, 16, 8, False),
+    "q8_reg7_weighted_R16_rb16": (8, 7, 1202, 16, 16, True),   # a regular degree without an unrolled instantiation
+    "q8_er_csr_R16_rb8": (8, 0, 1204, 16, 8, False),           # rows of different lengths, isolated nodes
+    "q4_er_csr_weighted_R32_rb16": (4, 0, 1204, 32, 16, True),
+    "q8_reg10_R16_rb8_n1201": (8, 10, 1201, 16, 8, False),     # n not a multiple of 32 / Rb: the kernel does not apply
+}
+
+
+@pytest.mark.parametrize("opt", ["adam", "sgd_mom", "rmsprop"])
+@pytest.mark.parametrize("case", list(SI_CASES))
+def test_potts_si_bit_identical_to_team_kernel(fem, case, opt):
+    """The Potts step on state-innermost replica blocks (k_step_potts_si.cu: arrays re-laid out in place for the fp32
+    steps of a fem_anneal call, a lane owns the q states of one (variable, replica) cell) against the register path:
+    same arithmetic in the same order, so fields, moments, energies and part sizes must be bit-identical -- also across
+    a resume point (two relayouts in, two out); the counter proves which kernel ran."""
+    q, d, n, R, rb, weighted = SI_CASES[case]
+    if d == 0:
+        er = wl.erdos_renyi_maxcut(n, 0.0045, 2040 + q, pm1=False)
+        assert 0 < np.diff(er.row_ptr).max() and np.diff(er.row_ptr).min() == 0
+        inst = wl.Instance(wl.BMINCUT, er.n, q, er.row_ptr, er.col_idx, None, lam=0.03)
+    else:
+        inst = wl.random_regular(n if (n * d) % 2 == 0 else n + 1, d, 2020 + q, wl.BMINCUT, q, lam=0.03)
+    if weighted:
+        w = np.random.default_rng(3).integers(1, 5, inst.nnz // 2).astype(np.float32)[edge_ids(inst)]
+        inst = wl.Instance(wl.BMINCUT, inst.n, q, inst.row_ptr, inst.col_idx, w, lam=0.03)
+    extra = {"adam": {}, "sgd_mom": dict(optimizer=2, lr=0.3, momentum=0.7, dampening=0.2),
+             "rmsprop": dict(optimizer=1, lr=0.03, alpha=0.9)}[opt]
+    sch = fem.Schedule(beta=fem.linear_temperature_schedule(1.0, 0.05, 40), precise_steps=4, **extra)
+    out = {}
+    for si in (1, 0):
+        eng = fem.Fem(inst, R)
+        eng.set_option("potts_si", si)
+        eng.set_option("potts_lane", 0)
+        eng.set_option("potts_tma", 0)
+        if rb:
+            eng.set_option("replica_block", rb)
+        eng.anneal(sch, R, seed=8, stop_after=17)
+        mid = eng.get_fields()                        # a hook between the two calls sees the standard layout
+        eng.anneal(sch, R, seed=8, stop_after=40)
+        out[si] = (eng.get_fields(), eng.get_moments(), eng.result(), mid, eng.get_marginals())
+        Rb = eng.info("replica_block")
+        blocks = R // Rb
+        applies = Rb in (4, 8, 16, 32) and inst.n % (32 // Rb) == 0
+        assert eng.info("si_launches") == (36 * blocks if si and applies else 0), case   # 40 steps - 4 wide, per block
+        if rb:
+            assert Rb == rb
+        eng.close()
+    assert np.array_equal(out[1][0], out[0][0])
+    assert np.array_equal(out[1][3], out[0][3])
+    assert np.array_equal(out[1][4], out[0][4])
+    assert np.array_equal(out[1][1][0], out[0][1][0]) and np.array_equal(out[1][1][1], out[0][1][1])
+    assert np.array_equal(out[1][2]["energy"], out[0][2]["energy"])
+    assert np.array_equal(out[1][2]["part_sizes"], out[0][2]["part_sizes"])
