@@ -415,7 +415,7 @@ def run_workload(args, name, steps, warmup, ctx, with_e2e=True):
     return entry, cfg, inst
 
 
-PER_CONFIG = ["cfg0", "cfg1", "cfg2", "cfg3", "cfg4a", "cfg4b"]
+PER_CONFIG = ["cfg0", "cfg1", "cfg2", "cfg3", "cfg4a", "cfg4b", "skew"]   # skew: not a BASELINE.json config (degree-skewed rows)
 
 
 def main():

@@ -178,6 +178,8 @@ fem_status fem_energy_of(fem_handle *h, const int32_t *cfg /* [count][n] */, int
  * GEMM) and "tc_tile_n" (replica columns per tensor-core tile: 0 = default, 32/64/128/256).
  * "persistent" (small sparse MAXCUT / ISING / MAXSAT problems with few enough replicas to run in at most three
  * waves of clusters: 1 = replica-persistent cluster kernel where the problem fits, the default; 0 = one launch per step; 1 + CS = force clusters of CS = 1, 2, 4 or 8 CTAs per replica) and
+ * "long_rows" (two-state graph kinds: 1 = rows with many entries are summed by a CTA each in a fixed order, the default;
+ * 0 = one thread per row as for short rows -- this one does change the summation order of those rows),
  * "potts_si" (BMINCUT, q = 4 or 8, replica blocks of 4 / 8 / 16 / 32 with n a multiple of 32 / block: 1 = fp32 steps on
  * state-innermost replica blocks, k_step_potts_si.cu, the default; 0 = off),
  * "potts_tma" (BMINCUT: 1 = rows staged by bulk asynchronous copies where the shape allows, the default; 0 =
@@ -187,7 +189,9 @@ fem_status fem_set_option(fem_handle *h, const char *key, int64_t value);
 /* Introspection for benchmarks: "launches" (kernels enqueued so far), "tc_launches" (of which tcgen05
  * dense steps), "persist_launches", "persist_cluster" (CTAs per replica of the persistent kernel),
  * "tma_launches" (TMA-staged Potts steps), "lane_launches" (lane-per-replica Potts steps), "si_launches" (state-innermost Potts steps), "t_done", "R", "replica_block", "nnz", "uniform_degree",
- * "integral_weights", "step_bytes" (algorithmic HBM bytes of one fused step of the last schedule's optimiser,
+ * "max_degree", "long_rows" (rows of a two-state graph kind with more than 96 entries, or more than 32 and four times the mean degree:
+ * the stepwise kernel gives each
+ * a CTA of its own), "integral_weights", "step_bytes" (algorithmic HBM bytes of one fused step of the last schedule's optimiser,
  * DESIGN.md section 6).  Unknown key: -1. */
 int64_t fem_get_info(const fem_handle *h, const char *key);
 

@@ -27,7 +27,7 @@ cudaError_t persist_run(Handle *hd, bool wide, int t_begin, int t_end, StepScala
 static std::string g_create_error;
 
 struct Layout {
-    size_t row_ptr, col, w, rowsum, J, Jlo, glo0, glo1, field, occ_ptr, occ, clause_ptr, lits;
+    size_t row_ptr, col, w, rowsum, long_rows, J, Jlo, glo0, glo1, field, occ_ptr, occ, clause_ptr, lits;
     size_t h, m1, m2, g0, g1, stage, hW, m1W, m2W, gW0, gW1, colsum0, colsum1, colsum2, cfg, e_part_i, e_part_d, part_part, e_int, e_real, part,
         best, total;
 };
@@ -45,6 +45,7 @@ static int occ_stride(int kmax) {
 struct ProblemShape {
     int64_t nnz = 0, nlits = 0, nocc = 0;
     int kmax = 0;
+    int64_t n_long = 0;  // rows with more than kLongRow entries (two-state graph kinds)
     bool weighted = false, dense = false;
 };
 
@@ -81,6 +82,9 @@ static bool shape_of(const fem_problem *pb, ProblemShape *s, std::string *err) {
     s->nnz = pb->row_ptr[pb->n];
     if (s->nnz < 0 || s->nnz >= (int64_t)1 << 31) return *err = "nnz out of range", false;
     s->weighted = pb->weight != nullptr;
+    if (pb->kind != FEM_BMINCUT)
+        for (int i = 0; i < pb->n; ++i)
+            if (is_long_row(pb->row_ptr[i + 1] - pb->row_ptr[i], s->nnz, pb->n)) ++s->n_long;
     return true;
 }
 
@@ -99,6 +103,7 @@ static Layout make_layout(const fem_problem *pb, const ProblemShape &s, int R_ca
     L.col = take((size_t)s.nnz * 4);
     L.w = take(s.weighted ? (size_t)s.nnz * 4 : 0);
     L.rowsum = take(s.nnz > 0 || pb->row_ptr ? (size_t)pb->n * 8 : 0);
+    L.long_rows = take((size_t)s.n_long * 4);
     L.J = take(s.dense ? (size_t)pb->n * pb->n * 4 : 0);
     L.Jlo = take(s.dense ? (size_t)pb->n * pb->n * 4 : 0);
     L.glo0 = take(s.dense ? state : 0);
@@ -427,6 +432,16 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
         dp.w = s.weighted ? reinterpret_cast<float *>(at(L.w)) : nullptr;
         if (pb->kind == FEM_ISING) hd->integral_weights = false;
         hd->structure_bytes = (dp.uniform_deg > 0 ? 0 : 4 * ((int64_t)pb->n + 1)) + (s.weighted ? 8 : 4) * s.nnz;
+        std::vector<int> h_long;  // long rows get a CTA each in the stepwise kernel (k_step_q2.cu)
+        if (pb->kind != FEM_BMINCUT)
+            for (int i = 0; i < pb->n; ++i)
+                if (is_long_row(pb->row_ptr[i + 1] - pb->row_ptr[i], s.nnz, pb->n)) h_long.push_back(i);
+        if (!h_long.empty()) {
+            up(at(L.long_rows), h_long.data(), h_long.size() * 4, "upload long rows");
+            dp.long_rows = reinterpret_cast<int *>(at(L.long_rows));
+            dp.n_long = (int)h_long.size();
+            if (ok) ok = cuda_ok(hd, cudaStreamSynchronize(hd->stream), "upload long rows");  // h_long is a local
+        }
         if (pb->kind != FEM_BMINCUT) persist_prepare(hd, pb->row_ptr);
         {   // sum_j |W_ij| per node, in double in CSR order (the normalisation factors of the manipulated gradients)
             std::vector<double> rs((size_t)pb->n, 0.0);
@@ -525,6 +540,9 @@ fem_status fem_set_option(fem_handle *h, const char *key, int64_t value) {
     } else if (!strcmp(key, "potts_lane")) {
         if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "potts_lane must be 0 or 1");
         hd->opt_potts_lane = value;
+    } else if (!strcmp(key, "long_rows")) {
+        if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "long_rows must be 0 or 1");
+        hd->opt_long_rows = value;
     } else if (!strcmp(key, "potts_si")) {
         if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "potts_si must be 0 or 1");
         hd->opt_potts_si = value;
@@ -553,6 +571,8 @@ int64_t fem_get_info(const fem_handle *h, const char *key) {
     if (!strcmp(key, "replica_block")) return hd->Rb;
     if (!strcmp(key, "nnz")) return hd->dp.kind == FEM_MAXSAT ? hd->pb.m : hd->dp.nnz;
     if (!strcmp(key, "uniform_degree")) return hd->dp.uniform_deg;
+    if (!strcmp(key, "max_degree")) return hd->dp.max_deg;
+    if (!strcmp(key, "long_rows")) return hd->dp.n_long;
     if (!strcmp(key, "integral_weights")) return hd->integral_weights;
     if (!strcmp(key, "step_bytes")) {
         // algorithmic HBM bytes of one fused step: 24 B per field (read and write h, m1, m2)

@@ -24,6 +24,12 @@ namespace fem {
 constexpr int kThreads = 256;
 constexpr int kMaxQ = 32;
 constexpr int kMaxClauseLen = 8;
+// two-state graph kinds, rows from row_ptr: a "long row" has more than kLongRow entries, or more than kLongRowSkew entries
+// when that is over four times the mean degree (the hubs of a degree-skewed graph) -- the stepwise kernel gives it a
+// whole CTA (k_step_q2.cu) instead of one thread per VEC replicas, and the replica-persistent kernel is not used
+constexpr int kLongRow = 96;
+constexpr int kLongRowSkew = 32;
+__host__ __device__ inline bool is_long_row(int64_t deg, int64_t nnz, int n) { return deg > kLongRow || (deg > kLongRowSkew && deg * n > 4 * nnz); }
 
 // Per-step scalars, computed on the host in double and narrowed in-kernel.
 struct StepScalars {
@@ -47,6 +53,8 @@ struct DevProblem {
     int uniform_deg;     // > 0 when every row has this many entries
     int max_deg;         // longest row
     int64_t nnz;
+    const int *long_rows;  // [n_long] variables whose row has more than kLongRow entries (two-state graph kinds), ascending
+    int n_long;
     const float *J;  // dense Ising, n*n
     // Max-SAT, variable-centric: occurrences of variable i are occ_ptr[i]..occ_ptr[i+1]; occurrence o
     // holds kstride = kmax-1 packed entries (stored with the stride padded to a power of two: 1, 2, 4 or 8 ints): (var << 1 | negated) of the OTHER literals of its clause,
@@ -132,6 +140,7 @@ struct Handle {
     int64_t lane_launches = 0;
     // Potts step on state-innermost replica blocks (k_step_potts_si.cu): q = 4 / 8, blocks of 4 / 8 / 16 / 32.  The fp32
     // arrays are re-laid out in place for the fp32 steps of one fem_anneal call (si_live) and back before it returns.
+    int64_t opt_long_rows = 1;   // 0: long rows stay with one thread per VEC replicas (measurements only)
     int64_t opt_potts_si = 1;
     int64_t si_launches = 0;
     bool si_live = false;

@@ -25,7 +25,13 @@ struct Q2Params {
     unsigned rv;        // Rb / VEC lanes per variable
     int rv_shift;       // log2(rv) when rv is a power of two, else -1
     unsigned total;     // n * rv threads per replica block
+    unsigned main_blocks;  // CTAs that map one thread to (variable, VEC replicas); the CTAs after them take one long row each
+    int long_on;        // rows longer than kLongRow are left to those CTAs (dp.long_rows)
+    unsigned long_chunks;  // CTAs per long row: ceil(rv / kLongLanes)
 };
+
+constexpr int kLongSlices = 32;  // interleaved slices a long row is cut into (fixed: the summation order depends on the row only)
+constexpr int kLongLanes = 32;   // lanes (VEC replicas each) one long-row CTA serves; a wider replica block takes several CTAs per row
 
 enum { MODE_MAXCUT = 0, MODE_ISING = 1, MODE_SAT = 3, MODE_FIELD = 4 };
 
@@ -33,14 +39,34 @@ enum { MODE_MAXCUT = 0, MODE_ISING = 1, MODE_SAT = 3, MODE_FIELD = 4 };
 // array (p.a.g_in == p.a.h) and m_j = tanh(h_j / 2) is recomputed per neighbour with the very function the owner
 // would have used, so the results are bit-identical while no gather array is written: 24 B of HBM traffic per field
 // and step instead of 28, for DEG more exp / rcp per field (cfg 4a is DRAM-bound: profiles/r02_cfg4a_step.md).
-template <typename T, int VEC, int MODE, int DEG, bool GH = false>
+template <typename T, int VEC, int MODE, int DEG, bool GH = false, int KB = 4>
 __global__ void __launch_bounds__(kThreads, GH ? 8 : 1) step_q2_kernel(const Q2Params<T> p) {
     using R = Row<T, VEC>;
     pdl_trigger();
+    // Degree-skewed rows (north_star subsystem 2; the paper's scale-free MaxCut instances, and the reason c_i
+    // exists).  One thread walking a hub's row alone is the tail of the whole launch, so a row with more
+    // than kLongRow entries gets a CTA of its own: the row is cut into kLongSlices interleaved slices (slice s = entries
+    // e0 + s, e0 + s + kLongSlices, ... in ascending order), a thread sums one slice for its VEC replicas, the partial
+    // sums meet in shared memory and are added in ascending s -- a FIXED order that depends on the row only, so results
+    // are deterministic and independent of the replica blocking -- and the first rv threads finish the update like any
+    // other thread.  The hub's own row of the gather array is read by all its neighbours and stays in L1 / L2.
+    constexpr bool LONG = (MODE == MODE_MAXCUT || MODE == MODE_ISING) && DEG == 0 && !GH;
+    bool long_cta = false;
+    if constexpr (LONG) long_cta = blockIdx.x >= p.main_blocks;
     const unsigned idx = blockIdx.x * kThreads + threadIdx.x;
-    if (idx >= p.total) return;
-    const unsigned i = p.rv_shift >= 0 ? idx >> p.rv_shift : idx / p.rv;
-    const unsigned c = (idx - i * p.rv) * VEC;
+    if (!long_cta && idx >= p.total) return;
+    unsigned i = p.rv_shift >= 0 ? idx >> p.rv_shift : idx / p.rv;
+    unsigned c = (idx - i * p.rv) * VEC;
+    unsigned lane0 = 0, lanes = 1;  // long-row CTA: the lanes of the replica block it serves
+    if constexpr (LONG) {
+        if (long_cta) {
+            const unsigned L = blockIdx.x - p.main_blocks;
+            i = (unsigned)__ldg(p.dp.long_rows + L / p.long_chunks);
+            lane0 = (L % p.long_chunks) * kLongLanes;
+            lanes = min((unsigned)kLongLanes, p.rv - lane0);
+            c = (lane0 + threadIdx.x % lanes) * VEC;  // (the first `lanes` threads finish the row; the others only sum slices)
+        }
+    }
     const int64_t blk = (int64_t)blockIdx.y * p.a.blk_stride;
     const unsigned Rb = p.a.Rb;
     const int64_t off = blk + (i * Rb + c);  // a replica block holds < 2^32 elements (checked at fem_anneal)
@@ -107,13 +133,86 @@ __global__ void __launch_bounds__(kThreads, GH ? 8 : 1) step_q2_kernel(const Q2P
                 for (int v = 0; v < VEC; ++v) dU[v] = fma((T)wj[k], nb[k].v[v], dU[v]);
         } else {
             const int e0 = __ldg(p.dp.row_ptr + i), e1 = __ldg(p.dp.row_ptr + i + 1);
-#pragma unroll 4
-            for (int e = e0; e < e1; ++e) {
-                const int j = __ldg(col + e);
-                const float wj = w ? __ldg(w + e) : 1.0f;
-                const R nb = gather((unsigned)j);
+            if constexpr (LONG) {
+                if (!long_cta && p.long_on && is_long_row(e1 - e0, p.dp.nnz, p.dp.n)) return;  // a CTA of its own does this row
+            }
+            if (LONG && long_cta) {
+                if constexpr (LONG) {
+                    __shared__ T red[kLongSlices * kLongLanes * VEC];
+                    const unsigned units = kLongSlices * lanes;  // (slice, lane) pairs; at most 4 per thread
+                    for (unsigned u = threadIdx.x; u < units; u += kThreads) {
+                        const unsigned sl = u / lanes, cl = u - sl * lanes;
+                        const T *__restrict__ gsl = p.a.g_in + blk + (lane0 + cl) * VEC;
+                        const signed char *__restrict__ gsl8 = p.g8_in + blk + (lane0 + cl) * VEC;
+                        T part[VEC];
 #pragma unroll
-                for (int v = 0; v < VEC; ++v) dU[v] = fma((T)wj, nb.v[v], dU[v]);
+                        for (int v = 0; v < VEC; ++v) part[v] = (T)0;
+                        // batches of 4 entries of the slice, all loads of a batch in flight (entries past the end: the
+                        // slice's first entry again with weight 0), added in ascending order
+                        for (int e = e0 + (int)sl; e < e1; e += 4 * kLongSlices) {
+                            unsigned jb[4];
+                            float wb[4];
+                            R nb[4];
+#pragma unroll
+                            for (int k = 0; k < 4; ++k) {
+                                const bool on = e + k * kLongSlices < e1;
+                                const int ee = on ? e + k * kLongSlices : e;
+                                jb[k] = (unsigned)__ldg(col + ee);
+                                wb[k] = on ? (w ? __ldg(w + ee) : 1.0f) : 0.0f;
+                            }
+#pragma unroll
+                            for (int k = 0; k < 4; ++k) {
+                                if (disc) {
+                                    int b[VEC];
+                                    ld_bytes<VEC>(gsl8 + jb[k] * Rb, b);
+#pragma unroll
+                                    for (int v = 0; v < VEC; ++v) nb[k].v[v] = (T)b[v];
+                                } else {
+                                    nb[k] = R::ld(reinterpret_cast<const T *>(reinterpret_cast<const char *>(gsl) + (unsigned long long)jb[k] * row_bytes));
+                                }
+                            }
+#pragma unroll
+                            for (int k = 0; k < 4; ++k)
+#pragma unroll
+                                for (int v = 0; v < VEC; ++v) part[v] = fma((T)wb[k], nb[k].v[v], part[v]);
+                        }
+#pragma unroll
+                        for (int v = 0; v < VEC; ++v) red[u * VEC + v] = part[v];
+                    }
+                    __syncthreads();
+                    if (threadIdx.x >= lanes) return;
+                    for (unsigned s2 = 0; s2 < kLongSlices; ++s2)
+#pragma unroll
+                        for (int v = 0; v < VEC; ++v) dU[v] += red[(s2 * lanes + threadIdx.x) * VEC + v];
+                }
+            } else {
+                // batches of kB entries: the column indices of a batch, then its neighbour rows, all in flight at once (a
+                // remainder loop would pay two dependent round trips per entry).  No branches inside a batch: entries past
+                // the end of the row re-read the row's last entry with weight 0 (fma(0, m, dU) = dU); added in CSR order
+                auto batched = [&](auto tag) {
+                    constexpr int kB = decltype(tag)::value;
+                    for (int e = e0; e < e1; e += kB) {
+                        unsigned jb[kB];
+                        float wb[kB];
+                        R nb[kB];
+#pragma unroll
+                        for (int k = 0; k < kB; ++k) {
+                            const int ee = min(e + k, e1 - 1);
+                            jb[k] = (unsigned)__ldg(col + ee);
+                            wb[k] = e + k < e1 ? (w ? __ldg(w + ee) : 1.0f) : 0.0f;
+                        }
+#pragma unroll
+                        for (int k = 0; k < kB; ++k) nb[k] = gather(jb[k]);
+#pragma unroll
+                        for (int k = 0; k < kB; ++k)
+#pragma unroll
+                            for (int v = 0; v < VEC; ++v) dU[v] = fma((T)wb[k], nb[k].v[v], dU[v]);
+                    }
+                };
+                // batch size KB by the mean degree (chosen at launch): 4 where most rows are short (measured on the scale-free
+                // workload: 19.3 us per launch against 21.6 with a remainder loop and 25+ with batches of 8), 8 for denser
+                // graphs (cfg 0 stepwise: 7.5 us against 9.4 with batches of 4)
+                batched(std::integral_constant<int, KB>{});
             }
         }
         if (MODE == MODE_ISING) {
@@ -430,6 +529,8 @@ static void launch_q2_deg(Handle *hd, const Q2Params<T> &p, dim3 grid) {
             launch_pdl(step_q2_kernel<T, VEC, MODE, 3>, grid, dim3(kThreads), hd->stream, p);
         else if (d == 4)
             launch_pdl(step_q2_kernel<T, VEC, MODE, 4>, grid, dim3(kThreads), hd->stream, p);
+        else if (std::is_same<T, float>::value && (MODE == MODE_MAXCUT || MODE == MODE_ISING) && hd->dp.nnz > 8 * (int64_t)hd->dp.n)
+            launch_pdl(step_q2_kernel<T, VEC, MODE, 0, false, 8>, grid, dim3(kThreads), hd->stream, p);
         else
             launch_pdl(step_q2_kernel<T, VEC, MODE, 0>, grid, dim3(kThreads), hd->stream, p);
     }
@@ -497,7 +598,11 @@ static void launch_step_q2_t(Handle *hd, const StepScalars &sc, int blk_begin, i
     p.rv = (unsigned)(Rb / VEC);
     p.rv_shift = (p.rv & (p.rv - 1)) == 0 ? __builtin_ctz(p.rv) : -1;
     p.total = (unsigned)hd->dp.n * p.rv;
-    dim3 grid((unsigned)ceil_div(p.total, kThreads), (unsigned)blk_count);
+    p.main_blocks = (unsigned)ceil_div(p.total, kThreads);
+    // long rows (CSR kinds without a uniform degree): one extra CTA each, when a row's lanes fit a CTA
+    p.long_on = (mode == MODE_MAXCUT || mode == MODE_ISING) && hd->opt_long_rows && hd->dp.n_long > 0 && hd->dp.uniform_deg == 0;
+    p.long_chunks = (unsigned)ceil_div(p.rv, kLongLanes);
+    dim3 grid(p.main_blocks + (p.long_on ? (unsigned)hd->dp.n_long * p.long_chunks : 0u), (unsigned)blk_count);
     if (VEC == 4) launch_q2_mode<T, 4>(hd, p, grid, mode);
     else launch_q2_mode<T, 1>(hd, p, grid, mode);
     hd->launches++;

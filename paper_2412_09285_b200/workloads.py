@@ -100,6 +100,41 @@ def torus_maxcut(L: int = 200, seed: int = 1001, W: Optional[int] = None) -> Ins
     return Instance(MAXCUT, L * W, 2, row_ptr, col, weight, name=f"maxcut_torus_{L}x{W}", meta={"edges": int(a.size)})
 
 
+def preferential_attachment(n: int = 100000, m: int = 3, seed: int = 1007, pm1: bool = True) -> Instance:
+    """Scale-free graph by preferential attachment (the shape of the G-set's scale-free family): nodes
+    0..m form a clique; every later node attaches to m DISTINCT earlier nodes drawn with probability proportional to their
+    degree (one draw = one entry of the list of all edge endpoints so far; repeats redrawn).  Weights +-1 fair coin or +1."""
+    rng = _rng(seed)
+    ends = np.empty(2 * (m * (m + 1) // 2 + (n - m - 1) * m), dtype=np.int64)
+    u_list, v_list = [], []
+    k = 0
+    for a in range(m + 1):
+        for b in range(a + 1, m + 1):
+            u_list.append(a); v_list.append(b)
+            ends[k] = a; ends[k + 1] = b
+            k += 2
+    draws = rng.random((n, 2 * m + 8))  # uniform numbers per node: enough for the redraws in all but freak cases
+    for node in range(m + 1, n):
+        chosen = []
+        t = 0
+        while len(chosen) < m:
+            x = draws[node, t] if t < draws.shape[1] else rng.random()
+            t += 1
+            cand = int(ends[int(x * k)])
+            if cand not in chosen:
+                chosen.append(cand)
+        for cnd in chosen:
+            u_list.append(cnd); v_list.append(node)
+            ends[k] = cnd; ends[k + 1] = node
+            k += 2
+    u = np.asarray(u_list, dtype=np.int64)
+    v = np.asarray(v_list, dtype=np.int64)
+    w = rng.integers(0, 2, size=u.size).astype(np.float32) * 2 - 1 if pm1 else None
+    row_ptr, col, weight = csr_from_edges(n, u, v, w)
+    return Instance(MAXCUT, n, 2, row_ptr, col, weight, name=f"maxcut_scalefree_n{n}_m{m}",
+                    meta={"edges": int(u.size), "max_degree": int(np.diff(row_ptr).max())})
+
+
 def _random_regular_edges(n: int, d: int, rng: np.random.Generator):
     """Pairing model with repair: shuffle the d*n stubs, pair consecutive stubs, then re-pair the stubs
     of bad pairs (self loops, repeated edges) together with as many random good pairs until none is left."""
@@ -208,5 +243,9 @@ CONFIGS = {
     # 50-800 replicas, 50-500 steps; mean 0.074 s per instance on the paper's GPU), for the replica-persistent Max-SAT kernel
     "sat2016": Config("sat2016 Max-4-SAT n=300 m=2600 R=128 N=500 (MaxSAT-2016-sized stand-in)",
                       lambda: random_ksat(300, 2600, 4, 1006), 128, 500),
+    # not a BASELINE.json config: degree-skewed rows (north_star subsystem 2), shaped like the G-set's scale-free graphs
+    # scaled up: preferential attachment, 3 edges per new node, weights +-1
+    "skew": Config("skew MaxCut scale-free (preferential attachment m=3) n=100000 W=+-1 R=64 N=1000",
+                   lambda: preferential_attachment(100000, 3, 1007, pm1=True), 64, 1000),
     "cfg4b": Config("cfg4b SK dense n=4096 J~N(0,1/n) R=1024 N=1000", lambda: sk_dense(4096, 1005), 1024, 1000),
 }

@@ -60,6 +60,9 @@ def cases():
         "empty_graph": (_graph(wl.MAXCUT, 37, []), 5),
         "isolated_nodes": (_graph(wl.MAXCUT, 50, [(0, 1), (1, 2), (7, 9)], weights=[1.0, -2.0, 3.0]), 1),
         "star_degree_1499": (_graph(wl.MAXCUT, 1500, star), 6),
+        # degree-skewed rows (north_star subsystem 2): hubs of a scale-free graph get a CTA each (rows > 96 entries)
+        "scalefree_n3000_R12": (wl.preferential_attachment(3000, 3, 31, pm1=True), 12),
+        "scalefree_ising_n2000_R64": (wl.sparse_ising_from(wl.preferential_attachment(2000, 4, 32, pm1=False), -0.5), 64),
         "ising_two_spins": (_graph(wl.ISING, 2, [(0, 1)], weights=[0.75]), 4),
         "potts_q2_ring": (_graph(wl.BMINCUT, 40, ring, q=2, lam=0.05), 8),
         "potts_q32_ring": (_graph(wl.BMINCUT, 40, ring, q=32, lam=0.02), 3),
@@ -103,6 +106,27 @@ def test_degenerate_inputs_against_the_oracle(fem, name, manipulated):
             assert np.array_equal(res["energy_int"], e_int) and np.array_equal(res["energy"], e_real)
         assert res["best_replica"] == fo.argmin(e_real)
         eng.close()
+
+
+@pytest.mark.parametrize("name", ["star_degree_1499", "scalefree_n3000_R12", "scalefree_ising_n2000_R64"])
+def test_long_rows_take_the_cta_path_and_are_deterministic(fem, name):
+    """Rows with more than 96 entries are summed by a CTA in a fixed order: the counter shows the path is taken (and the
+    replica-persistent kernel, which has no such path, is not), two runs agree bit for bit, and the replica blocking
+    changes nothing (a long row is always cut into the same 16 interleaved slices)."""
+    inst, R = CASES[name]
+    R = 12 if R == 6 else R
+    sch = fem.Schedule(beta=fem.linear_temperature_schedule(1.0, 0.05, 40), precise_steps=4)
+    out = []
+    for rb in (0, 0, 4):
+        eng = fem.Fem(inst, R)
+        if rb:
+            eng.set_option("replica_block", rb)
+        eng.anneal(sch, R, seed=5)
+        assert eng.info("long_rows") > 0 and eng.info("persist_launches") == 0
+        out.append((eng.get_fields(), eng.result()["energy"]))
+        eng.close()
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
+    assert np.array_equal(out[0][0], out[2][0]) and np.array_equal(out[0][1], out[2][1])   # the order depends on the row only
 
 
 def test_zero_steps_reads_out_the_initial_fields(fem):
