@@ -80,6 +80,11 @@ typedef struct {
     const int64_t *clause_ptr; /* [m+1] */
     const int32_t *lits;       /* [clause_ptr[m]] */
     double lambda;             /* BMINCUT balance weight when the schedule gives no per-step lambda */
+    /* ---- ABI version 4 ---- BMINCUT only, optional: node weights V_i of the balance term (S33-S35),
+     * HOST [n], integral values in 1 .. 2^20, or NULL (= all 1).  The energy becomes cut + lambda * sum_k (sum_{i in k} V_i
+     * - sum_i V_i / q)^2, part_sizes the sums of V_i per part, and the balance term of the gradient
+     * 2 lambda V_i [sum_j V_j P_j(s) - V_i P_i(s)].  Must be NULL for the other kinds. */
+    const float *node_weight;
 } fem_problem;
 
 /* Annealing schedule and optimiser.  Step t = 0..steps-1 uses beta[t]

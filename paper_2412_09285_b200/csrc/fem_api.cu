@@ -27,7 +27,7 @@ cudaError_t persist_run(Handle *hd, bool wide, int t_begin, int t_end, StepScala
 static std::string g_create_error;
 
 struct Layout {
-    size_t row_ptr, col, w, rowsum, long_rows, J, Jlo, glo0, glo1, field, occ_ptr, occ, clause_ptr, lits;
+    size_t row_ptr, col, w, rowsum, long_rows, vw, J, Jlo, glo0, glo1, field, occ_ptr, occ, clause_ptr, lits;
     size_t h, m1, m2, g0, g1, stage, hW, m1W, m2W, gW0, gW1, colsum0, colsum1, colsum2, cfg, e_part_i, e_part_d, part_part, e_int, e_real, part,
         best, total;
 };
@@ -58,6 +58,7 @@ static bool shape_of(const fem_problem *pb, ProblemShape *s, std::string *err) {
     } else if (pb->q != 2) {
         return *err = "q must be 2 for MAXCUT / ISING / MAXSAT", false;
     }
+    if (pb->node_weight && pb->kind != FEM_BMINCUT) return *err = "node_weight is for BMINCUT only", false;
     if (pb->kind == FEM_MAXSAT) {
         if (pb->m < 1 || !pb->clause_ptr || !pb->lits) return *err = "MAXSAT needs m >= 1, clause_ptr and lits", false;
         if (pb->clause_ptr[0] != 0) return *err = "clause_ptr[0] must be 0", false;
@@ -82,6 +83,13 @@ static bool shape_of(const fem_problem *pb, ProblemShape *s, std::string *err) {
     s->nnz = pb->row_ptr[pb->n];
     if (s->nnz < 0 || s->nnz >= (int64_t)1 << 31) return *err = "nnz out of range", false;
     s->weighted = pb->weight != nullptr;
+    if (pb->node_weight) {
+        if (pb->kind != FEM_BMINCUT) return *err = "node_weight is for BMINCUT only", false;
+        for (int i = 0; i < pb->n; ++i) {
+            const float v = pb->node_weight[i];
+            if (!(v >= 1.f) || v > 1048576.f || v != std::nearbyint(v)) return *err = "node_weight must be integral, in 1 .. 2^20", false;
+        }
+    }
     if (pb->kind != FEM_BMINCUT)
         for (int i = 0; i < pb->n; ++i)
             if (is_long_row(pb->row_ptr[i + 1] - pb->row_ptr[i], s->nnz, pb->n)) ++s->n_long;
@@ -104,6 +112,7 @@ static Layout make_layout(const fem_problem *pb, const ProblemShape &s, int R_ca
     L.w = take(s.weighted ? (size_t)s.nnz * 4 : 0);
     L.rowsum = take(s.nnz > 0 || pb->row_ptr ? (size_t)pb->n * 8 : 0);
     L.long_rows = take((size_t)s.n_long * 4);
+    L.vw = take(pb->node_weight ? (size_t)pb->n * 4 : 0);
     L.J = take(s.dense ? (size_t)pb->n * pb->n * 4 : 0);
     L.Jlo = take(s.dense ? (size_t)pb->n * pb->n * 4 : 0);
     L.glo0 = take(s.dense ? state : 0);
@@ -251,7 +260,7 @@ using namespace fem;
 
 extern "C" {
 
-int32_t fem_abi_version(void) { return 3; }
+int32_t fem_abi_version(void) { return 4; }
 
 // a5: the two schedules, in double on the host.  beta(0) = beta_min, beta(N-1) = beta_max.
 fem_status fem_schedule_inverse_proportional(double T_max, double T_min, int32_t N, double *beta_out) {
@@ -306,6 +315,7 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
     hd->pb.dense_J = nullptr;
     hd->pb.clause_ptr = nullptr;
     hd->pb.lits = nullptr;
+    hd->pb.node_weight = nullptr;
     hd->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     hd->R_cap = R_cap;
     DevProblem &dp = hd->dp;
@@ -443,6 +453,15 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
             if (ok) ok = cuda_ok(hd, cudaStreamSynchronize(hd->stream), "upload long rows");  // h_long is a local
         }
         if (pb->kind != FEM_BMINCUT) persist_prepare(hd, pb->row_ptr);
+        dp.vtotal = (double)pb->n;
+        if (pb->node_weight) {  // balance-term node weights (S33-S35); pb->node_weight outlives the upload (synchronised below)
+            up(at(L.vw), pb->node_weight, (size_t)pb->n * 4, "upload node weights");
+            dp.vw = reinterpret_cast<float *>(at(L.vw));
+            double tot = 0.0;
+            for (int i = 0; i < pb->n; ++i) tot += (double)pb->node_weight[i];
+            dp.vtotal = tot;
+            hd->structure_bytes += 4 * (int64_t)pb->n;
+        }
         {   // sum_j |W_ij| per node, in double in CSR order (the normalisation factors of the manipulated gradients)
             std::vector<double> rs((size_t)pb->n, 0.0);
             for (int i = 0; i < pb->n; ++i)
@@ -475,9 +494,15 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
     hd->colsum[0] = reinterpret_cast<long long *>(at(L.colsum0));
     hd->colsum[1] = reinterpret_cast<long long *>(at(L.colsum1));
     hd->colsum[2] = reinterpret_cast<long long *>(at(L.colsum2));
-    {   // |sum_i D_i(s)| < n: the largest power of two (up to 2^44) that keeps n * scale below 2^62
+    {   // |sum_i V_i D_i(s)| < sum_i V_i (= n without node weights): the largest power of two (up to 2^44) that keeps
+        // that bound times the scale below 2^62
+        int64_t bound = pb->n;
+        if (pb->node_weight) {
+            bound = 0;
+            for (int i = 0; i < pb->n; ++i) bound += (int64_t)pb->node_weight[i];
+        }
         int bits = 0;
-        while (((int64_t)1 << bits) <= pb->n) ++bits;
+        while (((int64_t)1 << bits) <= bound) ++bits;
         hd->colsum_scale = std::ldexp(1.0, std::min(44, 62 - bits));
     }
     hd->cfg = reinterpret_cast<int8_t *>(at(L.cfg));

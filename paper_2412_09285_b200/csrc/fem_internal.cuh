@@ -53,6 +53,8 @@ struct DevProblem {
     int uniform_deg;     // > 0 when every row has this many entries
     int max_deg;         // longest row
     int64_t nnz;
+    const float *vw;       // BMINCUT: node weights V_i of the balance term (S33-S35), or nullptr (= all 1)
+    double vtotal;         // sum_i V_i (= n without node weights)
     const int *long_rows;  // [n_long] variables whose row has more than kLongRow entries (two-state graph kinds), ascending
     int n_long;
     const float *J;  // dense Ising, n*n

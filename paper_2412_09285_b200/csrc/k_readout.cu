@@ -81,8 +81,9 @@ __global__ void __launch_bounds__(kThreads) energy_graph_kernel(const ReadoutPar
             }
         }
         if (KIND == FEM_BMINCUT) {
+            const int vi = p.dp.vw ? (int)llrintf(__ldg(p.dp.vw + i)) : 1;  // part sizes are sums of node weights (S35)
 #pragma unroll
-            for (int k = 0; k < kMaxQ; ++k) cnt[k] += (ci == k);
+            for (int k = 0; k < kMaxQ; ++k) cnt[k] += (ci == k) ? vi : 0;
         }
     }
     if (ok) {
@@ -167,6 +168,7 @@ void launch_dense_field_f64(Handle *hd, const double *M, double *C, int n, int R
 struct FinalizeParams {
     int kind, n, q, R, nchunks, integral;
     double lambda;
+    double vtotal;  // sum of the node weights (n without them)
     const long long *part_i;
     const double *part_d;
     const int *part_cnt;
@@ -206,7 +208,7 @@ __global__ void __launch_bounds__(kThreads) energy_finalize_kernel(const Finaliz
         er = sd;
     } else {  // BMINCUT: cut + lambda * sum_k (n_k - n/q)^2, k ascending, no FMA contraction
         double pen = 0.0;
-        const double target = __ddiv_rn((double)p.n, (double)p.q);
+        const double target = __ddiv_rn(p.vtotal, (double)p.q);
         for (int k = 0; k < p.q; ++k) {
             int ck = 0;
             for (int c = lane; c < p.nchunks; c += 32) ck += p.part_cnt[((int64_t)c * p.q + k) * p.R + a];
@@ -320,6 +322,7 @@ static void run_energy(Handle *hd, int R, int Rb, double lambda) {
     f.nchunks = p.nchunks;
     f.integral = hd->integral_weights ? 1 : 0;
     f.lambda = lambda;
+    f.vtotal = dp.vw ? dp.vtotal : (double)dp.n;
     f.part_i = hd->e_part_i;
     f.part_d = hd->e_part_d;
     f.part_cnt = hd->part_part;

@@ -104,6 +104,9 @@ __global__ void __launch_bounds__(kThreads, DISC ? 3 : kTeamMinCtas) potts_team_
         const int i = base + tw;
         const bool ok = lane_ok && i < n;
         const int64_t off = blk + (int64_t)(ok ? i : 0) * p.row_len + lo;
+        // node weight V_i of the balance term (S33-S35; integral, 1 without node weights): the term is
+        // 2 lambda V_i [sum_j V_j P_j(s) - V_i P_i(s)], and the column sums are those of V_i D_i(s)
+        const T Vi = (p.dp.vw && ok) ? (T)__ldg(p.dp.vw + i) : (T)1;
         T h[VEC];
         {
             R r;
@@ -228,8 +231,9 @@ __global__ void __launch_bounds__(kThreads, DISC ? 3 : kTeamMinCtas) potts_team_
                 T gp = (T)0;
                 if (ok) {
                     // explicit fma: potts_tma_kernel must round exactly alike
-                    if (DISC) gp = fma(h[v], sc.inv_beta, fma(lam_c, Ss[v] - own[v], -(cf * f[v])));
-                    else gp = fma(h[v], sc.inv_beta, fma(sc.two_lambda, Ss[v] - P[v], -f[v]));
+                    // (V_i = 1: the products below are exact, so nothing changes without node weights)
+                    if (DISC) gp = fma(h[v], sc.inv_beta, fma(lam_c * Vi, Ss[v] - Vi * own[v], -(cf * f[v])));
+                    else gp = fma(h[v], sc.inv_beta, fma(sc.two_lambda * Vi, Ss[v] - Vi * P[v], -f[v]));
                 }
                 T gbar = P[v] * gp;
 #pragma unroll
@@ -267,7 +271,7 @@ __global__ void __launch_bounds__(kThreads, DISC ? 3 : kTeamMinCtas) potts_team_
                 po.v[v] = (win[v] == s ? (T)1 : (T)0) - inv_q;
             }
             // fixed point straight from the compute type: the scale is a power of two, so the product is exact
-            if (ok) colacc[v] += fixed_of(po.v[v], fx_scale_t);
+            if (ok) colacc[v] += (long long)Vi * fixed_of(po.v[v], fx_scale_t);
         }
         if (DISC) {  // the state-0 lane of each replica group stores the VEC winners as bytes
             if (ok && s == 0) st_bytes<VEC>(p.g8_out + blk + (int64_t)i * p.a.Rb + (unsigned)rl * VEC, win);

@@ -398,6 +398,7 @@ __global__ void __launch_bounds__(kLaneMaxWarps * 32, 2) potts_lane_kernel(const
 // ---- host side ----
 bool potts_lane_applicable(const Handle *hd) {
     const int q = hd->dp.q, Rb = hd->Rb, deg = hd->dp.max_deg;
+    if (hd->dp.vw) return false;  // node-weighted balance term: register path / state-innermost kernel only
     if (hd->opt_potts_lane == 0 || hd->gather_disc) return false;
     if (q < 2 || q > 8 || (Rb != 8 && Rb != 16 && Rb != 32)) return false;
     return deg >= 1 && deg <= kLaneMaxDeg && hd->dp.nnz < ((int64_t)1 << 31);

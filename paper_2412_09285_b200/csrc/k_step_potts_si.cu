@@ -38,6 +38,7 @@ struct PottsSiParams {
     const int *col;
     const float *w;       // nullptr = unit weights
     const int *row_ptr;
+    const float *vw;      // node weights V_i of the balance term (S33-S35), or nullptr
     Sc<float> sc;
     const long long *S_in;
     long long *S_out, *S_zero;
@@ -300,11 +301,13 @@ __global__ void __launch_bounds__(kSiWarps * 32, MINB) potts_si_kernel(const __g
 #pragma unroll
             for (int s = 0; s < Q; ++s) P[s] = e[s] * rz;
         }
-        // ---- g^p (S26), g^h = P (g^p - <g^p>_P) (S20), optimiser
+        // ---- g^p (S26; with node weights S33-S35: 2 lambda V_i [sum_j V_j P_j - V_i P_i]), g^h = P (g^p - <g^p>_P) (S20), optimiser
+        const float Vi = p.vw ? __ldg(p.vw + it * G + g) : 1.0f;  // (V_i = 1: the products are exact, nothing changes)
         {
             float gp[Q], t[Q];
+            const float lamV = sc.two_lambda * Vi;
 #pragma unroll
-            for (int s = 0; s < Q; ++s) gp[s] = fma(h[s], sc.inv_beta, fma(sc.two_lambda, Ss[s] - P[s], -f[s]));
+            for (int s = 0; s < Q; ++s) gp[s] = fma(h[s], sc.inv_beta, fma(lamV, Ss[s] - Vi * P[s], -f[s]));
 #pragma unroll
             for (int s = 0; s < Q; ++s) t[s] = __fmul_rn(P[s], gp[s]);  // (never contracted into the adds)
             const float gbar = si_tree_sum<Q>(t);
@@ -325,7 +328,7 @@ __global__ void __launch_bounds__(kSiWarps * 32, MINB) potts_si_kernel(const __g
 #pragma unroll
             for (int s = 0; s < Q; ++s) {
                 po[s] = fma(e[s], rz, -inv_q);
-                colacc[s] += __float2ll_rn(po[s] * fx_scale_t);
+                colacc[s] += (long long)Vi * __float2ll_rn(po[s] * fx_scale_t);
             }
         }
 #pragma unroll
@@ -496,6 +499,7 @@ bool launch_potts_si(Handle *hd, const StepScalars &sc, int blk_begin, int blk_c
     p.col = hd->dp.col;
     p.w = hd->dp.w;
     p.row_ptr = hd->dp.row_ptr;
+    p.vw = hd->dp.vw;
     p.sc = Sc<float>(sc);
     const int64_t so = (int64_t)blk_begin * q * Rb;
     const int t = sc.t;  // column-sum buffers rotate with the step number exactly as in launch_potts_typed

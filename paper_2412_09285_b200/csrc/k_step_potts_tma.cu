@@ -315,6 +315,7 @@ __global__ void __launch_bounds__(kTmaWarps * 32, 4) potts_tma_kernel(const __gr
 // ---- host side ----
 bool potts_tma_applicable(const Handle *hd) {
     const int q = hd->dp.q, Rb = hd->Rb, deg = hd->dp.max_deg;
+    if (hd->dp.vw) return false;  // node-weighted balance term: register path / state-innermost kernel only
     if (hd->opt_potts_tma == 0) return false;
     if (hd->gather_disc && Rb % 16 != 0) return false;  // id rows travel as bulk copies of Rb bytes (q <= 8)
     if (q < 2 || (q & (q - 1)) != 0 || Rb % 4 != 0 || q * (Rb / 4) != 32) return false;  // one variable = one warp of float4 lanes

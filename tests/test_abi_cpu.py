@@ -31,7 +31,7 @@ def test_every_declared_symbol_is_exported(lib):
     for name in names:
         assert hasattr(lib, name), name
     assert sorted(fem.EXPORTS) == names
-    assert lib.fem_abi_version() == 3
+    assert lib.fem_abi_version() == 4
 
 
 def cproblem(inst, keep):
