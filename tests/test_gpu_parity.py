@@ -547,3 +547,32 @@ def test_potts_si_bit_identical_to_team_kernel(fem, case, opt):
     assert np.array_equal(out[1][1][0], out[0][1][0]) and np.array_equal(out[1][1][1], out[0][1][1])
     assert np.array_equal(out[1][2]["energy"], out[0][2]["energy"])
     assert np.array_equal(out[1][2]["part_sizes"], out[0][2]["part_sizes"])
+
+
+def test_two_handles_with_rank_seeds_match_single_runs(fem):
+    """The N > 1 path on one device: two handles, seeded as ranks 0 and 1 (multigpu.replica_seed), advanced in turns on
+    the same stream, give bit for bit what each seed gives alone -- handles share nothing -- and the Eq.5 pick over the
+    two is the better of the two bests, rank 0 on ties (tests/test_multirank_cpu.py covers the exchange itself)."""
+    from paper_2412_09285_b200 import multigpu
+    inst, R = get("maxcut_reg3_pm1")
+    sch = fem.Schedule(beta=fem.linear_temperature_schedule(1.0, 0.01, 120), precise_steps=8)
+    alone = []
+    for r in range(2):
+        eng = fem.Fem(inst, R)
+        eng.anneal(sch, R, seed=multigpu.replica_seed(4, r))
+        alone.append(eng.result())
+        eng.close()
+    engs = [fem.Fem(inst, R) for _ in range(2)]
+    for stop in (30, 31, 90, 120):                       # interleaved on one stream
+        for r, eng in enumerate(engs):
+            eng.anneal(sch, R, seed=multigpu.replica_seed(4, r), stop_after=stop)
+    both = [eng.result() for eng in engs]
+    for r in range(2):
+        assert np.array_equal(both[r]["energy_int"], alone[r]["energy_int"])
+        assert np.array_equal(both[r]["best_config"], alone[r]["best_config"])
+        engs[r].close()
+    assert not np.array_equal(alone[0]["energy_int"], alone[1]["energy_int"])   # different replicas on the two "ranks"
+    bests = [float(x["energy"][x["best_replica"]]) for x in both]
+    e, owner, cfg = multigpu.best_over_ranks(bests[int(np.argmin(bests))], both[int(np.argmin(bests))]["best_config"],
+                                             __import__("torch").device("cpu"))
+    assert e == min(bests) and np.array_equal(cfg, both[int(np.argmin(bests))]["best_config"])
