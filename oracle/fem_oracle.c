@@ -68,13 +68,19 @@ typedef struct {
     const int32_t *lits;
     /* BMINCUT only, optional: node weights V_i > 0 of the balance term (S33-S35); NULL = all 1 */
     const double *node_weight;
+    /* MAXSAT only, optional: non-Boolean SAT ("W_mi has q > 2 states").  lit_state[x] = W_mi in 0..q-1 of the
+     * x-th literal slot, lits[x] = +v (1-based variable); every variable then has q states and q fields (softmax marginals,
+     * PAPER.md:76), and E = sum_m prod_{i in dm} [1 - delta(W_mi, sigma_i)] (Eq.8).  NULL = Boolean SAT. */
+    const int32_t *lit_state;
 } femo_problem;
 
 typedef struct {
     double lr, beta1, beta2, eps, weight_decay;
 } femo_adam_cfg;
 
-int32_t femo_fields_per_var(const femo_problem *pb) { return pb->kind == FEMO_BMINCUT ? pb->q : 1; }
+/* q fields per variable for the Potts kind and for non-Boolean SAT, one (h(+1) - h(-1)) otherwise */
+static int multistate(const femo_problem *pb) { return pb->kind == FEMO_BMINCUT || (pb->kind == FEMO_MAXSAT && pb->lit_state); }
+int32_t femo_fields_per_var(const femo_problem *pb) { return multistate(pb) ? pb->q : 1; }
 
 /* ------------------------------------------------------------------------------------------
  * Marginals from fields.  P_i(s) = exp h_i(s) / sum_s' exp h_i(s');
@@ -98,7 +104,7 @@ static double logsumexp(const double *h, int q) {
 /* one replica: h[n*F] -> P[n*F]; two-state kinds return P_i = P_i(state 1) */
 void femo_marginals(const femo_problem *pb, const double *h, double *P) {
     int n = pb->n;
-    if (pb->kind != FEMO_BMINCUT) {
+    if (!multistate(pb)) {
         for (int i = 0; i < n; ++i) P[i] = sigmoid(h[i]);
         return;
     }
@@ -124,7 +130,7 @@ static double entropy_two_state(double h) {
 double femo_entropy(const femo_problem *pb, const double *h) {
     double S = 0.0;
     int n = pb->n;
-    if (pb->kind != FEMO_BMINCUT) {
+    if (!multistate(pb)) {
         for (int i = 0; i < n; ++i) S += entropy_two_state(h[i]);
         return S;
     }
@@ -204,6 +210,14 @@ double femo_internal_energy(const femo_problem *pb, const double *h, double lamb
             v2 += nodew(pb, i) * nodew(pb, i);
         }
         U += lambda * (v2 - v1 * v1 / (double)q);
+    } else if (pb->lit_state) { /* non-Boolean SAT, S16 with q states: U = sum_m prod_i [1 - P_i(W_mi)] */
+        int q = pb->q;
+        for (int c = 0; c < pb->m; ++c) {
+            double prod = 1.0;
+            for (int64_t x = pb->clause_ptr[c]; x < pb->clause_ptr[c + 1]; ++x)
+                prod *= 1.0 - P[(size_t)(pb->lits[x] - 1) * q + pb->lit_state[x]];
+            U += prod;
+        }
     } else { /* MAXSAT */
         for (int c = 0; c < pb->m; ++c) {
             double prod = 1.0;
@@ -268,6 +282,35 @@ void femo_grad_h(const femo_problem *pb, const double *h, double beta, double la
         free(P);
         free(col);
         free(gp);
+        return;
+    }
+    if (pb->kind == FEMO_MAXSAT && pb->lit_state) {
+        /* non-Boolean SAT: S28 per state, dU/dP_i(s) = -sum_{m ni i, W_mi = s} prod_{k != i} [1 - P_k(W_mk)],
+         * g^p_i(s) = dU/dP_i(s) + (1/beta)[ln P_i(s) + 1], then the chain rule S20 */
+        int q = pb->q;
+        double *P = (double *)malloc(sizeof(double) * (size_t)n * q);
+        double *dP = (double *)calloc((size_t)n * q, sizeof(double));
+        femo_marginals(pb, h, P);
+        for (int c = 0; c < pb->m; ++c) {
+            int64_t a = pb->clause_ptr[c], b = pb->clause_ptr[c + 1];
+            for (int64_t x = a; x < b; ++x) {
+                double loo = 1.0; /* leave-one-out product, by multiplication only */
+                for (int64_t y = a; y < b; ++y)
+                    if (y != x) loo *= 1.0 - P[(size_t)(pb->lits[y] - 1) * q + pb->lit_state[y]];
+                dP[(size_t)(pb->lits[x] - 1) * q + pb->lit_state[x]] -= loo;
+            }
+        }
+        for (int i = 0; i < n; ++i) {
+            const double *hi = h + (size_t)i * q;
+            const double *Pi = P + (size_t)i * q;
+            double lse = logsumexp(hi, q);
+            double gbar = 0.0;
+            for (int s = 0; s < q; ++s) gbar += Pi[s] * (dP[(size_t)i * q + s] + (hi[s] - lse + 1.0) / beta);
+            for (int s = 0; s < q; ++s)
+                g[(size_t)i * q + s] = Pi[s] * (dP[(size_t)i * q + s] + (hi[s] - lse + 1.0) / beta - gbar);
+        }
+        free(P);
+        free(dP);
         return;
     }
     double *dU = (double *)calloc((size_t)n, sizeof(double));
@@ -350,7 +393,7 @@ void femo_grad_h_manipulated(const femo_problem *pb, const double *h, double bet
     int n = pb->n;
     if (pb->kind == FEMO_MAXSAT || (pb->kind == FEMO_ISING && pb->dense_J)) {
         femo_grad_h(pb, h, beta, lambda, g);
-        for (int i = 0; i < n; ++i) g[i] *= gamma;
+        for (int64_t i = 0; i < (int64_t)n * femo_fields_per_var(pb); ++i) g[i] *= gamma;
         return;
     }
     if (pb->kind == FEMO_BMINCUT) {
@@ -624,6 +667,14 @@ void femo_energy(const femo_problem *pb, const int32_t *cfg, double lambda, int6
             if (part) memcpy(part, cnt, sizeof(int32_t) * (size_t)q);
             free(cnt);
         }
+    } else if (pb->kind == FEMO_MAXSAT && pb->lit_state) { /* a clause is satisfied when some variable takes its clause value */
+        for (int c = 0; c < pb->m; ++c) {
+            int sat = 0;
+            for (int64_t x = pb->clause_ptr[c]; x < pb->clause_ptr[c + 1]; ++x)
+                if (cfg[pb->lits[x] - 1] == pb->lit_state[x]) sat = 1;
+            if (!sat) ei += 1;
+        }
+        er = (double)ei;
     } else if (pb->kind == FEMO_MAXSAT) {
         for (int c = 0; c < pb->m; ++c) {
             int sat = 0;

@@ -41,7 +41,7 @@ class _Problem(C.Structure):
         ("row_ptr", C.c_void_p), ("col_idx", C.c_void_p), ("weight", C.c_void_p),
         ("dense_J", C.c_void_p),
         ("m", C.c_int32), ("clause_ptr", C.c_void_p), ("lits", C.c_void_p),
-        ("node_weight", C.c_void_p),
+        ("node_weight", C.c_void_p), ("lit_state", C.c_void_p),
     ]
 
 
@@ -91,6 +91,7 @@ class Problem:
     clause_ptr: Optional[np.ndarray] = None  # int64 [m+1]
     lits: Optional[np.ndarray] = None        # int32, signed 1-based
     node_weight: Optional[np.ndarray] = None  # float64 [n], BMINCUT balance weights V_i (S33-S35) or None (= all 1)
+    lit_state: Optional[np.ndarray] = None    # int32 [len(lits)], non-Boolean SAT: W_mi in 0..q-1 or None
     _keep: list = field(default_factory=list, repr=False)
 
     def __post_init__(self):
@@ -103,14 +104,16 @@ class Problem:
         self.clause_ptr = cast(self.clause_ptr, np.int64)
         self.lits = cast(self.lits, np.int32)
         self.node_weight = cast(self.node_weight, np.float64)
+        self.lit_state = cast(self.lit_state, np.int32)
 
     @property
     def fields_per_var(self) -> int:
-        return self.q if self.kind == BMINCUT else 1
+        return self.q if (self.kind == BMINCUT or (self.kind == MAXSAT and self.lit_state is not None)) else 1
 
     def c(self) -> _Problem:
         return _Problem(self.kind, self.n, self.q, _p(self.row_ptr), _p(self.col_idx), _p(self.weight),
-                        _p(self.dense_J), self.m, _p(self.clause_ptr), _p(self.lits), _p(self.node_weight))
+                        _p(self.dense_J), self.m, _p(self.clause_ptr), _p(self.lits), _p(self.node_weight),
+                        _p(self.lit_state))
 
 
 @dataclass

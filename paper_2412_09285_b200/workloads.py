@@ -34,10 +34,11 @@ class Instance:
     name: str = ""
     meta: dict = field(default_factory=dict)
     node_weight: Optional[np.ndarray] = None  # float32 [n], bMinCut balance weights V_i (integral, > 0) or None (= all 1)
+    lit_state: Optional[np.ndarray] = None    # int32 [len(lits)], non-Boolean SAT: the clause value W_mi in 0..q-1, or None
 
     @property
     def fields_per_var(self) -> int:
-        return self.q if self.kind == BMINCUT else 1
+        return self.q if (self.kind == BMINCUT or (self.kind == MAXSAT and self.lit_state is not None)) else 1
 
     @property
     def nnz(self) -> int:
@@ -193,6 +194,21 @@ def random_ksat(n: int = 20000, m: int = 200000, k: int = 4, seed: int = 1003) -
     clause_ptr = np.arange(m + 1, dtype=np.int64) * k
     return Instance(MAXSAT, n, 2, m=m, clause_ptr=clause_ptr, lits=lits.ravel().copy(),
                     name=f"max{k}sat_n{n}_m{m}", meta={"k": k})
+
+
+def random_qsat(n: int, m: int, k: int, q: int, seed: int, kmin: Optional[int] = None) -> Instance:
+    """Random non-Boolean SAT: m clauses of k (or kmin..k) distinct variables, each with a uniformly drawn
+    clause value W_mi in 0..q-1; a clause is violated when no variable takes its clause value."""
+    rng = _rng(seed)
+    ptr, lits, states = [0], [], []
+    for _ in range(m):
+        kk = k if kmin is None else int(rng.integers(kmin, k + 1))
+        vs = rng.choice(n, size=kk, replace=False)
+        lits += [int(v) + 1 for v in vs]
+        states += [int(x) for x in rng.integers(0, q, size=kk)]
+        ptr.append(len(lits))
+    return Instance(MAXSAT, n, q, m=m, clause_ptr=np.asarray(ptr, np.int64), lits=np.asarray(lits, np.int32),
+                    lit_state=np.asarray(states, np.int32), name=f"qsat_q{q}_k{k}_n{n}_m{m}")
 
 
 def sk_dense(n: int = 4096, seed: int = 1005) -> Instance:

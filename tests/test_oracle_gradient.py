@@ -16,7 +16,7 @@ from paper_2412_09285_b200 import workloads as wl
 def as_problem(inst: wl.Instance) -> fo.Problem:
     return fo.Problem(kind=inst.kind, n=inst.n, q=inst.q, row_ptr=inst.row_ptr, col_idx=inst.col_idx,
                       weight=inst.weight, dense_J=inst.dense_J, m=inst.m, clause_ptr=inst.clause_ptr, lits=inst.lits,
-                      node_weight=inst.node_weight)
+                      node_weight=inst.node_weight, lit_state=getattr(inst, "lit_state", None))
 
 
 def small_graph(n, p, seed, pm1=True, real=False):
