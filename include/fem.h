@@ -85,6 +85,12 @@ typedef struct {
      * - sum_i V_i / q)^2, part_sizes the sums of V_i per part, and the balance term of the gradient
      * 2 lambda V_i [sum_j V_j P_j(s) - V_i P_i(s)].  Must be NULL for the other kinds. */
     const float *node_weight;
+    /* MAXSAT only, optional: non-Boolean SAT ("W_mi has q > 2 states").  HOST [clause_ptr[m]]: lit_state[x] =
+     * W_mi in 0..q-1 of literal slot x, lits[x] = +v (1-based variable, must be > 0), q in 2..8.  Every variable then has q
+     * states and q fields (softmax marginals; logical layouts as for BMINCUT, F = q), the energy is the number of clauses in
+     * which NO variable takes its clause value (Eq.8), and the gradient is S28 per state with the
+     * chain rule S20.  NULL = Boolean SAT (q must be 2). */
+    const int32_t *lit_state;
 } fem_problem;
 
 /* Annealing schedule and optimiser.  Step t = 0..steps-1 uses beta[t]

@@ -19,6 +19,7 @@ bool potts_block_ok(int q, int Rb);
 bool potts_si_applicable(const Handle *hd);                  // k_step_potts_si.cu
 void launch_potts_si_relayout(Handle *hd, bool to_si);
 void launch_potts_softmax(Handle *hd, float *out);
+void launch_qsat(Handle *hd, const StepScalars &sc, bool wide, bool step, int blk_begin, int blk_count);  // k_step_qsat.cu
 void launch_tc_split(Handle *hd);
 bool persist_eligible(const Handle *hd);
 void persist_prepare(Handle *hd, const int64_t *row_ptr);
@@ -27,7 +28,7 @@ cudaError_t persist_run(Handle *hd, bool wide, int t_begin, int t_end, StepScala
 static std::string g_create_error;
 
 struct Layout {
-    size_t row_ptr, col, w, rowsum, long_rows, vw, J, Jlo, glo0, glo1, field, occ_ptr, occ, clause_ptr, lits;
+    size_t row_ptr, col, w, rowsum, long_rows, vw, lit_state, J, Jlo, glo0, glo1, field, occ_ptr, occ, clause_ptr, lits;
     size_t h, m1, m2, g0, g1, stage, hW, m1W, m2W, gW0, gW1, colsum0, colsum1, colsum2, cfg, e_part_i, e_part_d, part_part, e_int, e_real, part,
         best, total;
 };
@@ -55,9 +56,12 @@ static bool shape_of(const fem_problem *pb, ProblemShape *s, std::string *err) {
     if (pb->kind < FEM_MAXCUT || pb->kind > FEM_MAXSAT) return *err = "unknown kind", false;
     if (pb->kind == FEM_BMINCUT) {
         if (pb->q < 2 || pb->q > kMaxQ) return *err = "q must be in 2..32 for BMINCUT", false;
+    } else if (pb->kind == FEM_MAXSAT && pb->lit_state) {
+        if (pb->q < 2 || pb->q > 8) return *err = "q must be in 2..8 for non-Boolean MAXSAT", false;
     } else if (pb->q != 2) {
-        return *err = "q must be 2 for MAXCUT / ISING / MAXSAT", false;
+        return *err = "q must be 2 for MAXCUT / ISING / Boolean MAXSAT", false;
     }
+    if (pb->lit_state && pb->kind != FEM_MAXSAT) return *err = "lit_state is for MAXSAT only", false;
     if (pb->node_weight && pb->kind != FEM_BMINCUT) return *err = "node_weight is for BMINCUT only", false;
     if (pb->kind == FEM_MAXSAT) {
         if (pb->m < 1 || !pb->clause_ptr || !pb->lits) return *err = "MAXSAT needs m >= 1, clause_ptr and lits", false;
@@ -104,7 +108,7 @@ static Layout make_layout(const fem_problem *pb, const ProblemShape &s, int R_ca
         o = align_up(o + bytes);
         return at;
     };
-    const int F = pb->kind == FEM_BMINCUT ? pb->q : 1;
+    const int F = (pb->kind == FEM_BMINCUT || (pb->kind == FEM_MAXSAT && pb->lit_state)) ? pb->q : 1;
     const size_t rows = (size_t)pb->n * F + 1;
     const size_t state = rows * (size_t)R_cap * sizeof(float);
     L.row_ptr = take(((size_t)pb->n + 1) * 4);
@@ -118,7 +122,8 @@ static Layout make_layout(const fem_problem *pb, const ProblemShape &s, int R_ca
     L.glo0 = take(s.dense ? state : 0);
     L.glo1 = take(s.dense ? state : 0);
     L.field = take(s.dense ? 2 * state : 0);  // fp64 in the wide phase
-    L.occ_ptr = take(pb->kind == FEM_MAXSAT ? ((size_t)pb->n + 1) * 4 : 0);
+    L.occ_ptr = take(pb->kind == FEM_MAXSAT ? ((size_t)pb->n * F + 1) * 4 : 0);
+    L.lit_state = take(pb->lit_state ? (size_t)s.nlits * 4 : 0);
     L.occ = take((size_t)s.nocc * occ_stride(s.kmax) * 4);
     L.clause_ptr = take(pb->kind == FEM_MAXSAT ? ((size_t)pb->m + 1) * 4 : 0);
     L.lits = take((size_t)s.nlits * 4);
@@ -316,13 +321,14 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
     hd->pb.clause_ptr = nullptr;
     hd->pb.lits = nullptr;
     hd->pb.node_weight = nullptr;
+    hd->pb.lit_state = nullptr;
     hd->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     hd->R_cap = R_cap;
     DevProblem &dp = hd->dp;
     dp.kind = pb->kind;
     dp.n = pb->n;
     dp.q = pb->q;
-    dp.F = pb->kind == FEM_BMINCUT ? pb->q : 1;
+    dp.F = (pb->kind == FEM_BMINCUT || (pb->kind == FEM_MAXSAT && pb->lit_state)) ? pb->q : 1;
     dp.nnz = s.nnz;
     hd->rows = (int64_t)dp.n * dp.F + 1;
     char *base = static_cast<char *>(workspace);
@@ -350,14 +356,20 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
         dp.m = m;
         dp.kstride = ks;
         const int kst = occ_stride(s.kmax);
-        h_occ_ptr.assign((size_t)n + 1, 0);
+        const int32_t *qs = pb->lit_state;  // non-Boolean SAT: rows are (variable, clause value) pairs
+        const int F = dp.F;
+        h_occ_ptr.assign((size_t)n * F + 1, 0);
         for (int c = 0; c < m; ++c) {
             for (int64_t x = pb->clause_ptr[c]; x < pb->clause_ptr[c + 1]; ++x) {
                 const int lit = pb->lits[x];
                 const int v = (lit > 0 ? lit : -lit) - 1;
-                if (lit == 0 || v >= n) {
+                if (lit == 0 || v >= n || (qs && lit < 0)) {
                     delete hd;
                     return fail(nullptr, FEM_EINVAL, "literal out of range");
+                }
+                if (qs && (qs[x] < 0 || qs[x] >= pb->q)) {
+                    delete hd;
+                    return fail(nullptr, FEM_EINVAL, "lit_state out of range");
                 }
                 for (int64_t y = pb->clause_ptr[c]; y < x; ++y) {
                     const int l2 = pb->lits[y];
@@ -366,25 +378,28 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
                         return fail(nullptr, FEM_EINVAL, "a clause repeats a variable");
                     }
                 }
-                h_occ_ptr[(size_t)v + 1]++;
+                h_occ_ptr[(size_t)(qs ? v * F + qs[x] : v) + 1]++;
             }
         }
-        for (int i = 0; i < n; ++i) h_occ_ptr[(size_t)i + 1] += h_occ_ptr[i];
-        h_occ.assign((size_t)s.nocc * kst, (n << 1) | 1);  // padding: the constant-1 row, read as "p"
+        for (int64_t i = 0; i < (int64_t)n * F; ++i) h_occ_ptr[(size_t)i + 1] += h_occ_ptr[i];
+        // padding: Boolean -- the constant-1 row, read as "p"; non-Boolean -- the row n*q, which holds -1/q so that
+        // its factor (1 - 1/q) - D is 1
+        h_occ.assign((size_t)s.nocc * kst, qs ? n * F : ((n << 1) | 1));
         std::vector<int> fill(h_occ_ptr.begin(), h_occ_ptr.end() - 1);
         for (int c = 0; c < m; ++c) {  // clause order inside each variable's list == the oracle's summation order
             const int64_t a = pb->clause_ptr[c], b = pb->clause_ptr[c + 1];
             for (int64_t x = a; x < b; ++x) {
                 const int lit = pb->lits[x];
                 const int v = (lit > 0 ? lit : -lit) - 1;
-                int *ent = h_occ.data() + (size_t)fill[v]++ * kst;
+                int *ent = h_occ.data() + (size_t)fill[qs ? v * F + qs[x] : v]++ * kst;
                 int k = 0;
                 for (int64_t y = a; y < b; ++y) {
                     if (y == x) continue;
                     const int l2 = pb->lits[y];
-                    ent[k++] = (((l2 > 0 ? l2 : -l2) - 1) << 1) | (l2 < 0 ? 1 : 0);
+                    if (qs) ent[k++] = (l2 - 1) * F + qs[y];
+                    else ent[k++] = (((l2 > 0 ? l2 : -l2) - 1) << 1) | (l2 < 0 ? 1 : 0);
                 }
-                if (lit > 0) ent[0] |= 0x80000000;
+                if (!qs && lit > 0) ent[0] |= 0x80000000;
             }
         }
         h_cptr.resize((size_t)m + 1);
@@ -397,9 +412,13 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
         dp.occ = reinterpret_cast<int *>(at(L.occ));
         dp.clause_ptr = reinterpret_cast<int *>(at(L.clause_ptr));
         dp.lits = reinterpret_cast<int *>(at(L.lits));
+        if (qs) {
+            up(at(L.lit_state), qs, (size_t)s.nlits * 4, "upload lit_state");
+            dp.lit_state = reinterpret_cast<int *>(at(L.lit_state));
+        }
         hd->integral_weights = true;
-        hd->structure_bytes = 4 * ((int64_t)n + 1) + 4 * (int64_t)s.nocc * kst;
-        {   // sliced-ELL sizes of the replica-persistent kernel, from the occurrence counts
+        hd->structure_bytes = 4 * ((int64_t)n * F + 1) + 4 * (int64_t)s.nocc * kst;
+        if (!qs) {   // sliced-ELL sizes of the replica-persistent kernel, from the occurrence counts
             hd->dp = dp;
             std::vector<int64_t> optr(h_occ_ptr.begin(), h_occ_ptr.end());
             persist_prepare(hd, optr.data());
@@ -661,6 +680,7 @@ static void ensure_gather(Handle *hd) {
     StepScalars sc{};
     sc.t = hd->t_done;
     if (hd->dp.kind == FEM_BMINCUT) launch_potts(hd, sc, hd->wide_live, /*step=*/false, 0, hd->R / hd->Rb);
+    else if (hd->dp.lit_state) launch_qsat(hd, sc, hd->wide_live, /*step=*/false, 0, hd->R / hd->Rb);
     else launch_prepare_q2(hd, hd->wide_live);
     hd->gather_valid = true;
 }
@@ -671,7 +691,7 @@ fem_status fem_get_marginals(fem_handle *h, float *marginals) {
     if (hd->R < 1) return fail(hd, FEM_ESTATE, "no fields yet");
     // the fp32 scratch array (g[cur ^ 1]) is free here: the next step (or the narrowing) overwrites it anyway
     float *scratch = hd->scratch();
-    if (hd->dp.kind == FEM_BMINCUT) launch_potts_softmax(hd, scratch);
+    if (hd->dp.F > 1) launch_potts_softmax(hd, scratch);
     else launch_sigmoid(hd, scratch);
     return fetch_state(hd, scratch, nullptr, marginals);
 }
@@ -768,6 +788,7 @@ fem_status fem_anneal(fem_handle *h, const fem_schedule *sch, int32_t R, uint64_
     ensure_gather(hd);
     auto one_step = [&](int t, int b0, int bc) {
         if (hd->dp.kind == FEM_BMINCUT) launch_potts(hd, scalars(t), hd->wide_live, true, b0, bc);
+        else if (hd->dp.lit_state) launch_qsat(hd, scalars(t), hd->wide_live, true, b0, bc);
         else launch_step_q2(hd, scalars(t), hd->wide_live, b0, bc);
     };
     const int t0 = hd->t_done;

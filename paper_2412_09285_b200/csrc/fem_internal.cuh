@@ -66,6 +66,10 @@ struct DevProblem {
     const int *occ;
     const int *clause_ptr;  // [m+1], for the unsat count
     const int *lits;        // signed 1-based
+    // non-Boolean SAT (F = q fields per variable): occ_ptr has n*q + 1 entries (occurrences of variable i with clause value s
+    // are occ_ptr[i*q+s]..), an occurrence holds the gather ROWS k*q + W_mk of the other variables of its clause, padded with
+    // row n*q; lit_state [nlits] is kept for the unsat count
+    const int *lit_state;
 };
 
 // One replica block's state arrays (block base pointers; a launch with gridDim.y > 1 walks blocks).

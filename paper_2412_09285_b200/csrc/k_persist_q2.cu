@@ -272,7 +272,7 @@ static int persist_choose(const Handle *hd, int R) {
     if (hd->opt_persistent == 0) return -1;
     const bool graph = hd->dp.kind == FEM_MAXCUT || (hd->dp.kind == FEM_ISING && !hd->dp.J);
     // Max-SAT: clause length <= 5 (one kernel per k_max - 1 = 1..4), packed entries (var << 1 | negated) in 16 bits
-    const bool sat = hd->dp.kind == FEM_MAXSAT && hd->dp.kstride >= 1 && hd->dp.kstride <= 4 && hd->dp.n <= 32767;
+    const bool sat = hd->dp.kind == FEM_MAXSAT && !hd->dp.lit_state && hd->dp.kstride >= 1 && hd->dp.kstride <= 4 && hd->dp.n <= 32767;
     if (!graph && !sat) return -1;
     if (graph && hd->dp.n_long > 0 && hd->opt_long_rows) return -1;  // long rows: the stepwise kernel splits them over a CTA (k_step_q2.cu)
     int best = -1;

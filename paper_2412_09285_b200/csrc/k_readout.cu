@@ -112,7 +112,9 @@ __global__ void __launch_bounds__(kThreads) energy_sat_kernel(const ReadoutParam
             const int lit = __ldg(p.dp.lits + x);
             const int v = (lit > 0 ? lit : -lit) - 1;
             const int s = cf[(int64_t)v * p.Rb];
-            sat = sat || ((lit > 0) == (s == 1));
+            // non-Boolean SAT: satisfied when some variable takes its clause value W_mi
+            if (p.dp.lit_state) sat = sat || (s == __ldg(p.dp.lit_state + x));
+            else sat = sat || ((lit > 0) == (s == 1));
         }
         unsat += sat ? 0 : 1;
     }

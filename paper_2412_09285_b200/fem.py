@@ -41,6 +41,7 @@ class CProblem(C.Structure):
         ("row_ptr", C.c_void_p), ("col_idx", C.c_void_p), ("weight", C.c_void_p), ("dense_J", C.c_void_p),
         ("m", C.c_int32), ("clause_ptr", C.c_void_p), ("lits", C.c_void_p), ("lambda_", C.c_double),
         ("node_weight", C.c_void_p),   # ABI 4: BMINCUT node weights V_i (float32 [n]) or NULL
+        ("lit_state", C.c_void_p),     # ABI 4: non-Boolean MAXSAT clause values W_mi (int32 [nlits]) or NULL
     ]
 
 
@@ -173,7 +174,8 @@ class Fem:
                             _ptr(host(inst.col_idx, np.int32)), _ptr(host(inst.weight, np.float32)),
                             _ptr(host(inst.dense_J, np.float32)), inst.m, _ptr(host(inst.clause_ptr, np.int64)),
                             _ptr(host(inst.lits, np.int32)), float(inst.lam),
-                            _ptr(host(getattr(inst, "node_weight", None), np.float32)))
+                            _ptr(host(getattr(inst, "node_weight", None), np.float32)),
+                            _ptr(host(getattr(inst, "lit_state", None), np.int32)))
         nbytes = self._lib.fem_workspace_bytes(C.byref(self._cp), self.R_cap)
         if nbytes == 0:
             raise FemError(FEM_EINVAL, "fem_workspace_bytes rejected the problem")
