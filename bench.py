@@ -267,7 +267,7 @@ def run_workload(args, name, steps, warmup, ctx, with_e2e=True):
     readout_ms = sum(e[1].elapsed_time(e[4]) for e in bulk_events) / max(len(bulk_events), 1)
     # algorithmic bytes of one launch: the whole step's bytes spread over the launches that make up a step
     step_bytes = eng.info("step_bytes") * (N - K) * steps / max(bulk_launches, 1)
-    info = {k: eng.info(k) for k in ("tc_launches", "persist_launches", "tma_launches", "lane_launches", "si_launches", "replica_block", "nnz")}
+    info = {k: eng.info(k) for k in ("tc_launches", "tc8_launches", "persist_launches", "tma_launches", "lane_launches", "si_launches", "replica_block", "nnz")}
     eng.close()
 
     # ---- e2e through the public API from host buffers (pinned), host<->device copies inside the timed region
@@ -320,14 +320,22 @@ def run_workload(args, name, steps, warmup, ctx, with_e2e=True):
         # three MMAs per algorithmic product; `achieved` counts the ALGORITHMIC flops only.
         flops = 2.0 * n * n * R
         achieved = flops / (kernel_us * 1e-6) / 1e12
-        tf32_peak = 0.5 * float(peaks.get("bf16_tflops_sustained", peaks.get("bf16_tflops", 1671.0)))
+        bf16 = float(peaks.get("bf16_tflops_sustained", peaks.get("bf16_tflops", 1671.0)))
+        tf32_peak = 0.5 * bf16
+        i8 = info["tc8_launches"] > 0
         roofline = {"bound": "tensor",
-                    "kernel": "dense_tc_step_kernel (tcgen05 3xTF32 GEMM, FEM update fused in the TMEM epilogue)",
+                    "kernel": ("dense_i8_step_kernel (tcgen05 kind::i8: both operands as three signed 8-bit digits of a 23-bit fixed point, six "
+                               "MMAs per product into exact int32 accumulators; FEM update fused in the TMEM epilogue)" if i8 else
+                               "dense_tc_step_kernel (tcgen05 3xTF32 GEMM, FEM update fused in the TMEM epilogue)"),
                     "achieved": achieved, "peak": tf32_peak, "unit": "TFLOP/s", "frac": achieved / tf32_peak,
                     "traffic": load_traffic(name),
-                    "peak_source": "0.5 x measured sustained bf16 cuBLAS TFLOP/s (MEASURED_PEAKS.json; "
-                                   "tf32:bf16 nominal ratio 1:2)",
-                    "algorithmic_flops_per_launch": flops, "mma_tflops_issued": 3.0 * achieved,
+                    "peak_source": "0.5 x measured sustained bf16 cuBLAS TFLOP/s (MEASURED_PEAKS.json; tf32:bf16 nominal ratio 1:2): the "
+                                   "roof of an fp32-accurate product issued as ONE tf32 MMA per product; `achieved` counts the algorithmic "
+                                   "2 n^2 R flop only",
+                    "algorithmic_flops_per_launch": flops,
+                    "mma_tflops_issued": (6.0 if i8 else 3.0) * achieved,
+                    "issued_frac_of_own_dtype_peak": ((6.0 * achieved) / (2.0 * bf16)) if i8 else (3.0 * achieved / tf32_peak),
+                    "own_dtype_peak_source": ("int8: 2 x measured sustained bf16 (nominal ratio 2:1)" if i8 else "tf32: 0.5 x measured sustained bf16"),
                     "kernel_us": kernel_us, "kernel_share_of_step": share}
     elif info["persist_launches"] > 0:
         # small sparse two-state problem: replica-persistent cluster kernel, state in registers, gathers from shared

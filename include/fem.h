@@ -185,8 +185,9 @@ fem_status fem_energy_of(fem_handle *h, const int32_t *cfg /* [count][n] */, int
  * device's L2 size, the default; >= R = no blocking), "steps_per_block" (steps run on one replica
  * block before moving to the next; 0 = the whole anneal per block, the default; 1 = step-major).
  * Results do not depend on either (replicas are independent).  Dense ISING only: "tensor_cores"
- * (1 = tcgen05 3xTF32 step, the default where it applies: n % 4 == 0 and R % 32 == 0; 0 = CUDA-core
- * GEMM) and "tc_tile_n" (replica columns per tensor-core tile: 0 = default, 32/64/128/256).
+ * (1 = the default: the int8 digit step on tcgen05 (kind::i8, k_dense_i8.cu) where it applies -- R a multiple of 32, plain
+ * Adam on the exact gradient --, else the 3xTF32 step; 2 = the 3xTF32 step (kind::tf32; n % 4 == 0); 0 = CUDA-core GEMM)
+ * and "tc_tile_n" (replica columns per tensor-core tile: 0 = default, 32/64/128, and 256 for the 3xTF32 step only).
  * "persistent" (small sparse MAXCUT / ISING / MAXSAT problems with few enough replicas to run in at most three
  * waves of clusters: 1 = replica-persistent cluster kernel where the problem fits, the default; 0 = one launch per step; 1 + CS = force clusters of CS = 1, 2, 4 or 8 CTAs per replica) and
  * "long_rows" (two-state graph kinds: 1 = rows with many entries are summed by a CTA each in a fixed order, the default;
@@ -198,7 +199,7 @@ fem_status fem_energy_of(fem_handle *h, const int32_t *cfg /* [count][n] */, int
  * 0 = the default).  None of them changes a single bit of the results.  Unknown key: FEM_EINVAL. */
 fem_status fem_set_option(fem_handle *h, const char *key, int64_t value);
 /* Introspection for benchmarks: "launches" (kernels enqueued so far), "tc_launches" (of which tcgen05
- * dense steps), "persist_launches", "persist_cluster" (CTAs per replica of the persistent kernel),
+ * dense steps; "tc8_launches": of those, int8 digit steps), "persist_launches", "persist_cluster" (CTAs per replica of the persistent kernel),
  * "tma_launches" (TMA-staged Potts steps), "lane_launches" (lane-per-replica Potts steps), "si_launches" (state-innermost Potts steps), "t_done", "R", "replica_block", "nnz", "uniform_degree",
  * "max_degree", "long_rows" (rows of a two-state graph kind with more than 96 entries, or more than 32 and four times the mean degree:
  * the stepwise kernel gives each

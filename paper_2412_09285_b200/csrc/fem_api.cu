@@ -28,7 +28,7 @@ cudaError_t persist_run(Handle *hd, bool wide, int t_begin, int t_end, StepScala
 static std::string g_create_error;
 
 struct Layout {
-    size_t row_ptr, col, w, rowsum, long_rows, vw, lit_state, J, Jlo, glo0, glo1, field, occ_ptr, occ, clause_ptr, lits;
+    size_t row_ptr, col, w, rowsum, long_rows, vw, lit_state, J, Jlo, glo0, glo1, J8, gt8_0, gt8_1, jscale, field, occ_ptr, occ, clause_ptr, lits;
     size_t h, m1, m2, g0, g1, stage, hW, m1W, m2W, gW0, gW1, colsum0, colsum1, colsum2, cfg, e_part_i, e_part_d, part_part, e_int, e_real, part,
         best, total;
 };
@@ -121,6 +121,11 @@ static Layout make_layout(const fem_problem *pb, const ProblemShape &s, int R_ca
     L.Jlo = take(s.dense ? (size_t)pb->n * pb->n * 4 : 0);
     L.glo0 = take(s.dense ? state : 0);
     L.glo1 = take(s.dense ? state : 0);
+    const size_t np8 = ((size_t)pb->n + 15) & ~(size_t)15;  // int8 digit planes (k_dense_i8.cu): rows padded to 16 bytes
+    L.J8 = take(s.dense ? 3 * (size_t)pb->n * np8 : 0);
+    L.gt8_0 = take(s.dense ? 3 * (size_t)R_cap * np8 : 0);
+    L.gt8_1 = take(s.dense ? 3 * (size_t)R_cap * np8 : 0);
+    L.jscale = take(s.dense ? (size_t)pb->n * 8 : 0);
     L.field = take(s.dense ? 2 * state : 0);  // fp64 in the wide phase
     L.occ_ptr = take(pb->kind == FEM_MAXSAT ? ((size_t)pb->n * F + 1) * 4 : 0);
     L.lit_state = take(pb->lit_state ? (size_t)s.nlits * 4 : 0);
@@ -443,6 +448,11 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
         hd->Jlo = reinterpret_cast<float *>(at(L.Jlo));
         hd->glo[0] = reinterpret_cast<float *>(at(L.glo0));
         hd->glo[1] = reinterpret_cast<float *>(at(L.glo1));
+        hd->J8 = reinterpret_cast<signed char *>(at(L.J8));
+        hd->gt8[0] = reinterpret_cast<signed char *>(at(L.gt8_0));
+        hd->gt8[1] = reinterpret_cast<signed char *>(at(L.gt8_1));
+        hd->jscale = reinterpret_cast<double *>(at(L.jscale));
+        hd->i8_np = (n + 15) & ~15;
         if (ok) launch_tc_split(hd);  // J_lo = J - tf32(J) for the 3xTF32 tensor-core path
         hd->integral_weights = false;
         hd->structure_bytes = 4 * (int64_t)n * n;
@@ -554,6 +564,7 @@ fem_status fem_reset(fem_handle *h) {
     hd->readout_valid = false;
     hd->wide_live = false;
     hd->tc_ready = false;
+    hd->tc8_ready = false;
     hd->gather_h = hd->gather_h_want = false;
     return FEM_OK;
 }
@@ -591,7 +602,7 @@ fem_status fem_set_option(fem_handle *h, const char *key, int64_t value) {
         if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "potts_si must be 0 or 1");
         hd->opt_potts_si = value;
     } else if (!strcmp(key, "tensor_cores")) {
-        if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "tensor_cores must be 0 or 1");
+        if (value < 0 || value > 2) return fail(hd, FEM_EINVAL, "tensor_cores must be 0, 1 or 2");
         hd->opt_tensor_cores = value;
     } else {
         return fail(hd, FEM_EINVAL, "unknown option");
@@ -604,6 +615,7 @@ int64_t fem_get_info(const fem_handle *h, const char *key) {
     if (!hd || !key) return -1;
     if (!strcmp(key, "launches")) return hd->launches;
     if (!strcmp(key, "tc_launches")) return hd->tc_launches;
+    if (!strcmp(key, "tc8_launches")) return hd->tc8_launches;
     if (!strcmp(key, "persist_launches")) return hd->persist_launches;
     if (!strcmp(key, "persist_cluster")) return hd->persist_cluster;
     if (!strcmp(key, "tma_launches")) return hd->tma_launches;
@@ -645,6 +657,7 @@ fem_status fem_set_fields(fem_handle *h, int32_t R, const float *fields) {
     hd->readout_valid = false;
     hd->wide_live = false;
     hd->tc_ready = false;
+    hd->tc8_ready = false;
     hd->gather_h = hd->gather_h_want = false;  // the injected fields are in hd->h
     return FEM_OK;
 }
@@ -738,6 +751,7 @@ fem_status fem_anneal(fem_handle *h, const fem_schedule *sch, int32_t R, uint64_
         }
         hd->gather_valid = false;
         hd->tc_ready = false;
+        hd->tc8_ready = false;
         hd->gather_h = hd->gather_h_want = false;
     }
     const int nb = hd->R / hd->Rb;
@@ -808,6 +822,7 @@ fem_status fem_anneal(fem_handle *h, const fem_schedule *sch, int32_t R, uint64_
         launch_narrow(hd, false);
         hd->wide_live = false;
         hd->tc_ready = false;
+        hd->tc8_ready = false;
     }
     if (hd->gather_h_want && !hd->gather_h && !hd->wide_live && t < stop_after) {
         // The first fp32 step of a trajectory takes the default path: its gather array is the accurately rounded one

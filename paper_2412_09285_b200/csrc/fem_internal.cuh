@@ -101,6 +101,14 @@ struct Handle {
     alignas(64) unsigned char tc_maps[6 * 128];  // CUtensorMap x6: J, Jlo, GT[0], GTlo[0], GT[1], GTlo[1]
     int tc_maps_R = -1, tc_maps_bn = -1;     // the maps bake in R (rows of GT) and the tile height bn
     bool tc_ready = false;                   // g[cur]/glo[cur] hold GT / GT_lo of the current fields
+    // dense Ising on the int8 tensor-core path (k_dense_i8.cu): digit planes of J and of the transposed magnetisations
+    signed char *J8 = nullptr, *gt8[2] = {nullptr, nullptr};  // [3][n][np], [3][R_cap][np] x 2
+    double *jscale = nullptr;                // [n] row scales of J (over 64)
+    int i8_np = 0;                           // row pitch of the digit planes: n rounded up to 16
+    alignas(64) unsigned char tc8_maps[9 * 128];  // CUtensorMap x9: J digits 0..2, GT8[0] digits, GT8[1] digits
+    int tc8_maps_R = -1, tc8_maps_bn = -1;
+    bool tc8_ready = false, tc8_split_done = false;  // gt8[cur] holds the digits of the current fields; J8 / jscale are made
+    int64_t tc8_launches = 0;
     double *rowsum = nullptr;  // graph kinds: sum_j |W_ij| per node (manipulated gradients: c_i, c^f_i, c^a_i)
     int bytes_per_field = 24;  // algorithmic HBM bytes per field per step: read + write of h and of the moments in use
     bool plain_adam = true;    // Adam on the exact gradient: the only update the tcgen05 dense step implements

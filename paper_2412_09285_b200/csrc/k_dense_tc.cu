@@ -360,7 +360,7 @@ void launch_tc_split(Handle *hd) {
 bool launch_step_dense_tc(Handle *hd, const StepScalars &sc) {
     const int n = hd->dp.n, Rb = hd->Rb;
     const int bn = tc_tile_n(n, Rb, (int)hd->opt_tc_tile_n);
-    if (bn == 0 || hd->R != Rb || !hd->Jlo || !hd->opt_tensor_cores) return false;
+    if (bn == 0 || hd->R != Rb || !hd->Jlo || !hd->opt_tensor_cores) return false;  // (tensor_cores = 2 forces this path)
     if (hd->tc_maps_R != hd->R || hd->tc_maps_bn != bn) {  // the maps bake in R (rows of GT) and the box height bn
         CUtensorMap *m = reinterpret_cast<CUtensorMap *>(hd->tc_maps);
         bool ok = make_map(&m[0], hd->dp.J, n, n, TC_BM) && make_map(&m[1], hd->Jlo, n, n, TC_BM);

@@ -547,14 +547,22 @@ static void launch_q2_mode(Handle *hd, const Q2Params<T> &p, dim3 grid, int mode
 }
 
 bool launch_step_dense_tc(Handle *hd, const StepScalars &sc);  // k_dense_tc.cu
+bool launch_step_dense_i8(Handle *hd, const StepScalars &sc);  // k_dense_i8.cu
 void launch_prepare_q2(Handle *hd, bool wide);
 
 template <typename T>
 static void launch_step_q2_t(Handle *hd, const StepScalars &sc, int blk_begin, int blk_count) {
     using S = StateOf<T>;
-    if (std::is_same<T, float>::value && hd->dp.kind == FEM_ISING && hd->dp.J && blk_begin == 0 && blk_count == 1 && hd->plain_adam &&
-        launch_step_dense_tc(hd, sc))
-        return;  // dense couplings: tcgen05 GEMM with the update fused in its epilogue
+    if (std::is_same<T, float>::value && hd->dp.kind == FEM_ISING && hd->dp.J && blk_begin == 0 && blk_count == 1 && hd->plain_adam) {
+        // dense couplings: tcgen05 GEMM with the update fused in its epilogue -- the int8 digit path (k_dense_i8.cu) where it
+        // applies, else 3xTF32 (k_dense_tc.cu).  A trajectory stays on the path its first tensor-core step took.
+        if (!hd->tc_ready && launch_step_dense_i8(hd, sc)) return;
+        if (!hd->tc8_ready && launch_step_dense_tc(hd, sc)) return;
+    }
+    if (std::is_same<T, float>::value && hd->tc8_ready) {  // the fp32 gather array was not maintained by the int8 steps
+        hd->tc8_ready = false;
+        launch_prepare_q2(hd, false);
+    }
     if (std::is_same<T, float>::value && hd->tc_ready) {
         // a tensor-core step (or its preparation) left g[cur] in the TRANSPOSED layout GT[a][i]; this path reads
         // g[cur] as [i][Rb].  Rebuild it from the fields before gathering from it.

@@ -240,24 +240,26 @@ def test_full_anneal_energy_distribution_cfg0(fem):
 
 
 def test_dense_tensor_core_path_is_taken_and_agrees_with_cuda_cores(fem):
-    """Dense Ising: the tcgen05 3xTF32 step (default) against the CUDA-core GEMM step on the same fields, and
-    against the oracle; the info counter proves which kernel ran."""
+    """Dense Ising: the tcgen05 int8 digit step (default) and the 3xTF32 step against the CUDA-core GEMM step on the same
+    fields, and against the oracle; the info counters prove which kernel ran."""
     inst, R = get("ising_dense_sk_tc")
     beta = fem.linear_temperature_schedule(1.0, 0.01, 500)
     h0 = fo.init_fields(5, R, inst.n, 1).astype(np.float32)
     pb, st = oracle_run(inst, h0, beta, 30, inst.lam)
     P_ref = fo.marginals(pb, st.h)
     out = {}
-    for tc in (1, 0):
+    for tc in (1, 2, 0):                                            # int8 digit step (default), 3xTF32 step, CUDA cores
         eng = fem.Fem(inst, R)
         eng.set_option("tensor_cores", tc)
         eng.set_fields(h0)
         eng.anneal(fem.Schedule(beta=beta, precise_steps=8), R, stop_after=30)
         out[tc] = eng.get_marginals().astype(np.float64)
-        assert (eng.info("tc_launches") == 22) == (tc == 1)         # 30 steps - 8 wide ones
+        assert (eng.info("tc_launches") == 22) == (tc != 0)         # 30 steps - 8 wide ones
+        assert (eng.info("tc8_launches") == 22) == (tc == 1)
         assert np.max(np.abs(out[tc] - P_ref.reshape(out[tc].shape))) < MARGINAL_TOL
+        print("tensor_cores", tc, "max |dP| vs oracle", np.max(np.abs(out[tc] - P_ref.reshape(out[tc].shape))))
         eng.close()
-    assert np.max(np.abs(out[1] - out[0])) < MARGINAL_TOL
+    assert np.max(np.abs(out[1] - out[0])) < MARGINAL_TOL and np.max(np.abs(out[2] - out[0])) < MARGINAL_TOL
 
 
 @pytest.mark.parametrize("bn", [32, 64, 128, 256])
