@@ -595,6 +595,11 @@ fem_status fem_set_option(fem_handle *h, const char *key, int64_t value) {
     } else if (!strcmp(key, "potts_lane")) {
         if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "potts_lane must be 0 or 1");
         hd->opt_potts_lane = value;
+    } else if (!strcmp(key, "tc_debug")) {
+        hd->opt_tc_debug = value;
+    } else if (!strcmp(key, "tc_cluster")) {
+        if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "tc_cluster must be 0 or 1");
+        hd->opt_tc_cluster = value;
     } else if (!strcmp(key, "long_rows")) {
         if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "long_rows must be 0 or 1");
         hd->opt_long_rows = value;

@@ -109,6 +109,8 @@ struct Handle {
     int tc8_maps_R = -1, tc8_maps_bn = -1;
     bool tc8_ready = false, tc8_split_done = false;  // gt8[cur] holds the digits of the current fields; J8 / jscale are made
     int64_t tc8_launches = 0;
+    int64_t opt_tc_debug = 0;  // TEMPORARY
+    int64_t opt_tc_cluster = 1;  // int8 dense step: 2 x 2 clusters with operand multicast where the grid allows it
     double *rowsum = nullptr;  // graph kinds: sum_j |W_ij| per node (manipulated gradients: c_i, c^f_i, c^a_i)
     int bytes_per_field = 24;  // algorithmic HBM bytes per field per step: read + write of h and of the moments in use
     bool plain_adam = true;    // Adam on the exact gradient: the only update the tcgen05 dense step implements

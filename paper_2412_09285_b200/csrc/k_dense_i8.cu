@@ -26,14 +26,17 @@ namespace fem {
 constexpr int I8_BM = 128;       // rows of F per CTA = TMEM lanes
 constexpr int I8_BK = 128;       // int8 elements per k-block = one 128-byte swizzle atom
 constexpr int I8_UMMA_K = 32;    // int8 elements per tcgen05.mma
-constexpr int I8_THREADS = 192;
+constexpr int I8_EPI_GROUPS = 2;  // epilogue warps per TMEM lane quadrant (each takes BN / groups columns)
+constexpr int I8_THREADS = 64 + 128 * I8_EPI_GROUPS;
 constexpr int I8_FRAC_BITS = 22; // fixed point: |x| <= 2^22 - 1, digits d0 in [-64, 64], d1, d2 in [-128, 127]
 
 template <int BN>
 struct I8Shape {
     static constexpr int kStageBytes = 3 * I8_BM * 128 + 3 * BN * 128;  // three digits of A and of B
     static constexpr int kStages = BN >= 128 ? 2 : 3;
-    static constexpr int kSmem = kStages * kStageBytes + 1024;
+    static constexpr int kColsWarp = BN / I8_EPI_GROUPS >= 16 ? BN / I8_EPI_GROUPS : 16;
+    static constexpr int kEpiBytes = 4 * I8_EPI_GROUPS * 3 * 32 * (kColsWarp + 4) * 4;  // epilogue staging (reuses the stages)
+    static constexpr int kSmem = (kStages * kStageBytes > kEpiBytes ? kStages * kStageBytes : kEpiBytes) + 1024;
     static constexpr int kTmemCols = 3 * BN <= 128 ? 128 : (3 * BN <= 256 ? 256 : 512);
 };
 
@@ -43,6 +46,7 @@ struct I8Params {
     const double *jscale;      // [n] sJ_i / 2^6: F = jscale_i * (2^16 acc0 + 2^8 acc1 + acc2)
     Sc<float> sc;
     int n, np, Rb;
+    int debug;  // TEMPORARY
 };
 
 // ---- PTX wrappers (as in k_dense_tc.cu) ----
@@ -72,6 +76,23 @@ __device__ __forceinline__ void i8_tma_load_2d(void *smem_dst, const CUtensorMap
             i8_smem_u32(smem_dst)),
         "l"(tm), "r"(c0), "r"(c1), "r"(i8_smem_u32(bar))
         : "memory");
+}
+// the same tile delivered to the same shared-memory offset (and mbarrier) of every CTA of the cluster named in cta_mask
+__device__ __forceinline__ void i8_tma_load_2d_mc(void *smem_dst, const CUtensorMap *tm, int c0, int c1, uint64_t *bar, uint16_t cta_mask) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.multicast::cluster [%0], [%1, {%2, %3}], [%4], %5;" ::"r"(
+            i8_smem_u32(smem_dst)),
+        "l"(tm), "r"(c0), "r"(c1), "r"(i8_smem_u32(bar)), "h"(cta_mask)
+        : "memory");
+}
+__device__ __forceinline__ void i8_commit_mc(uint64_t *bar, uint16_t cta_mask) {  // arrive on the barrier at this offset in every CTA of the mask
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(i8_smem_u32(bar)),
+                 "h"(cta_mask)
+                 : "memory");
+}
+__device__ __forceinline__ void i8_cluster_sync() {
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 __device__ __forceinline__ uint64_t i8_desc_sw128(uint32_t smem_addr) {
     return (uint64_t)((smem_addr & 0x3FFFF) >> 4) | (1ull << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
@@ -115,9 +136,16 @@ __device__ __forceinline__ int i8_fixed_of(float m) {  // |m| <= 1
 }
 
 // ---- the fused step ----
-// Warp roles (192 threads): warp 0 = TMA producer (one elected lane), warp 1 = TMEM allocator + MMA issuer (one elected
-// lane), warps 2..5 = epilogue (warp w reads TMEM lanes 32*(w%4) .. +31).
-template <int BN>
+// Warp roles: warp 0 = TMA producer (one elected lane), warp 1 = TMEM allocator + MMA issuer (one elected lane), warps 2..9 =
+// epilogue (warp w reads TMEM lanes 32*(w%4) .. +31; the two warps of a lane quadrant split the BN columns).  With one warp per
+// scheduler the epilogue was bound by its own dependency chains and by DRAM round trips (2 x 44 us of a 147 us step): two warps
+// per scheduler, and the h / m1 / m2 rows of a 16-column block are requested one block ahead (the first before the main loop ends).
+// CL: 2 x 2 thread-block clusters with operand multicast.  The four CTAs of a cluster compute a 256 x 2 BN block of F; the two
+// CTAs with the same rows share the J digits, the two with the same replica columns share the GT8 digits: every CTA fetches
+// HALF of each of its operand tiles and multicasts it to the CTA that needs it too, so the L2 -> SMEM traffic per CTA is
+// halved (the int8 main loop is bound by that feed: 96 KB per 24 MMAs).  A stage may be refilled when the CTA itself and
+// both CTAs it multicasts to have consumed it: the MMA issuer's commit arrives on the empty barrier of all three.
+template <int BN, bool CL>
 __global__ void __launch_bounds__(I8_THREADS, 1)
 dense_i8_step_kernel(const __grid_constant__ CUtensorMap tmJ0, const __grid_constant__ CUtensorMap tmJ1,
                      const __grid_constant__ CUtensorMap tmJ2, const __grid_constant__ CUtensorMap tmG0,
@@ -131,7 +159,12 @@ dense_i8_step_kernel(const __grid_constant__ CUtensorMap tmJ0, const __grid_cons
     uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int m0 = blockIdx.x * I8_BM, n0 = blockIdx.y * BN;
-    const int nkb = (p.n + I8_BK - 1) / I8_BK;
+    const int nkb = (p.debug & 2) ? 1 : (p.n + I8_BK - 1) / I8_BK;
+    uint32_t cx = 0, cy = 0;  // position inside the 2 x 2 cluster (rank = cx + 2 cy)
+    if (CL) {
+        asm volatile("mov.u32 %0, %%cluster_ctaid.x;" : "=r"(cx));
+        asm volatile("mov.u32 %0, %%cluster_ctaid.y;" : "=r"(cy));
+    }
 
     if (warp == 0 && lane == 0) {
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmJ0));
@@ -142,7 +175,7 @@ dense_i8_step_kernel(const __grid_constant__ CUtensorMap tmJ0, const __grid_cons
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmG2));
         for (int s = 0; s < S::kStages; ++s) {
             i8_mbar_init(&full_bar[s], 1);
-            i8_mbar_init(&empty_bar[s], 1);
+            i8_mbar_init(&empty_bar[s], CL ? 3 : 1);  // CL: this CTA and the two it multicasts to
         }
         i8_mbar_init(&tmem_full_bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -154,6 +187,7 @@ dense_i8_step_kernel(const __grid_constant__ CUtensorMap tmJ0, const __grid_cons
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    if (CL) i8_cluster_sync();  // every CTA's barriers are initialised before a peer multicasts into it or arrives on them
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem_d = tmem_base_slot;
 
@@ -167,13 +201,30 @@ dense_i8_step_kernel(const __grid_constant__ CUtensorMap tmJ0, const __grid_cons
             i8_mbar_wait(&empty_bar[s], ph ^ 1);
             uint8_t *st = smem + (size_t)s * S::kStageBytes;
             i8_mbar_expect_tx(&full_bar[s], S::kStageBytes);
-            i8_tma_load_2d(st, &tmJ0, kb * I8_BK, m0, &full_bar[s]);
-            i8_tma_load_2d(st + I8_BM * 128, &tmJ1, kb * I8_BK, m0, &full_bar[s]);
-            i8_tma_load_2d(st + 2 * I8_BM * 128, &tmJ2, kb * I8_BK, m0, &full_bar[s]);
             uint8_t *sb = st + 3 * I8_BM * 128;
-            i8_tma_load_2d(sb, &tmG0, kb * I8_BK, n0, &full_bar[s]);
-            i8_tma_load_2d(sb + BN * 128, &tmG1, kb * I8_BK, n0, &full_bar[s]);
-            i8_tma_load_2d(sb + 2 * BN * 128, &tmG2, kb * I8_BK, n0, &full_bar[s]);
+            if (CL) {
+                // my half of the J rows (the other CTA of my row pair loads the other half), to both of us
+                const uint16_t maskA = (uint16_t)((1u << cx) | (1u << (cx + 2)));
+                uint8_t *da = st + cy * (I8_BM / 2) * 128;
+                const int ra = m0 + (int)cy * (I8_BM / 2);
+                i8_tma_load_2d_mc(da, &tmJ0, kb * I8_BK, ra, &full_bar[s], maskA);
+                i8_tma_load_2d_mc(da + I8_BM * 128, &tmJ1, kb * I8_BK, ra, &full_bar[s], maskA);
+                i8_tma_load_2d_mc(da + 2 * I8_BM * 128, &tmJ2, kb * I8_BK, ra, &full_bar[s], maskA);
+                // my half of the GT8 rows, to both CTAs of my column pair
+                const uint16_t maskB = (uint16_t)(3u << (2 * cy));
+                uint8_t *db = sb + cx * (BN / 2) * 128;
+                const int rb = n0 + (int)cx * (BN / 2);
+                i8_tma_load_2d_mc(db, &tmG0, kb * I8_BK, rb, &full_bar[s], maskB);
+                i8_tma_load_2d_mc(db + BN * 128, &tmG1, kb * I8_BK, rb, &full_bar[s], maskB);
+                i8_tma_load_2d_mc(db + 2 * BN * 128, &tmG2, kb * I8_BK, rb, &full_bar[s], maskB);
+            } else {
+                i8_tma_load_2d(st, &tmJ0, kb * I8_BK, m0, &full_bar[s]);
+                i8_tma_load_2d(st + I8_BM * 128, &tmJ1, kb * I8_BK, m0, &full_bar[s]);
+                i8_tma_load_2d(st + 2 * I8_BM * 128, &tmJ2, kb * I8_BK, m0, &full_bar[s]);
+                i8_tma_load_2d(sb, &tmG0, kb * I8_BK, n0, &full_bar[s]);
+                i8_tma_load_2d(sb + BN * 128, &tmG1, kb * I8_BK, n0, &full_bar[s]);
+                i8_tma_load_2d(sb + 2 * BN * 128, &tmG2, kb * I8_BK, n0, &full_bar[s]);
+            }
         }
     } else if (warp == 1 && lane == 0) {
         // ===== MMA issuer: acc0 = S00, acc1 = S01 + S10, acc2 = S02 + S11 + S20 =====
@@ -201,63 +252,109 @@ dense_i8_step_kernel(const __grid_constant__ CUtensorMap tmJ0, const __grid_cons
                 i8_umma(acc2, dA2, dB0, idesc, 1);
                 started = 1;
             }
-            i8_commit(&empty_bar[s]);  // frees the smem stage when these MMAs have read it
+            // frees the smem stage when these MMAs have read it -- here and, with clusters, in the two CTAs that multicast into it
+            if (CL) i8_commit_mc(&empty_bar[s], (uint16_t)((1u << (cx + 2 * cy)) | (1u << (cx + 2 * (1 - cy))) | (1u << ((1 - cx) + 2 * cy))));
+            else i8_commit(&empty_bar[s]);
         }
         i8_commit(&tmem_full_bar);  // accumulators complete
     } else if (warp >= 2) {
         // ===== epilogue: TMEM -> registers -> FEM update -> HBM =====
-        i8_mbar_wait(&tmem_full_bar, 0);
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         const int quad = warp & 3;
         const int i = m0 + quad * 32 + lane;
         const bool row_ok = i < p.n;
         const Sc<float> &sc = p.sc;
-        const size_t rowoff = (size_t)(row_ok ? i : 0) * p.Rb + n0;
-        const double js = row_ok ? p.jscale[i] : 0.0;
+        constexpr int kCols = BN / I8_EPI_GROUPS >= 16 ? BN / I8_EPI_GROUPS : 16;  // columns of this warp
+        const int cbeg = ((warp - 2) >> 2) * kCols;
+        const bool has_cols = cbeg < BN;
+        const float js = row_ok ? (float)p.jscale[i] : 0.0f;
         const size_t plane = (size_t)p.Rb * p.np;  // one digit plane of GT8
+        // TMEM lanes are rows i, so a lane's h / m1 / m2 values sit a whole row pitch apart in HBM: read straight from there,
+        // every load instruction touched 32 different lines and the epilogue was bound by L1 tag lookups and exposed DRAM round
+        // trips (2 x 31 us of a 137 us step).  When the accumulators are complete the operand stages are free: each warp stages its
+        // 32 x kCols sub-tile of the three arrays there with cp.async -- 16 lanes per row, coalesced, the whole sub-tile in flight
+        // at once --, works out of shared memory (rows padded to kPitch floats: conflict-free 16-byte accesses), and writes the
+        // results back through the same slots.
+        constexpr int kPitch = kCols + 4;                    // floats per staged row
+        constexpr int kArr = 32 * kPitch;                    // floats per staged array
+        float *stg = reinterpret_cast<float *>(smem) + (size_t)(warp - 2) * (3 * kArr);
+        constexpr int kChunks = kCols / 4;                   // 16-byte pieces per row
+        i8_mbar_wait(&tmem_full_bar, 0);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        if (has_cols && !(p.debug & 1)) {
+            const int rows_ok = min(32, p.n - (m0 + quad * 32));  // rows of this warp inside the matrix (<= 0: none)
+            const float *src[3] = {p.h, p.m1, p.m2};
+#pragma unroll
+            for (int arr = 0; arr < 3; ++arr)
+                for (int x = lane; x < 32 * kChunks; x += 32) {
+                    const int r = x / kChunks, ch = x - r * kChunks;
+                    if (r < rows_ok) {
+                        const float *g = src[arr] + (size_t)(m0 + quad * 32 + r) * p.Rb + n0 + cbeg + ch * 4;
+                        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(i8_smem_u32(stg + arr * kArr + r * kPitch + ch * 4)), "l"(g)
+                                     : "memory");
+                    }
+                }
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+            __syncwarp();
+            float *my = stg + lane * kPitch;
 #pragma unroll 1
-        for (int c0 = 0; c0 < BN; c0 += 16) {
-            int s0[16], s1[16], s2[16];
-            const uint32_t lane_base = tmem_d + ((uint32_t)(quad * 32) << 16) + (uint32_t)c0;
-            i8_tmem_ld16(lane_base, s0);  // warp-collective: no divergence here
-            i8_tmem_ld16(lane_base + (uint32_t)BN, s1);
-            i8_tmem_ld16(lane_base + (uint32_t)(2 * BN), s2);
-            if (row_ok) {
-                float hv[16], a1[16], a2[16];
+            for (int c0 = 0; c0 < kCols; c0 += 16) {
+                int s0[16], s1[16], s2[16];
+                const uint32_t lane_base = tmem_d + ((uint32_t)(quad * 32) << 16) + (uint32_t)(cbeg + c0);
+                i8_tmem_ld16(lane_base, s0);  // warp-collective: no divergence here
+                i8_tmem_ld16(lane_base + (uint32_t)BN, s1);
+                i8_tmem_ld16(lane_base + (uint32_t)(2 * BN), s2);
+                if (row_ok) {
+                    float hv[16], a1[16], a2[16];
 #pragma unroll
-                for (int v = 0; v < 4; ++v) {
-                    const float4 x = __ldcs(reinterpret_cast<const float4 *>(p.h + rowoff + c0) + v);
-                    const float4 y = __ldcs(reinterpret_cast<const float4 *>(p.m1 + rowoff + c0) + v);
-                    const float4 z = __ldcs(reinterpret_cast<const float4 *>(p.m2 + rowoff + c0) + v);
-                    hv[4 * v] = x.x, hv[4 * v + 1] = x.y, hv[4 * v + 2] = x.z, hv[4 * v + 3] = x.w;
-                    a1[4 * v] = y.x, a1[4 * v + 1] = y.y, a1[4 * v + 2] = y.z, a1[4 * v + 3] = y.w;
-                    a2[4 * v] = z.x, a2[4 * v + 1] = z.y, a2[4 * v + 2] = z.z, a2[4 * v + 3] = z.w;
-                }
+                    for (int v = 0; v < 4; ++v) {
+                        const float4 x = *reinterpret_cast<const float4 *>(my + c0 + 4 * v);
+                        const float4 y = *reinterpret_cast<const float4 *>(my + kArr + c0 + 4 * v);
+                        const float4 z = *reinterpret_cast<const float4 *>(my + 2 * kArr + c0 + 4 * v);
+                        hv[4 * v] = x.x, hv[4 * v + 1] = x.y, hv[4 * v + 2] = x.z, hv[4 * v + 3] = x.w;
+                        a1[4 * v] = y.x, a1[4 * v + 1] = y.y, a1[4 * v + 2] = y.z, a1[4 * v + 3] = y.w;
+                        a2[4 * v] = z.x, a2[4 * v + 1] = z.y, a2[4 * v + 2] = z.z, a2[4 * v + 3] = z.w;
+                    }
+                    signed char *gp = p.gt8_out + (size_t)(n0 + cbeg + c0) * p.np + i;  // GT8[digit][a][i]: lanes = consecutive i
 #pragma unroll
-                for (int k = 0; k < 16; ++k) {
-                    const long long t = ((long long)s0[k] << 16) + ((long long)s1[k] << 8) + (long long)s2[k];  // exact
-                    const float f = (float)(js * (double)t);  // F_i = sum_j J_ij m_j
-                    const float hk = hv[k];
-                    const float g = (-2.0f * f + hk * sc.inv_beta) * p1mp_of(hk);  // dU/dp = -2 sum_j J_ij m_j
-                    hv[k] = opt_update(hk, g, a1[k], a2[k], sc);
-                    int d0, d1, d2;
-                    i8_digits(i8_fixed_of(mag_of(hv[k])), d0, d1, d2);
-                    const size_t go = (size_t)(n0 + c0 + k) * p.np + i;  // GT8[digit][a][i]: lanes = consecutive i
-                    p.gt8_out[go] = (signed char)d0;
-                    p.gt8_out[plane + go] = (signed char)d1;
-                    p.gt8_out[2 * plane + go] = (signed char)d2;
-                }
+                    for (int k = 0; k < 16; ++k) {
+                        // 2^16 acc0 + 2^8 acc1 + acc2 in fp32: |acc0| <= 2^24 converts exactly, the other two round at 2^-24 of
+                        // themselves, the sums at 2^-24 of the total -- the level of the digits that were dropped
+                        const float t = fmaf((float)s0[k], 65536.0f, fmaf((float)s1[k], 256.0f, (float)s2[k]));
+                        const float f = js * t;  // F_i = sum_j J_ij m_j
+                        const float hk = hv[k];
+                        const float g = (-2.0f * f + hk * sc.inv_beta) * p1mp_of(hk);  // dU/dp = -2 sum_j J_ij m_j
+                        hv[k] = opt_update(hk, g, a1[k], a2[k], sc);
+                        int d0, d1, d2;
+                        i8_digits(i8_fixed_of(mag_of(hv[k])), d0, d1, d2);
+                        gp[0] = (signed char)d0;
+                        gp[plane] = (signed char)d1;
+                        gp[2 * plane] = (signed char)d2;
+                        gp += p.np;
+                    }
 #pragma unroll
-                for (int v = 0; v < 4; ++v) {
-                    __stcs(reinterpret_cast<float4 *>(p.h + rowoff + c0) + v, make_float4(hv[4 * v], hv[4 * v + 1], hv[4 * v + 2], hv[4 * v + 3]));
-                    __stcs(reinterpret_cast<float4 *>(p.m1 + rowoff + c0) + v, make_float4(a1[4 * v], a1[4 * v + 1], a1[4 * v + 2], a1[4 * v + 3]));
-                    __stcs(reinterpret_cast<float4 *>(p.m2 + rowoff + c0) + v, make_float4(a2[4 * v], a2[4 * v + 1], a2[4 * v + 2], a2[4 * v + 3]));
+                    for (int v = 0; v < 4; ++v) {
+                        *reinterpret_cast<float4 *>(my + c0 + 4 * v) = make_float4(hv[4 * v], hv[4 * v + 1], hv[4 * v + 2], hv[4 * v + 3]);
+                        *reinterpret_cast<float4 *>(my + kArr + c0 + 4 * v) = make_float4(a1[4 * v], a1[4 * v + 1], a1[4 * v + 2], a1[4 * v + 3]);
+                        *reinterpret_cast<float4 *>(my + 2 * kArr + c0 + 4 * v) = make_float4(a2[4 * v], a2[4 * v + 1], a2[4 * v + 2], a2[4 * v + 3]);
+                    }
                 }
             }
+            __syncwarp();
+            float *dst[3] = {p.h, p.m1, p.m2};
+#pragma unroll
+            for (int arr = 0; arr < 3; ++arr)
+                for (int x = lane; x < 32 * kChunks; x += 32) {
+                    const int r = x / kChunks, ch = x - r * kChunks;
+                    if (r < rows_ok)
+                        __stcs(reinterpret_cast<float4 *>(dst[arr] + (size_t)(m0 + quad * 32 + r) * p.Rb + n0 + cbeg + ch * 4),
+                               *reinterpret_cast<const float4 *>(stg + arr * kArr + r * kPitch + ch * 4));
+                }
         }
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     }
     __syncthreads();
+    if (CL) i8_cluster_sync();  // no CTA leaves while a peer may still arrive on its barriers
     if (warp == 1) {
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_d), "r"((uint32_t)S::kTmemCols));
@@ -354,12 +451,12 @@ static int i8_tile_n(int Rb, int forced) {  // 0 = not applicable (three accumul
     return 0;
 }
 
-template <int BN>
+template <int BN, bool CL>
 static bool i8_launch(Handle *hd, const I8Params &p, const CUtensorMap *maps) {
     using S = I8Shape<BN>;
-    const void *fn = reinterpret_cast<const void *>(&dense_i8_step_kernel<BN>);
+    const void *fn = reinterpret_cast<const void *>(&dense_i8_step_kernel<BN, CL>);
     if (!hd->attr_done.count(fn)) {
-        if (cudaFuncSetAttribute(dense_i8_step_kernel<BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::kSmem) != cudaSuccess) return false;
+        if (cudaFuncSetAttribute(dense_i8_step_kernel<BN, CL>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::kSmem) != cudaSuccess) return false;
         hd->attr_done.insert(fn);
     }
     cudaLaunchConfig_t cfg = {};
@@ -367,12 +464,19 @@ static bool i8_launch(Handle *hd, const I8Params &p, const CUtensorMap *maps) {
     cfg.blockDim = dim3(I8_THREADS);
     cfg.dynamicSmemBytes = S::kSmem;
     cfg.stream = hd->stream;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, dense_i8_step_kernel<BN>, maps[0], maps[1], maps[2], maps[3], maps[4], maps[5], p) == cudaSuccess;
+    if (CL) {
+        attr[1].id = cudaLaunchAttributeClusterDimension;
+        attr[1].val.clusterDim.x = 2;
+        attr[1].val.clusterDim.y = 2;
+        attr[1].val.clusterDim.z = 1;
+        cfg.numAttrs = 2;
+    }
+    cfg.attrs = attr;
+    return cudaLaunchKernelEx(&cfg, dense_i8_step_kernel<BN, CL>, maps[0], maps[1], maps[2], maps[3], maps[4], maps[5], p) == cudaSuccess;
 }
 
 // One fp32 step of the dense kind on the int8 tensor-core path.  Returns false when the path does not apply (the caller
@@ -381,16 +485,19 @@ bool launch_step_dense_i8(Handle *hd, const StepScalars &sc) {
     const int n = hd->dp.n, Rb = hd->Rb, np = hd->i8_np;
     const int bn = i8_tile_n(Rb, (int)hd->opt_tc_tile_n);
     if (bn == 0 || hd->R != Rb || !hd->J8 || hd->opt_tensor_cores != 1) return false;
+    // 2 x 2 clusters with operand multicast where the grid allows it ("tc_cluster" option: 1 = automatic, 0 = off)
+    const bool cl = hd->opt_tc_cluster != 0 && bn >= 64 && ceil_div(n, I8_BM) % 2 == 0 && (Rb / bn) % 2 == 0;
     CUtensorMap *m = reinterpret_cast<CUtensorMap *>(hd->tc8_maps);
-    if (hd->tc8_maps_R != hd->R || hd->tc8_maps_bn != bn) {  // the maps bake in R (rows of GT8) and the box height bn
+    const int key_bn = cl ? -bn : bn;  // the maps bake in R (rows of GT8) and the box heights (halved with multicast)
+    if (hd->tc8_maps_R != hd->R || hd->tc8_maps_bn != key_bn) {
         bool ok = true;
-        for (int d = 0; d < 3 && ok; ++d) ok = i8_make_map(&m[d], hd->J8 + (size_t)d * n * np, n, n, np, I8_BM);
+        for (int d = 0; d < 3 && ok; ++d) ok = i8_make_map(&m[d], hd->J8 + (size_t)d * n * np, n, n, np, cl ? I8_BM / 2 : I8_BM);
         for (int k = 0; k < 2 && ok; ++k)
             for (int d = 0; d < 3 && ok; ++d)
-                ok = i8_make_map(&m[3 + 3 * k + d], hd->gt8[k] + (size_t)d * hd->R * np, hd->R, n, np, bn);
+                ok = i8_make_map(&m[3 + 3 * k + d], hd->gt8[k] + (size_t)d * hd->R * np, hd->R, n, np, cl ? bn / 2 : bn);
         if (!ok) return false;
         hd->tc8_maps_R = hd->R;
-        hd->tc8_maps_bn = bn;
+        hd->tc8_maps_bn = key_bn;
     }
     if (!hd->tc8_split_done) {
         i8_split_J_kernel<<<(unsigned)n, 256, 0, hd->stream>>>(hd->dp.J, hd->J8, hd->jscale, n, np);
@@ -413,12 +520,13 @@ bool launch_step_dense_i8(Handle *hd, const StepScalars &sc) {
     p.n = n;
     p.np = np;
     p.Rb = Rb;
+    p.debug = (int)hd->opt_tc_debug;
     CUtensorMap maps[6] = {m[0], m[1], m[2], m[3 + 3 * hd->cur], m[4 + 3 * hd->cur], m[5 + 3 * hd->cur]};
     bool ok = false;
     switch (bn) {
-        case 128: ok = i8_launch<128>(hd, p, maps); break;
-        case 64: ok = i8_launch<64>(hd, p, maps); break;
-        default: ok = i8_launch<32>(hd, p, maps); break;
+        case 128: ok = cl ? i8_launch<128, true>(hd, p, maps) : i8_launch<128, false>(hd, p, maps); break;
+        case 64: ok = cl ? i8_launch<64, true>(hd, p, maps) : i8_launch<64, false>(hd, p, maps); break;
+        default: ok = i8_launch<32, false>(hd, p, maps); break;
     }
     if (ok) {
         hd->launches++;

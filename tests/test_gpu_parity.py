@@ -578,3 +578,29 @@ def test_two_handles_with_rank_seeds_match_single_runs(fem):
     e, owner, cfg = multigpu.best_over_ranks(bests[int(np.argmin(bests))], both[int(np.argmin(bests))]["best_config"],
                                              __import__("torch").device("cpu"))
     assert e == min(bests) and np.array_equal(cfg, both[int(np.argmin(bests))]["best_config"])
+
+
+@pytest.mark.parametrize("shape", [(512, 256, 0), (640, 128, 64), (384, 256, 0)])
+def test_dense_int8_cluster_multicast_matches_single_cta(fem, shape):
+    """The int8 digit step in 2 x 2 clusters with operand multicast (tc_cluster = 1, taken when the grid has an even number
+    of row and column tiles) against the same step without clusters: integer accumulation is exact, so the two agree bit
+    for bit; and against the oracle on a replica subset.  (384, 256): three row tiles -> no clusters either way."""
+    n, R, tile = shape
+    inst = wl.sk_dense(n, 2012)
+    beta = fem.linear_temperature_schedule(1.0, 0.01, 500)
+    h0 = fo.init_fields(6, R, inst.n, 1).astype(np.float32)
+    pb, st = oracle_run(inst, h0[:16], beta, 30, inst.lam)
+    P_ref = fo.marginals(pb, st.h).reshape(16, inst.n)
+    out = []
+    for cl in (1, 0):
+        eng = fem.Fem(inst, R)
+        eng.set_option("tc_cluster", cl)
+        if tile:
+            eng.set_option("tc_tile_n", tile)
+        eng.set_fields(h0)
+        eng.anneal(fem.Schedule(beta=beta, precise_steps=8), R, stop_after=30)
+        out.append((eng.get_fields(), eng.get_marginals().astype(np.float64)))
+        assert eng.info("tc8_launches") == 22
+        eng.close()
+    assert np.array_equal(out[0][0], out[1][0])
+    assert np.max(np.abs(out[0][1][:16] - P_ref)) < MARGINAL_TOL
