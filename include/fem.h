@@ -187,7 +187,9 @@ fem_status fem_energy_of(fem_handle *h, const int32_t *cfg /* [count][n] */, int
  * Results do not depend on either (replicas are independent).  Dense ISING only: "tensor_cores"
  * (1 = the default: the int8 digit step on tcgen05 (kind::i8, k_dense_i8.cu) where it applies -- R a multiple of 32, plain
  * Adam on the exact gradient --, else the 3xTF32 step; 2 = the 3xTF32 step (kind::tf32; n % 4 == 0); 0 = CUDA-core GEMM)
- * and "tc_tile_n" (replica columns per tensor-core tile: 0 = default, 32/64/128, and 256 for the 3xTF32 step only).
+ * and "tc_tile_n" (replica columns per tensor-core tile: 0 = default, 32/64/128, and 256 for the 3xTF32 step only),
+ * "tc_cluster" (int8 step: 1 = 2 x 2 thread-block clusters with operand multicast where the tile grid is even in both
+ * directions, the default; 0 = off; bit-identical either way).
  * "persistent" (small sparse MAXCUT / ISING / MAXSAT problems with few enough replicas to run in at most three
  * waves of clusters: 1 = replica-persistent cluster kernel where the problem fits, the default; 0 = one launch per step; 1 + CS = force clusters of CS = 1, 2, 4 or 8 CTAs per replica) and
  * "long_rows" (two-state graph kinds: 1 = rows with many entries are summed by a CTA each in a fixed order, the default;

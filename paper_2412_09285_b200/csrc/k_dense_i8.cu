@@ -26,7 +26,7 @@ namespace fem {
 constexpr int I8_BM = 128;       // rows of F per CTA = TMEM lanes
 constexpr int I8_BK = 128;       // int8 elements per k-block = one 128-byte swizzle atom
 constexpr int I8_UMMA_K = 32;    // int8 elements per tcgen05.mma
-constexpr int I8_EPI_GROUPS = 2;  // epilogue warps per TMEM lane quadrant (each takes BN / groups columns)
+constexpr int I8_EPI_GROUPS = 4;  // epilogue warps per TMEM lane quadrant (each takes BN / groups columns)
 constexpr int I8_THREADS = 64 + 128 * I8_EPI_GROUPS;
 constexpr int I8_FRAC_BITS = 22; // fixed point: |x| <= 2^22 - 1, digits d0 in [-64, 64], d1, d2 in [-128, 127]
 
@@ -34,7 +34,7 @@ template <int BN>
 struct I8Shape {
     static constexpr int kStageBytes = 3 * I8_BM * 128 + 3 * BN * 128;  // three digits of A and of B
     static constexpr int kStages = BN >= 128 ? 2 : 3;
-    static constexpr int kColsWarp = BN / I8_EPI_GROUPS >= 16 ? BN / I8_EPI_GROUPS : 16;
+    static constexpr int kColsWarp = BN / I8_EPI_GROUPS >= 8 ? BN / I8_EPI_GROUPS : 8;
     static constexpr int kEpiBytes = 4 * I8_EPI_GROUPS * 3 * 32 * (kColsWarp + 4) * 4;  // epilogue staging (reuses the stages)
     static constexpr int kSmem = (kStages * kStageBytes > kEpiBytes ? kStages * kStageBytes : kEpiBytes) + 1024;
     static constexpr int kTmemCols = 3 * BN <= 128 ? 128 : (3 * BN <= 256 ? 256 : 512);
@@ -46,7 +46,6 @@ struct I8Params {
     const double *jscale;      // [n] sJ_i / 2^6: F = jscale_i * (2^16 acc0 + 2^8 acc1 + acc2)
     Sc<float> sc;
     int n, np, Rb;
-    int debug;  // TEMPORARY
 };
 
 // ---- PTX wrappers (as in k_dense_tc.cu) ----
@@ -123,6 +122,13 @@ __device__ __forceinline__ void i8_tmem_ld16(uint32_t taddr, int *v) {
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
 
+__device__ __forceinline__ void i8_tmem_ld8(uint32_t taddr, int *v) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+                 : "r"(taddr));
+}
+__device__ __forceinline__ void i8_tmem_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
 // x in [-(2^22 - 1), 2^22 - 1] -> three balanced digits, x = d0 2^16 + d1 2^8 + d2
 __host__ __device__ __forceinline__ void i8_digits(int x, int &d0, int &d1, int &d2) {
     d2 = ((x + 128) & 255) - 128;
@@ -136,7 +142,7 @@ __device__ __forceinline__ int i8_fixed_of(float m) {  // |m| <= 1
 }
 
 // ---- the fused step ----
-// Warp roles: warp 0 = TMA producer (one elected lane), warp 1 = TMEM allocator + MMA issuer (one elected lane), warps 2..9 =
+// Warp roles: warp 0 = TMA producer (one elected lane), warp 1 = TMEM allocator + MMA issuer (one elected lane), warps 2..17 =
 // epilogue (warp w reads TMEM lanes 32*(w%4) .. +31; the two warps of a lane quadrant split the BN columns).  With one warp per
 // scheduler the epilogue was bound by its own dependency chains and by DRAM round trips (2 x 44 us of a 147 us step): two warps
 // per scheduler, and the h / m1 / m2 rows of a 16-column block are requested one block ahead (the first before the main loop ends).
@@ -159,7 +165,7 @@ dense_i8_step_kernel(const __grid_constant__ CUtensorMap tmJ0, const __grid_cons
     uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int m0 = blockIdx.x * I8_BM, n0 = blockIdx.y * BN;
-    const int nkb = (p.debug & 2) ? 1 : (p.n + I8_BK - 1) / I8_BK;
+    const int nkb = (p.n + I8_BK - 1) / I8_BK;
     uint32_t cx = 0, cy = 0;  // position inside the 2 x 2 cluster (rank = cx + 2 cy)
     if (CL) {
         asm volatile("mov.u32 %0, %%cluster_ctaid.x;" : "=r"(cx));
@@ -263,7 +269,7 @@ dense_i8_step_kernel(const __grid_constant__ CUtensorMap tmJ0, const __grid_cons
         const int i = m0 + quad * 32 + lane;
         const bool row_ok = i < p.n;
         const Sc<float> &sc = p.sc;
-        constexpr int kCols = BN / I8_EPI_GROUPS >= 16 ? BN / I8_EPI_GROUPS : 16;  // columns of this warp
+        constexpr int kCols = BN / I8_EPI_GROUPS >= 8 ? BN / I8_EPI_GROUPS : 8;  // columns of this warp
         const int cbeg = ((warp - 2) >> 2) * kCols;
         const bool has_cols = cbeg < BN;
         const float js = row_ok ? (float)p.jscale[i] : 0.0f;
@@ -280,7 +286,7 @@ dense_i8_step_kernel(const __grid_constant__ CUtensorMap tmJ0, const __grid_cons
         constexpr int kChunks = kCols / 4;                   // 16-byte pieces per row
         i8_mbar_wait(&tmem_full_bar, 0);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        if (has_cols && !(p.debug & 1)) {
+        if (has_cols) {
             const int rows_ok = min(32, p.n - (m0 + quad * 32));  // rows of this warp inside the matrix (<= 0: none)
             const float *src[3] = {p.h, p.m1, p.m2};
 #pragma unroll
@@ -298,16 +304,17 @@ dense_i8_step_kernel(const __grid_constant__ CUtensorMap tmJ0, const __grid_cons
             __syncwarp();
             float *my = stg + lane * kPitch;
 #pragma unroll 1
-            for (int c0 = 0; c0 < kCols; c0 += 16) {
-                int s0[16], s1[16], s2[16];
+            for (int c0 = 0; c0 < kCols; c0 += 8) {  // 8 columns at a time: few live registers, four warps per scheduler
+                int s0[8], s1[8], s2[8];
                 const uint32_t lane_base = tmem_d + ((uint32_t)(quad * 32) << 16) + (uint32_t)(cbeg + c0);
-                i8_tmem_ld16(lane_base, s0);  // warp-collective: no divergence here
-                i8_tmem_ld16(lane_base + (uint32_t)BN, s1);
-                i8_tmem_ld16(lane_base + (uint32_t)(2 * BN), s2);
+                i8_tmem_ld8(lane_base, s0);  // warp-collective: no divergence here
+                i8_tmem_ld8(lane_base + (uint32_t)BN, s1);
+                i8_tmem_ld8(lane_base + (uint32_t)(2 * BN), s2);
+                i8_tmem_wait();
                 if (row_ok) {
-                    float hv[16], a1[16], a2[16];
+                    float hv[8], a1[8], a2[8];
 #pragma unroll
-                    for (int v = 0; v < 4; ++v) {
+                    for (int v = 0; v < 2; ++v) {
                         const float4 x = *reinterpret_cast<const float4 *>(my + c0 + 4 * v);
                         const float4 y = *reinterpret_cast<const float4 *>(my + kArr + c0 + 4 * v);
                         const float4 z = *reinterpret_cast<const float4 *>(my + 2 * kArr + c0 + 4 * v);
@@ -317,7 +324,7 @@ dense_i8_step_kernel(const __grid_constant__ CUtensorMap tmJ0, const __grid_cons
                     }
                     signed char *gp = p.gt8_out + (size_t)(n0 + cbeg + c0) * p.np + i;  // GT8[digit][a][i]: lanes = consecutive i
 #pragma unroll
-                    for (int k = 0; k < 16; ++k) {
+                    for (int k = 0; k < 8; ++k) {
                         // 2^16 acc0 + 2^8 acc1 + acc2 in fp32: |acc0| <= 2^24 converts exactly, the other two round at 2^-24 of
                         // themselves, the sums at 2^-24 of the total -- the level of the digits that were dropped
                         const float t = fmaf((float)s0[k], 65536.0f, fmaf((float)s1[k], 256.0f, (float)s2[k]));
@@ -333,7 +340,7 @@ dense_i8_step_kernel(const __grid_constant__ CUtensorMap tmJ0, const __grid_cons
                         gp += p.np;
                     }
 #pragma unroll
-                    for (int v = 0; v < 4; ++v) {
+                    for (int v = 0; v < 2; ++v) {
                         *reinterpret_cast<float4 *>(my + c0 + 4 * v) = make_float4(hv[4 * v], hv[4 * v + 1], hv[4 * v + 2], hv[4 * v + 3]);
                         *reinterpret_cast<float4 *>(my + kArr + c0 + 4 * v) = make_float4(a1[4 * v], a1[4 * v + 1], a1[4 * v + 2], a1[4 * v + 3]);
                         *reinterpret_cast<float4 *>(my + 2 * kArr + c0 + 4 * v) = make_float4(a2[4 * v], a2[4 * v + 1], a2[4 * v + 2], a2[4 * v + 3]);
@@ -520,7 +527,6 @@ bool launch_step_dense_i8(Handle *hd, const StepScalars &sc) {
     p.n = n;
     p.np = np;
     p.Rb = Rb;
-    p.debug = (int)hd->opt_tc_debug;
     CUtensorMap maps[6] = {m[0], m[1], m[2], m[3 + 3 * hd->cur], m[4 + 3 * hd->cur], m[5 + 3 * hd->cur]};
     bool ok = false;
     switch (bn) {
