@@ -363,6 +363,10 @@ def run_workload(args, name, steps, warmup, ctx, with_e2e=True):
                     "peak_source": "L2 -> SM read bandwidth measured in this run (fem_probe_l2_read: 32 MiB resident buffer, 16-byte loads bypassing L1)",
                     "algorithmic_l2_bytes_per_launch": per_launch, "kernel_us": kernel_us, "kernel_share_of_step": share,
                     "hbm_frac_of_compulsory_bytes": step_bytes / (kernel_us * 1e-6) / 1e9 / peak,
+                    "l2_gather_probe_gbs": {"32MiB": fem.probe_l2_gather(f"cuda:{local_rank}", 32, int(min(512, max(64, 4 * R)))),
+                                            "row_bytes": int(min(512, max(64, 4 * R))),
+                                            "what": "random-row reads of the same row length out of a 32 MiB working set (fem_probe_l2_gather): the "
+                                                    "rate of the step's own access pattern; `peak` above is the sequential-read figure"},
                     "note": "state is L2-resident: the binding roof is L2 -> SM gather bandwidth, not HBM (DESIGN.md section 6); "
                             "rows gathered more than once by an SM can be served by its L1, so `achieved` (algorithmic gather bytes) is an upper bound on the L2 traffic"}
     else:

@@ -181,8 +181,11 @@ class Fem:
             raise FemError(FEM_EINVAL, "fem_workspace_bytes rejected the problem")
         self.workspace_bytes = int(nbytes)
         with torch.cuda.device(self.device):
-            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
-            base = self._ws.data_ptr()
+            # (guard bytes on both sides of the workspace, filled with a pattern: tests check that the library never writes
+            # outside the bytes it asked for)
+            self._guard = 1 << 16
+            self._ws = torch.full((nbytes + 256 + 2 * self._guard,), 0xA5, dtype=torch.uint8, device=self.device)
+            base = self._ws.data_ptr() + self._guard
             self._ws_ptr = (base + 255) & ~255
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             h = C.c_void_p()
@@ -192,6 +195,12 @@ class Fem:
             raise FemError(st, (self._lib.fem_last_error(None) or b"").decode())
         self._h = h
         self.R = 0
+
+    def guards_intact(self) -> bool:
+        """True when no byte outside the workspace handed to fem_create has been written (64 KiB checked on each side)."""
+        lo = self._ws_ptr - self._ws.data_ptr()
+        hi = lo + self.workspace_bytes
+        return bool((self._ws[:lo] == 0xA5).all().item()) and bool((self._ws[hi:] == 0xA5).all().item())
 
     # -- plumbing
     def _check(self, st: int):

@@ -159,3 +159,30 @@ def test_invalid_problems_are_rejected(fem):
                                lits=np.array([2, -2], np.int32))
         with pytest.raises(fem.FemError):
             fem.Fem(inst, 4)
+
+
+def test_no_kernel_writes_outside_the_workspace(fem):
+    """Every kind through its default kernels (Potts state-innermost and register paths, long rows, persistent clusters, Max-SAT,
+    non-Boolean SAT, dense int8 and 3xTF32, node weights), wide phase, hooks and readout: the guard bytes around the caller's
+    workspace stay untouched (compute-sanitizer is not available on this pool)."""
+    rng = np.random.default_rng(3)
+    b8 = wl.random_regular(1200, 10, 2031, wl.BMINCUT, 8, lam=0.02)
+    V = rng.integers(1, 5, b8.n).astype(np.float32)
+    runs = [
+        (b8, 16, {"replica_block": 8}), (wl.Instance(wl.BMINCUT, b8.n, 8, b8.row_ptr, b8.col_idx, None, lam=0.02, node_weight=V), 16, {}),
+        (wl.random_regular(1201, 6, 2032, wl.BMINCUT, 5, lam=0.03), 12, {}),
+        (wl.preferential_attachment(3000, 3, 31, pm1=True), 12, {}), (wl.erdos_renyi_maxcut(800, 0.06, 1000), 32, {}),
+        (wl.torus_maxcut(30, 5, W=34), 64, {"replica_block": 16}), (wl.random_ksat(500, 4000, 4, 7), 16, {}),
+        (wl.random_qsat(150, 900, 3, 3, 2103), 8, {}), (wl.sk_dense(512, 2012), 256, {}), (wl.sk_dense(328, 2011), 96, {"tensor_cores": 2}),
+    ]
+    for inst, R, opts in runs:
+        eng = fem.Fem(inst, R + 4)
+        for k, v in opts.items():
+            eng.set_option(k, v)
+        sch = fem.Schedule(beta=fem.linear_temperature_schedule(1.0, 0.05, 40), precise_steps=4)
+        eng.anneal(sch, R, seed=1, stop_after=17)
+        eng.get_marginals(); eng.get_moments()
+        eng.anneal(sch, R, seed=1)
+        eng.result(); eng.get_configs()
+        assert eng.guards_intact(), inst.name
+        eng.close()
