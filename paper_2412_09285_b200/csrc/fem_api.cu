@@ -28,7 +28,7 @@ cudaError_t persist_run(Handle *hd, bool wide, int t_begin, int t_end, StepScala
 static std::string g_create_error;
 
 struct Layout {
-    size_t row_ptr, col, w, rowsum, long_rows, vw, lit_state, J, Jlo, glo0, glo1, J8, gt8_0, gt8_1, jscale, field, occ_ptr, occ, clause_ptr, lits;
+    size_t row_ptr, col, w, rowsum, long_rows, vw, lit_state, order, J, Jlo, glo0, glo1, J8, gt8_0, gt8_1, jscale, field, occ_ptr, occ, clause_ptr, lits;
     size_t h, m1, m2, g0, g1, stage, hW, m1W, m2W, gW0, gW1, colsum0, colsum1, colsum2, cfg, e_part_i, e_part_d, part_part, e_int, e_real, part,
         best, total;
 };
@@ -117,6 +117,7 @@ static Layout make_layout(const fem_problem *pb, const ProblemShape &s, int R_ca
     L.rowsum = take(s.nnz > 0 || pb->row_ptr ? (size_t)pb->n * 8 : 0);
     L.long_rows = take((size_t)s.n_long * 4);
     L.vw = take(pb->node_weight ? (size_t)pb->n * 4 : 0);
+    L.order = take(pb->kind != FEM_BMINCUT && pb->row_ptr ? (size_t)pb->n * 4 : 0);
     L.J = take(s.dense ? (size_t)pb->n * pb->n * 4 : 0);
     L.Jlo = take(s.dense ? (size_t)pb->n * pb->n * 4 : 0);
     L.glo0 = take(s.dense ? state : 0);
@@ -480,6 +481,18 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
             dp.long_rows = reinterpret_cast<int *>(at(L.long_rows));
             dp.n_long = (int)h_long.size();
             if (ok) ok = cuda_ok(hd, cudaStreamSynchronize(hd->stream), "upload long rows");  // h_long is a local
+        }
+        if (pb->kind != FEM_BMINCUT && dp.uniform_deg == 0 && pb->n > 1) {
+            // degree-sorted processing order of the stepwise kernel (counting sort, ascending, stable): a warp's variables
+            // then have rows of nearly the same length, so its batched gather loop does no idle iterations on a
+            // degree-skewed graph.  Which thread takes which variable changes no arithmetic.
+            std::vector<int> cnt((size_t)dp.max_deg + 2, 0), ord((size_t)pb->n);
+            for (int i = 0; i < pb->n; ++i) cnt[(size_t)(pb->row_ptr[i + 1] - pb->row_ptr[i]) + 1]++;
+            for (size_t d = 1; d < cnt.size(); ++d) cnt[d] += cnt[d - 1];
+            for (int i = 0; i < pb->n; ++i) ord[(size_t)cnt[(size_t)(pb->row_ptr[i + 1] - pb->row_ptr[i])]++] = i;
+            up(at(L.order), ord.data(), ord.size() * 4, "upload order");
+            dp.order = reinterpret_cast<int *>(at(L.order));
+            if (ok) ok = cuda_ok(hd, cudaStreamSynchronize(hd->stream), "upload order");  // ord is a local
         }
         if (pb->kind != FEM_BMINCUT) persist_prepare(hd, pb->row_ptr);
         dp.vtotal = (double)pb->n;

@@ -55,6 +55,9 @@ struct DevProblem {
     int64_t nnz;
     const float *vw;       // BMINCUT: node weights V_i of the balance term (S33-S35), or nullptr (= all 1)
     double vtotal;         // sum_i V_i (= n without node weights)
+    const int *order;      // [n] two-state graph kinds with rows of different lengths: the variables sorted by degree (ascending), the
+                           // order in which the stepwise kernel's threads take them, so that the variables of a warp have rows of
+                           // (nearly) the same length; nullptr = index order
     const int *long_rows;  // [n_long] variables whose row has more than kLongRow entries (two-state graph kinds), ascending
     int n_long;
     const float *J;  // dense Ising, n*n

@@ -57,6 +57,9 @@ __global__ void __launch_bounds__(kThreads, GH ? 8 : 1) step_q2_kernel(const Q2P
     if (!long_cta && idx >= p.total) return;
     unsigned i = p.rv_shift >= 0 ? idx >> p.rv_shift : idx / p.rv;
     unsigned c = (idx - i * p.rv) * VEC;
+    if constexpr (LONG) {  // rows of different lengths: threads take the variables in degree-sorted order (fem_create)
+        if (!long_cta && p.dp.order) i = (unsigned)__ldg(p.dp.order + i);
+    }
     unsigned lane0 = 0, lanes = 1;  // long-row CTA: the lanes of the replica block it serves
     if constexpr (LONG) {
         if (long_cta) {
