@@ -431,18 +431,22 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
         }
     } else if (s.dense) {
         const int n = pb->n;
-        for (int i = 0; i < n; ++i) {
+        for (int i = 0; i < n; ++i)
             if (pb->dense_J[(size_t)i * n + i] != 0.f) {
                 delete hd;
                 return fail(nullptr, FEM_EINVAL, "dense_J must have a zero diagonal");
             }
-            for (int j = i + 1; j < n; ++j)
-                if (pb->dense_J[(size_t)i * n + j] != pb->dense_J[(size_t)j * n + i] ||
-                    !std::isfinite(pb->dense_J[(size_t)i * n + j])) {
-                    delete hd;
-                    return fail(nullptr, FEM_EINVAL, "dense_J must be symmetric and finite");
-                }
-        }
+        // symmetry and finiteness in 64 x 64 blocks (the transposed element of a block stays in cache: 16.7 M elements at
+        // cfg 4b took 60 ms row by column, inside every end-to-end pass)
+        constexpr int kBlk = 64;
+        for (int i0 = 0; i0 < n; i0 += kBlk)
+            for (int j0 = i0; j0 < n; j0 += kBlk)
+                for (int i = i0; i < std::min(n, i0 + kBlk); ++i)
+                    for (int j = std::max(j0, i + 1); j < std::min(n, j0 + kBlk); ++j)
+                        if (pb->dense_J[(size_t)i * n + j] != pb->dense_J[(size_t)j * n + i] || !std::isfinite(pb->dense_J[(size_t)i * n + j])) {
+                            delete hd;
+                            return fail(nullptr, FEM_EINVAL, "dense_J must be symmetric and finite");
+                        }
         up(at(L.J), pb->dense_J, (size_t)n * n * 4, "upload J");
         dp.J = reinterpret_cast<float *>(at(L.J));
         hd->field = reinterpret_cast<float *>(at(L.field));
