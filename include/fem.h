@@ -196,9 +196,11 @@ fem_status fem_energy_of(fem_handle *h, const int32_t *cfg /* [count][n] */, int
  * 0 = one thread per row as for short rows -- this one does change the summation order of those rows),
  * "potts_si" (BMINCUT, q = 4 or 8, replica blocks of 4 / 8 / 16 / 32 with n a multiple of 32 / block: 1 = fp32 steps on
  * state-innermost replica blocks, k_step_potts_si.cu, the default; 0 = off),
- * "potts_tma" (BMINCUT: 1 = rows staged by bulk asynchronous copies where the shape allows, the default; 0 =
- * register path) and "potts_lane" (BMINCUT, q <= 8, replica blocks of 8 / 16 / 32: 1 = the lane-per-replica kernel, k_step_potts_lane.cu;
- * 0 = the default).  None of them changes a single bit of the results.  Unknown key: FEM_EINVAL. */
+ * "potts_tma" (BMINCUT shapes the state-innermost kernel does not take, or with "potts_si" = 0: 1 = rows staged by bulk
+ * asynchronous copies where the shape allows, the default; 0 = register path) and "potts_lane" (BMINCUT, q <= 8, replica
+ * blocks of 8 / 16 / 32: 1 = the lane-per-replica kernel, k_step_potts_lane.cu; 0 = the default).  Apart from "long_rows" and
+ * the three "tensor_cores" modes (different roundings of the dense product) none of them changes a single bit of the
+ * results.  Unknown key: FEM_EINVAL. */
 fem_status fem_set_option(fem_handle *h, const char *key, int64_t value);
 /* Introspection for benchmarks: "launches" (kernels enqueued so far), "tc_launches" (of which tcgen05
  * dense steps; "tc8_launches": of those, int8 digit steps), "persist_launches", "persist_cluster" (CTAs per replica of the persistent kernel),
