@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstring>
 #include <new>
+#include <thread>
 
 #include "fem_internal.cuh"
 
@@ -194,18 +195,38 @@ static bool validate_graph(const fem_problem *pb, int64_t nnz, bool *integral, i
             if (w != std::nearbyint(w) || std::fabs(w) > 1e6f) *integral = false;
         }
     }
-    // symmetry in O(nnz): sweeping the rows i in ascending order, the entries (j, i) of any row j come up in ascending i,
-    // i.e. in the order row j stores them (columns are strictly ascending), so one cursor per row suffices
+    // symmetry: every entry (i, j) has its mirror (j, i) with the same weight -- a binary search in row j (columns are strictly
+    // ascending), rows shared out over the host threads (the one-cursor-per-row sweep it replaces took 42 ms at cfg 4a,
+    // inside every end-to-end pass)
     {
-        std::vector<int64_t> cursor(pb->row_ptr, pb->row_ptr + n);
-        for (int i = 0; i < n; ++i)
-            for (int64_t e = pb->row_ptr[i]; e < pb->row_ptr[i + 1]; ++e) {
-                const int j = pb->col_idx[e];
-                const int64_t c = cursor[j];
-                if (c >= pb->row_ptr[j + 1] || pb->col_idx[c] != i) return *err = "CSR is not symmetric", false;
-                if (pb->weight && pb->weight[c] != pb->weight[e]) return *err = "weights are not symmetric", false;
-                cursor[j] = c + 1;
-            }
+        const unsigned hw = std::max(1u, std::min(16u, std::thread::hardware_concurrency()));
+        const unsigned nt = n < 4096 ? 1u : hw;
+        std::vector<int> bad(nt, 0);  // 0 ok, 1 not symmetric, 2 weights not symmetric
+        auto work = [&](unsigned t) {
+            const int a = (int)((int64_t)n * t / nt), b = (int)((int64_t)n * (t + 1) / nt);
+            for (int i = a; i < b && !bad[t]; ++i)
+                for (int64_t e = pb->row_ptr[i]; e < pb->row_ptr[i + 1]; ++e) {
+                    const int j = pb->col_idx[e];
+                    const int32_t *lo = pb->col_idx + pb->row_ptr[j], *hi = pb->col_idx + pb->row_ptr[j + 1];
+                    const int32_t *it = std::lower_bound(lo, hi, i);
+                    if (it == hi || *it != i) {
+                        bad[t] = 1;
+                        break;
+                    }
+                    if (pb->weight && pb->weight[it - pb->col_idx] != pb->weight[e]) {
+                        bad[t] = 2;
+                        break;
+                    }
+                }
+        };
+        std::vector<std::thread> pool;
+        for (unsigned t = 1; t < nt; ++t) pool.emplace_back(work, t);
+        work(0);
+        for (auto &th : pool) th.join();
+        for (unsigned t = 0; t < nt; ++t) {
+            if (bad[t] == 1) return *err = "CSR is not symmetric", false;
+            if (bad[t] == 2) return *err = "weights are not symmetric", false;
+        }
     }
     *uniform_deg = (uniform && d0 > 0 && d0 <= 64) ? (int)d0 : 0;
     int64_t mx = 0;
