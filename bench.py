@@ -267,7 +267,7 @@ def run_workload(args, name, steps, warmup, ctx, with_e2e=True):
     readout_ms = sum(e[1].elapsed_time(e[4]) for e in bulk_events) / max(len(bulk_events), 1)
     # algorithmic bytes of one launch: the whole step's bytes spread over the launches that make up a step
     step_bytes = eng.info("step_bytes") * (N - K) * steps / max(bulk_launches, 1)
-    info = {k: eng.info(k) for k in ("tc_launches", "tc8_launches", "persist_launches", "tma_launches", "lane_launches", "si_launches", "replica_block", "nnz")}
+    info = {k: eng.info(k) for k in ("tc_launches", "tc8_launches", "persist_launches", "tma_launches", "si_launches", "replica_block", "nnz")}
     eng.close()
 
     # ---- e2e through the public API from host buffers (pinned), host<->device copies inside the timed region
@@ -373,8 +373,6 @@ def run_workload(args, name, steps, warmup, ctx, with_e2e=True):
         achieved = step_bytes / (kernel_us * 1e-6) / 1e9
         kname = (("potts_si_kernel (state-innermost replica blocks: a lane owns the q states of a (variable, replica) cell; fused "
                   "softmax + gather + balance + chain rule + optimiser)" if info["si_launches"] > 0 else
-                  "potts_lane_kernel (a lane owns a replica; fused softmax + gather + balance + chain rule + optimiser)"
-                  if info["lane_launches"] > 0 else
                   "potts_tma_kernel (rows staged by cp.async.bulk one variable ahead; fused softmax + gather + balance + "
                   "chain rule + optimiser)" if info["tma_launches"] > 0 else
                   "potts_team_kernel<float> (fused softmax + gather + balance + chain rule + optimiser)")

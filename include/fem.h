@@ -197,14 +197,13 @@ fem_status fem_energy_of(fem_handle *h, const int32_t *cfg /* [count][n] */, int
  * "potts_si" (BMINCUT, q = 4 or 8, replica blocks of 4 / 8 / 16 / 32 with n a multiple of 32 / block: 1 = fp32 steps on
  * state-innermost replica blocks, k_step_potts_si.cu, the default; 0 = off),
  * "potts_tma" (BMINCUT shapes the state-innermost kernel does not take, or with "potts_si" = 0: 1 = rows staged by bulk
- * asynchronous copies where the shape allows, the default; 0 = register path) and "potts_lane" (BMINCUT, q <= 8, replica
- * blocks of 8 / 16 / 32: 1 = the lane-per-replica kernel, k_step_potts_lane.cu; 0 = the default).  Apart from "long_rows" and
+ * asynchronous copies where the shape allows, the default; 0 = register path).  Apart from "long_rows" and
  * the three "tensor_cores" modes (different roundings of the dense product) none of them changes a single bit of the
  * results.  Unknown key: FEM_EINVAL. */
 fem_status fem_set_option(fem_handle *h, const char *key, int64_t value);
 /* Introspection for benchmarks: "launches" (kernels enqueued so far), "tc_launches" (of which tcgen05
  * dense steps; "tc8_launches": of those, int8 digit steps), "persist_launches", "persist_cluster" (CTAs per replica of the persistent kernel),
- * "tma_launches" (TMA-staged Potts steps), "lane_launches" (lane-per-replica Potts steps), "si_launches" (state-innermost Potts steps), "t_done", "R", "replica_block", "nnz", "uniform_degree",
+ * "tma_launches" (TMA-staged Potts steps), "si_launches" (state-innermost Potts steps), "t_done", "R", "replica_block", "nnz", "uniform_degree",
  * "max_degree", "long_rows" (rows of a two-state graph kind with more than 96 entries, or more than 32 and four times the mean degree:
  * the stepwise kernel gives each
  * a CTA of its own), "integral_weights", "step_bytes" (algorithmic HBM bytes of one fused step of the last schedule's optimiser,

@@ -630,9 +630,6 @@ fem_status fem_set_option(fem_handle *h, const char *key, int64_t value) {
     } else if (!strcmp(key, "gather_fields")) {
         if (value < -1 || value > 1) return fail(hd, FEM_EINVAL, "gather_fields must be -1, 0 or 1");
         hd->opt_gather_fields = value;
-    } else if (!strcmp(key, "potts_lane")) {
-        if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "potts_lane must be 0 or 1");
-        hd->opt_potts_lane = value;
     } else if (!strcmp(key, "tc_debug")) {
         hd->opt_tc_debug = value;
     } else if (!strcmp(key, "tc_cluster")) {
@@ -662,7 +659,6 @@ int64_t fem_get_info(const fem_handle *h, const char *key) {
     if (!strcmp(key, "persist_launches")) return hd->persist_launches;
     if (!strcmp(key, "persist_cluster")) return hd->persist_cluster;
     if (!strcmp(key, "tma_launches")) return hd->tma_launches;
-    if (!strcmp(key, "lane_launches")) return hd->lane_launches;
     if (!strcmp(key, "si_launches")) return hd->si_launches;
     if (!strcmp(key, "gather_fields")) return hd->gather_h || hd->gather_h_want ? 1 : 0;
     if (!strcmp(key, "t_done")) return hd->t_done;

@@ -154,9 +154,6 @@ struct Handle {
     int64_t persist_launches = 0, persist_cluster = 0;
     int64_t opt_potts_tma = 1;    // Potts step with TMA-staged rows (k_step_potts_tma.cu) where it applies
     int64_t tma_launches = 0;
-    int64_t opt_potts_lane = 0;   // Potts step with a lane per replica (k_step_potts_lane.cu): measured slower than the
-                                  // TMA-staged team kernel on cfg 2, so off unless asked for
-    int64_t lane_launches = 0;
     // Potts step on state-innermost replica blocks (k_step_potts_si.cu): q = 4 / 8, blocks of 4 / 8 / 16 / 32.  The fp32
     // arrays are re-laid out in place for the fp32 steps of one fem_anneal call (si_live) and back before it returns.
     int64_t opt_long_rows = 1;   // 0: long rows stay with one thread per VEC replicas (measurements only)

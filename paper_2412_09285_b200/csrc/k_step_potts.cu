@@ -335,7 +335,6 @@ static void launch_potts_v(Handle *hd, const PottsParams<T> &p, dim3 grid, bool 
 }
 
 bool launch_potts_tma(Handle *hd, const StepScalars &sc, int blk_begin, int blk_count);  // k_step_potts_tma.cu
-bool launch_potts_lane(Handle *hd, const StepScalars &sc, int blk_begin, int blk_count);  // k_step_potts_lane.cu
 bool launch_potts_si(Handle *hd, const StepScalars &sc, int blk_begin, int blk_count);    // k_step_potts_si.cu
 
 int potts_qpad(int q) {
@@ -404,7 +403,6 @@ void launch_potts(Handle *hd, const StepScalars &sc, bool wide, bool step, int b
         (void)launch_potts_si(hd, sc, blk_begin, blk_count);  // a failed launch surfaces through cudaGetLastError
         return;
     }
-    if (!wide && step && launch_potts_lane(hd, sc, blk_begin, blk_count)) return;  // lane-per-replica fast path (q <= 8)
     if (!wide && step && launch_potts_tma(hd, sc, blk_begin, blk_count)) return;  // TMA-staged fast path where it applies
     if (wide) launch_potts_typed<double>(hd, sc, step, blk_begin, blk_count);
     else launch_potts_typed<float>(hd, sc, step, blk_begin, blk_count);

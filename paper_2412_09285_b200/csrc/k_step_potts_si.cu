@@ -3,7 +3,7 @@
 //
 // Why (profiles/r02_cfg2_step.md).  The team kernels spread the q states of a variable over lanes: every sum over
 // states is a butterfly of shuffles and every lane repeats the scalar work of its 4 fields (634 warp instructions per
-// 128 fields, issue-bound at 0.47 of the HBM roof on cfg 2).  The lane-per-replica kernel (k_step_potts_lane.cu) does
+// 128 fields, issue-bound at 0.47 of the HBM roof on cfg 2).  A lane-per-replica kernel (round 2, first half; removed: profiles/r02_cfg2_step.md) does
 // the arithmetic with a lane owning all q states of one (variable, replica) cell, but keeps the [state][replica] rows in
 // HBM, so every row passes through shared memory twice (22% of its instructions are LDS / STS and it stalls on them:
 // 9.1 ns per kilo-field against 7.4).  Here the LAYOUT follows the arithmetic instead.  For the fp32 steps of one

@@ -376,7 +376,6 @@ def test_potts_tma_bit_identical_to_team_kernel(fem, case, manipulated):
     out = {}
     for tma in (1, 0):
         eng = fem.Fem(inst, R)
-        eng.set_option("potts_lane", 0)              # (the lane-per-replica kernel would take the q <= 8 exact cases)
         eng.set_option("potts_si", 0)                # (and the state-innermost kernel the q = 4 / 8 ones)
         eng.set_option("potts_tma", tma)
         if rb:
@@ -389,104 +388,6 @@ def test_potts_tma_bit_identical_to_team_kernel(fem, case, manipulated):
     assert np.array_equal(out[1][0], out[0][0])
     assert np.array_equal(out[1][1][0], out[0][1][0]) and np.array_equal(out[1][1][1], out[0][1][1])
     assert np.array_equal(out[1][2]["energy"], out[0][2]["energy"])
-
-
-LANE_CASES = {
-    # name: (q, degree (0 = Erdos-Renyi CSR with rows of 0..16 entries), R, replica_block, weighted)
-    "q8_reg10_R16_rb8": (8, 10, 16, 8, False),          # cfg 2's shape: 4 variables per warp iteration
-    "q8_reg10_R32_rb16": (8, 10, 32, 16, False),        # 2 variables per warp iteration, two blocks
-    "q8_reg10_R16_auto": (8, 10, 16, 0, False),
-    "q4_reg6_weighted_R32": (4, 6, 32, 32, True),       # one variable per warp iteration
-    "q2_reg3_R64_rb16": (2, 3, 64, 16, False),
-    "q3_reg6_R24_rb8": (3, 6, 24, 8, False),            # q not a power of two: padded tree, padded shared rows
-    "q5_reg4_weighted_R16": (5, 4, 16, 16, True),
-    "q7_reg16_R8": (7, 16, 8, 8, False),                # the largest degree the slot holds
-    "q8_er_csr_R16_rb8": (8, 0, 16, 8, False),          # rows of different lengths, isolated nodes
-    "q6_er_csr_weighted_R32_rb16": (6, 0, 32, 16, True),
-}
-
-
-@pytest.mark.parametrize("opt", ["adam", "sgd_mom", "rmsprop"])
-@pytest.mark.parametrize("case", list(LANE_CASES))
-def test_potts_lane_bit_identical_to_team_kernel(fem, case, opt):
-    """The lane-per-replica Potts step (k_step_potts_lane.cu: a lane owns all q states of a replica, rows staged in
-    shared memory by cp.async one iteration ahead) against the register path: same arithmetic in the same order, so
-    fields, moments and energies must be bit-identical; the counter proves which one ran.  n is chosen so that the
-    last warp iteration is ragged."""
-    q, d, R, rb, weighted = LANE_CASES[case]
-    if d == 0:
-        er = wl.erdos_renyi_maxcut(1203, 0.0045, 2040 + q, pm1=False)
-        assert 0 < np.diff(er.row_ptr).max() <= 16 and np.diff(er.row_ptr).min() == 0
-        inst = wl.Instance(wl.BMINCUT, er.n, q, er.row_ptr, er.col_idx, None, lam=0.03)
-    else:
-        inst = wl.random_regular(1201 if d % 2 == 0 else 1202, d, 2020 + q, wl.BMINCUT, q, lam=0.03)
-    if weighted:
-        w = np.random.default_rng(3).integers(1, 5, inst.nnz // 2).astype(np.float32)[edge_ids(inst)]
-        inst = wl.Instance(wl.BMINCUT, inst.n, q, inst.row_ptr, inst.col_idx, w, lam=0.03)
-    extra = {"adam": {}, "sgd_mom": dict(optimizer=2, lr=0.3, momentum=0.7, dampening=0.2),
-             "rmsprop": dict(optimizer=1, lr=0.03, alpha=0.9)}[opt]
-    sch = fem.Schedule(beta=fem.linear_temperature_schedule(1.0, 0.05, 40), precise_steps=4, **extra)
-    out = {}
-    for lane in (1, 0):
-        eng = fem.Fem(inst, R)
-        eng.set_option("potts_lane", lane)
-        eng.set_option("potts_si", 0)
-        eng.set_option("potts_tma", 0)
-        if rb:
-            eng.set_option("replica_block", rb)
-        eng.anneal(sch, R, seed=8, stop_after=17)
-        eng.anneal(sch, R, seed=8, stop_after=40)
-        out[lane] = (eng.get_fields(), eng.get_moments(), eng.result())
-        blocks = R // eng.info("replica_block")
-        applies = eng.info("replica_block") in (8, 16, 32)
-        assert eng.info("lane_launches") == (36 * blocks if lane and applies else 0), case   # 40 steps - 4 wide, per block
-        if rb:
-            assert applies
-        eng.close()
-    assert np.array_equal(out[1][0], out[0][0])
-    assert np.array_equal(out[1][1][0], out[0][1][0]) and np.array_equal(out[1][1][1], out[0][1][1])
-    assert np.array_equal(out[1][2]["energy"], out[0][2]["energy"])
-    assert np.array_equal(out[1][2]["part_sizes"], out[0][2]["part_sizes"])
-
-
-@pytest.mark.parametrize("opt", ["adam", "sgd_mom"])
-@pytest.mark.parametrize("name", ["maxcut_torus_30x34", "maxcut_reg3_pm1", "ising_reg3"])
-def test_gather_fields_mode_is_bit_identical(fem, name, opt):
-    """Gather-the-fields mode of the sparse two-state step (regular degree 3 / 4): neighbours gathered from the field
-    array with tanh recomputed, fields ping-ponging between two arrays, no gather array written.  Same arithmetic, so
-    fields, moments, marginals and energies are bit-identical to the default path -- across resume points, replica
-    blocks and the parity hooks called in between (which use the spare array as scratch)."""
-    if name == "ising_reg3":
-        inst, R = wl.sparse_ising_from(wl.random_regular(1000, 3, 2050, pm1=True), scale=0.37), 24
-    else:
-        inst, R = get(name)
-    if R % 4:
-        R = 4 * (R // 4 + 1)
-    extra = {"adam": {}, "sgd_mom": dict(optimizer=2, lr=0.3, momentum=0.7, dampening=0.2)}[opt]
-    sch = fem.Schedule(beta=fem.linear_temperature_schedule(1.0, 0.05, 60), precise_steps=4, **extra)
-    out = {}
-    for mode, rb in ((0, 0), (1, 0), (1, 4)):
-        eng = fem.Fem(inst, R)
-        eng.set_option("persistent", 0)
-        eng.set_option("gather_fields", mode)
-        if rb:
-            eng.set_option("replica_block", rb)
-        eng.anneal(sch, R, seed=9, stop_after=3)                      # inside the wide phase
-        eng.anneal(sch, R, seed=9, stop_after=17)
-        p17, h17 = eng.get_marginals(), eng.get_fields()
-        eng.anneal(sch, R, seed=9, stop_after=18)                     # an odd number of fp32 steps later
-        p18 = eng.get_marginals()
-        eng.anneal(sch, R, seed=9)
-        assert eng.info("gather_fields") == mode
-        out[(mode, rb)] = (h17, p17, p18, eng.get_fields(), eng.get_moments(), eng.result(), eng.get_configs())
-        eng.close()
-    b = out[(0, 0)]
-    for key, a in out.items():
-        for k in range(4):
-            assert np.array_equal(a[k], b[k]), (key, k)
-        assert np.array_equal(a[4][0], b[4][0]) and np.array_equal(a[4][1], b[4][1]), key
-        assert np.array_equal(a[5]["energy"], b[5]["energy"]) and a[5]["best_replica"] == b[5]["best_replica"], key
-        assert np.array_equal(a[6], b[6]), key
 
 
 SI_CASES = {
@@ -528,7 +429,6 @@ def test_potts_si_bit_identical_to_team_kernel(fem, case, opt):
     for si in (1, 0):
         eng = fem.Fem(inst, R)
         eng.set_option("potts_si", si)
-        eng.set_option("potts_lane", 0)
         eng.set_option("potts_tma", 0)
         if rb:
             eng.set_option("replica_block", rb)
