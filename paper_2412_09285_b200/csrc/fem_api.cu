@@ -242,7 +242,9 @@ static void configure_R(Handle *hd, int R) {
     hd->R = R;
     int Rb = R;
     const double per_replica = 20.0 * (double)hd->dp.n * hd->dp.F;
-    const double budget = 0.45 * (double)hd->l2_bytes;
+    // (one die's half of the L2, 63 MB of 126: working sets beyond it are served at 9 - 11 TB/s instead of 13 - 17, DESIGN.md
+    // section 6; 0.52 rather than 0.5 keeps the 64 MB block of the scale-free workload, measured faster than its 32 MB one)
+    const double budget = 0.52 * (double)hd->l2_bytes;
     if (hd->dp.kind == FEM_BMINCUT) {
         // a block must fit the team mapping of the Potts kernel (one variable's lanes inside a warp); among the
         // divisors of R that do, take the requested one, else the largest that is L2-resident, else the smallest
