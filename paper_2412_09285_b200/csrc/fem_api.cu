@@ -258,7 +258,9 @@ static void configure_R(Handle *hd, int R) {
         for (int d = 1; d <= R; ++d) {
             if (R % d || !potts_block_ok(q, d)) continue;
             largest = d;
-            if (per_replica * d <= budget && d % 4 == 0 && (double)hd->dp.n * hd->dp.F * d >= 1.0e6) resident = d;
+            // (Potts: 45%, not the 52% of the two-state kinds -- a 64 MB block of cfg 2 (Rb = 4) does not stay resident in steady
+            // state and runs at 0.41 against 0.49 for Rb = 8 with only its gather buffers in L2: profiles/r02_cfg2_step.md)
+            if (per_replica * d <= 0.45 * (double)hd->l2_bytes && d % 4 == 0 && (double)hd->dp.n * hd->dp.F * d >= 1.0e6) resident = d;
             if (8.0 * (double)hd->dp.n * hd->dp.F * d <= 0.45 * (double)hd->l2_bytes) gathers_fit = d;
             if (!smallest_vec && d % 2 == 0) smallest_vec = d;
         }
