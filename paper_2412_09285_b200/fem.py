@@ -184,9 +184,12 @@ class Fem:
             # (guard bytes on both sides of the workspace, filled with a pattern: tests check that the library never writes
             # outside the bytes it asked for)
             self._guard = 1 << 16
-            self._ws = torch.full((nbytes + 256 + 2 * self._guard,), 0xA5, dtype=torch.uint8, device=self.device)
+            self._ws = torch.empty(nbytes + 256 + 2 * self._guard, dtype=torch.uint8, device=self.device)
             base = self._ws.data_ptr() + self._guard
             self._ws_ptr = (base + 255) & ~255
+            lo = self._ws_ptr - self._ws.data_ptr()
+            self._ws[:lo].fill_(0xA5)               # only the guards are filled, not the workspace
+            self._ws[lo + nbytes:].fill_(0xA5)
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             h = C.c_void_p()
             st = self._lib.fem_create(C.byref(self._cp), self.R_cap, C.c_void_p(self._ws_ptr), C.c_size_t(nbytes),

@@ -390,6 +390,46 @@ def test_potts_tma_bit_identical_to_team_kernel(fem, case, manipulated):
     assert np.array_equal(out[1][2]["energy"], out[0][2]["energy"])
 
 
+@pytest.mark.parametrize("opt", ["adam", "sgd_mom"])
+@pytest.mark.parametrize("name", ["maxcut_torus_30x34", "maxcut_reg3_pm1", "ising_reg3"])
+def test_gather_fields_mode_is_bit_identical(fem, name, opt):
+    """Gather-the-fields mode of the sparse two-state step (regular degree 3 / 4): neighbours gathered from the field
+    array with tanh recomputed, fields ping-ponging between two arrays, no gather array written.  Same arithmetic, so
+    fields, moments, marginals and energies are bit-identical to the default path -- across resume points, replica
+    blocks and the parity hooks called in between (which use the spare array as scratch)."""
+    if name == "ising_reg3":
+        inst, R = wl.sparse_ising_from(wl.random_regular(1000, 3, 2050, pm1=True), scale=0.37), 24
+    else:
+        inst, R = get(name)
+    if R % 4:
+        R = 4 * (R // 4 + 1)
+    extra = {"adam": {}, "sgd_mom": dict(optimizer=2, lr=0.3, momentum=0.7, dampening=0.2)}[opt]
+    sch = fem.Schedule(beta=fem.linear_temperature_schedule(1.0, 0.05, 60), precise_steps=4, **extra)
+    out = {}
+    for mode, rb in ((0, 0), (1, 0), (1, 4)):
+        eng = fem.Fem(inst, R)
+        eng.set_option("persistent", 0)
+        eng.set_option("gather_fields", mode)
+        if rb:
+            eng.set_option("replica_block", rb)
+        eng.anneal(sch, R, seed=9, stop_after=3)                      # inside the wide phase
+        eng.anneal(sch, R, seed=9, stop_after=17)
+        p17, h17 = eng.get_marginals(), eng.get_fields()
+        eng.anneal(sch, R, seed=9, stop_after=18)                     # an odd number of fp32 steps later
+        p18 = eng.get_marginals()
+        eng.anneal(sch, R, seed=9)
+        assert eng.info("gather_fields") == mode
+        out[(mode, rb)] = (h17, p17, p18, eng.get_fields(), eng.get_moments(), eng.result(), eng.get_configs())
+        eng.close()
+    b = out[(0, 0)]
+    for key, a in out.items():
+        for k in range(4):
+            assert np.array_equal(a[k], b[k]), (key, k)
+        assert np.array_equal(a[4][0], b[4][0]) and np.array_equal(a[4][1], b[4][1]), key
+        assert np.array_equal(a[5]["energy"], b[5]["energy"]) and a[5]["best_replica"] == b[5]["best_replica"], key
+        assert np.array_equal(a[6], b[6]), key
+
+
 SI_CASES = {
     # name: (q, degree (0 = Erdos-Renyi CSR with rows of 0..16 entries), n, R, replica_block, weighted)
     "q8_reg10_R16_rb8": (8, 10, 1200, 16, 8, False),           # cfg 2's shape: 4 variables per 32-cell group
