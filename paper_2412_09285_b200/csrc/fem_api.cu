@@ -195,12 +195,22 @@ static bool validate_graph(const fem_problem *pb, int64_t nnz, bool *integral, i
             if (w != std::nearbyint(w) || std::fabs(w) > 1e6f) *integral = false;
         }
     }
-    // symmetry: every entry (i, j) has its mirror (j, i) with the same weight -- a binary search in row j (columns are strictly
-    // ascending), rows shared out over the host threads (the one-cursor-per-row sweep it replaces took 42 ms at cfg 4a,
-    // inside every end-to-end pass)
-    {
+    // symmetry: every entry (i, j) has its mirror (j, i) with the same weight.  Small graphs (the CSR stays in the host
+    // caches): one cursor per row, rows in ascending order -- the mirror of (i, j) is the next unread entry of row j.
+    // Large graphs: a binary search in row j (columns are strictly ascending), rows shared out over the host threads (the
+    // cursor sweep took 42 ms at cfg 4a, the search 0.75 ms at cfg 0: both inside every end-to-end pass)
+    if (nnz <= (int64_t)1 << 20) {
+        std::vector<int64_t> cur(pb->row_ptr, pb->row_ptr + n);
+        for (int i = 0; i < n; ++i)
+            for (int64_t e = pb->row_ptr[i]; e < pb->row_ptr[i + 1]; ++e) {
+                const int j = pb->col_idx[e];
+                const int64_t c = cur[j]++;
+                if (c >= pb->row_ptr[j + 1] || pb->col_idx[c] != i) return *err = "CSR is not symmetric", false;
+                if (pb->weight && pb->weight[c] != pb->weight[e]) return *err = "weights are not symmetric", false;
+            }
+    } else {
         const unsigned hw = std::max(1u, std::min(16u, std::thread::hardware_concurrency()));
-        const unsigned nt = n < 4096 ? 1u : hw;
+        const unsigned nt = hw;
         std::vector<int> bad(nt, 0);  // 0 ok, 1 not symmetric, 2 weights not symmetric
         auto work = [&](unsigned t) {
             const int a = (int)((int64_t)n * t / nt), b = (int)((int64_t)n * (t + 1) / nt);
@@ -366,7 +376,8 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
     auto at = [&](size_t off) { return base + off; };
 
     // host staging vectors must outlive the async copies: they die after the synchronise below
-    std::vector<int> h_row, h_occ_ptr, h_occ, h_cptr;
+    std::vector<int> h_row, h_occ_ptr, h_occ, h_cptr, h_long, h_ord;  // staging of the uploads: alive until the synchronize below
+    std::vector<double> h_rowsum;
     bool ok = true;
     bool device_checked = false;
     auto up = [&](void *dst, const void *src, size_t bytes, const char *what) {
@@ -501,7 +512,7 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
         dp.w = s.weighted ? reinterpret_cast<float *>(at(L.w)) : nullptr;
         if (pb->kind == FEM_ISING) hd->integral_weights = false;
         hd->structure_bytes = (dp.uniform_deg > 0 ? 0 : 4 * ((int64_t)pb->n + 1)) + (s.weighted ? 8 : 4) * s.nnz;
-        std::vector<int> h_long;  // long rows get a CTA each in the stepwise kernel (k_step_q2.cu)
+        // long rows get a CTA each in the stepwise kernel (k_step_q2.cu)
         if (pb->kind != FEM_BMINCUT)
             for (int i = 0; i < pb->n; ++i)
                 if (is_long_row(pb->row_ptr[i + 1] - pb->row_ptr[i], s.nnz, pb->n)) h_long.push_back(i);
@@ -509,19 +520,19 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
             up(at(L.long_rows), h_long.data(), h_long.size() * 4, "upload long rows");
             dp.long_rows = reinterpret_cast<int *>(at(L.long_rows));
             dp.n_long = (int)h_long.size();
-            if (ok) ok = cuda_ok(hd, cudaStreamSynchronize(hd->stream), "upload long rows");  // h_long is a local
         }
         if (pb->kind != FEM_BMINCUT && dp.uniform_deg == 0 && pb->n > 1) {
             // degree-sorted processing order of the stepwise kernel (counting sort, ascending, stable): a warp's variables
             // then have rows of nearly the same length, so its batched gather loop does no idle iterations on a
             // degree-skewed graph.  Which thread takes which variable changes no arithmetic.
-            std::vector<int> cnt((size_t)dp.max_deg + 2, 0), ord((size_t)pb->n);
+            std::vector<int> cnt((size_t)dp.max_deg + 2, 0);
+            std::vector<int> &ord = h_ord;
+            ord.resize((size_t)pb->n);
             for (int i = 0; i < pb->n; ++i) cnt[(size_t)(pb->row_ptr[i + 1] - pb->row_ptr[i]) + 1]++;
             for (size_t d = 1; d < cnt.size(); ++d) cnt[d] += cnt[d - 1];
             for (int i = 0; i < pb->n; ++i) ord[(size_t)cnt[(size_t)(pb->row_ptr[i + 1] - pb->row_ptr[i])]++] = i;
             up(at(L.order), ord.data(), ord.size() * 4, "upload order");
             dp.order = reinterpret_cast<int *>(at(L.order));
-            if (ok) ok = cuda_ok(hd, cudaStreamSynchronize(hd->stream), "upload order");  // ord is a local
         }
         if (pb->kind != FEM_BMINCUT) persist_prepare(hd, pb->row_ptr);
         dp.vtotal = (double)pb->n;
@@ -534,13 +545,13 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
             hd->structure_bytes += 4 * (int64_t)pb->n;
         }
         {   // sum_j |W_ij| per node, in double in CSR order (the normalisation factors of the manipulated gradients)
-            std::vector<double> rs((size_t)pb->n, 0.0);
+            std::vector<double> &rs = h_rowsum;
+            rs.assign((size_t)pb->n, 0.0);
             for (int i = 0; i < pb->n; ++i)
                 for (int64_t e = pb->row_ptr[i]; e < pb->row_ptr[i + 1]; ++e)
                     rs[i] += std::fabs(pb->weight ? (double)pb->weight[e] : 1.0);
             up(at(L.rowsum), rs.data(), rs.size() * 8, "upload rowsum");
             hd->rowsum = reinterpret_cast<double *>(at(L.rowsum));
-            if (ok) ok = cuda_ok(hd, cudaStreamSynchronize(hd->stream), "upload rowsum");  // rs is a local
         }
     }
     hd->lambda_last = pb->lambda;
