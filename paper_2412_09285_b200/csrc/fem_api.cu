@@ -23,13 +23,13 @@ void launch_potts_softmax(Handle *hd, float *out);
 void launch_qsat(Handle *hd, const StepScalars &sc, bool wide, bool step, int blk_begin, int blk_count);  // k_step_qsat.cu
 void launch_tc_split(Handle *hd);
 bool persist_eligible(const Handle *hd);
-void persist_prepare(Handle *hd, const int64_t *row_ptr);
+void persist_prepare(Handle *hd, const int64_t *row_ptr, const int *order);
 cudaError_t persist_run(Handle *hd, bool wide, int t_begin, int t_end, StepScalars (*scalars)(void *, int), void *ctx);
 
 static std::string g_create_error;
 
 struct Layout {
-    size_t row_ptr, col, w, rowsum, long_rows, vw, lit_state, order, J, Jlo, glo0, glo1, J8, gt8_0, gt8_1, jscale, field, occ_ptr, occ, clause_ptr, lits;
+    size_t row_ptr, col, w, rowsum, long_rows, vw, lit_state, order, rank, J, Jlo, glo0, glo1, J8, gt8_0, gt8_1, jscale, field, occ_ptr, occ, clause_ptr, lits;
     size_t h, m1, m2, g0, g1, stage, hW, m1W, m2W, gW0, gW1, colsum0, colsum1, colsum2, cfg, e_part_i, e_part_d, part_part, e_int, e_real, part,
         best, total;
 };
@@ -119,6 +119,7 @@ static Layout make_layout(const fem_problem *pb, const ProblemShape &s, int R_ca
     L.long_rows = take((size_t)s.n_long * 4);
     L.vw = take(pb->node_weight ? (size_t)pb->n * 4 : 0);
     L.order = take(pb->kind != FEM_BMINCUT && pb->row_ptr ? (size_t)pb->n * 4 : 0);
+    L.rank = take(pb->kind != FEM_BMINCUT && pb->row_ptr ? (size_t)pb->n * 4 : 0);
     L.J = take(s.dense ? (size_t)pb->n * pb->n * 4 : 0);
     L.Jlo = take(s.dense ? (size_t)pb->n * pb->n * 4 : 0);
     L.glo0 = take(s.dense ? state : 0);
@@ -376,7 +377,7 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
     auto at = [&](size_t off) { return base + off; };
 
     // host staging vectors must outlive the async copies: they die after the synchronise below
-    std::vector<int> h_row, h_occ_ptr, h_occ, h_cptr, h_long, h_ord;  // staging of the uploads: alive until the synchronize below
+    std::vector<int> h_row, h_occ_ptr, h_occ, h_cptr, h_long, h_ord, h_rank;  // staging of the uploads: alive until the synchronize below
     std::vector<double> h_rowsum;
     bool ok = true;
     bool device_checked = false;
@@ -463,7 +464,7 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
         if (!qs) {   // sliced-ELL sizes of the replica-persistent kernel, from the occurrence counts
             hd->dp = dp;
             std::vector<int64_t> optr(h_occ_ptr.begin(), h_occ_ptr.end());
-            persist_prepare(hd, optr.data());
+            persist_prepare(hd, optr.data(), nullptr);
         }
     } else if (s.dense) {
         const int n = pb->n;
@@ -533,8 +534,12 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
             for (int i = 0; i < pb->n; ++i) ord[(size_t)cnt[(size_t)(pb->row_ptr[i + 1] - pb->row_ptr[i])]++] = i;
             up(at(L.order), ord.data(), ord.size() * 4, "upload order");
             dp.order = reinterpret_cast<int *>(at(L.order));
+            h_rank.resize((size_t)pb->n);  // the inverse: the replica-persistent kernel turns columns into positions
+            for (int pos = 0; pos < pb->n; ++pos) h_rank[(size_t)ord[(size_t)pos]] = pos;
+            up(at(L.rank), h_rank.data(), h_rank.size() * 4, "upload rank");
+            dp.rank = reinterpret_cast<int *>(at(L.rank));
         }
-        if (pb->kind != FEM_BMINCUT) persist_prepare(hd, pb->row_ptr);
+        if (pb->kind != FEM_BMINCUT) persist_prepare(hd, pb->row_ptr, dp.order ? h_ord.data() : nullptr);
         dp.vtotal = (double)pb->n;
         if (pb->node_weight) {  // balance-term node weights (S33-S35); pb->node_weight outlives the upload (synchronised below)
             up(at(L.vw), pb->node_weight, (size_t)pb->n * 4, "upload node weights");

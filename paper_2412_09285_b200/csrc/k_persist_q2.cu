@@ -48,6 +48,9 @@ struct PersistParams {
     T eps, b1, b2, omb1, omb2, wd, gamma;
     int opt, disc;
     int kst;             // Max-SAT: ints per occurrence in `col` (k_max - 1 rounded up to a power of two)
+    const int *order;    // processing order of the variables (degree-sorted, fem_api.cu) or nullptr = identity
+    const int *rank;     // inverse of `order` (position of each variable) or nullptr = identity
+    int gn;              // slots per buffer of the gathered vector (persist_gn)
     int first_step;      // index in this chunk of the anneal's step 0 (SGD momentum buffer starts there), or -1
     T inv_beta[PersistChunk<T>::kSteps];
     T step_size[PersistChunk<T>::kSteps];
@@ -55,40 +58,83 @@ struct PersistParams {
 };
 
 constexpr int kPersistUnroll = 8;     // ELL rows are padded to a multiple of this: warp-uniform, remainder-free gather loops
+constexpr int kPersistRegGroups = 9;   // register-resident columns: the longest row they hold, in groups of 8 entries (72)
 constexpr int kPersistMaxUnits = 128;  // (items per thread) x (warps per CTA) <= 4 x 32
 
-// IPT variables per thread: variable i = c*chunk + k*blockDim.x + threadIdx.x.  ISING: dU/dp = -2 sum_j J_ij m_j.
+// ---- mbarrier / bulk-copy primitives of the cluster exchange ----
+__device__ __forceinline__ unsigned ps_smem(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ unsigned ps_mapa(unsigned addr, unsigned cta) {  // the same offset in the shared memory of CTA `cta`
+    unsigned r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(cta));
+    return r;
+}
+__device__ __forceinline__ void ps_wait(unsigned long long *bar, unsigned parity) {
+    asm volatile(
+        "{\n.reg .pred p;\nPS_WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra PS_DONE_%=;\nbra PS_WAIT_%=;\nPS_DONE_%=:\n}" ::"r"(ps_smem(bar)), "r"(parity) : "memory");
+}
+
+// IPT variables per thread.  Unit u = k * (warps per CTA) + warp of CTA c takes the 32 positions starting at (u*CS + c)*32
+// of the processing order (warps dealt out to the CTAs of the cluster in turn: with a degree-sorted order every CTA gets the
+// same mix of short and long rows, and the rows of a warp have nearly the same length, so the padding of the sliced ELL is
+// small).  The gathered vector is kept in SLOT order: the variable of thread tid, item k of CTA c sits at c*cw + k*nt + tid
+// (cw = IPT * nt), so that what a CTA produces in a step is one contiguous run, and the ELL columns are slots.
+//
+// Exchange between the CTAs of a cluster, once per annealing step: every thread stores its new m into its own CTA's copy;
+// after a CTA-wide barrier CS - 1 threads each push the CTA's run into one peer with a bulk copy through distributed shared
+// memory (cp.async.bulk.shared::cluster.shared::cta) that completes, in bytes, on the PEER's mbarrier of that buffer; a CTA
+// starts the next step when its own mbarrier has seen the CS - 1 runs.  No cluster barrier and no per-lane remote stores
+// (measured at cfg 0, CS = 4: 0.32 - 0.66 us of a 1.7 us step went to the 4-byte remote stores, 0.18 to the cluster barrier).
+// Two buffers are enough: a peer pushes its step-t run into the buffer I read in step t-1 only after it has received my
+// step-(t-1) run, which I send after my last read of that buffer.
+//
+// ISING: dU/dp = -2 sum_j J_ij m_j.
 // SATK > 0: Max-SAT -- `row_ptr` / `col` are the variable -> occurrence table (fem_internal.cuh), SATK = k_max - 1 packed
-// entries (var << 1 | negated) per occurrence, own sign in bit 31 of entry 0; the ELL keeps SATK 16-bit arrays and a sign
-// byte per slot; slot n of the gathered vector is the constant 1 that pads short clauses.
-template <typename T, int IPT, bool ISING, bool WEIGHTED, int SATK>
-__global__ void __launch_bounds__(1024, 1) persist_q2_kernel(const __grid_constant__ PersistParams<T> p) {
+// entries (var << 1 | negated) per occurrence, own sign in bit 31 of entry 0; the ELL keeps SATK 16-bit arrays
+// (slot << 1 | negated) and a sign byte per ELL entry (entry-major: entry j of lane l at [j*32 + l]); the last slot of the
+// gathered vector is the constant 1 that pads short clauses.  Graph modes: eight 16-bit columns per lane and 16-byte load
+// (entries 8g .. 8g+7 of lane l at [g*256 + l*8 ..]), the last slot is the constant 0.
+// RG > 0 (graph modes, IPT = 1, rows of at most 8 * RG entries): the thread keeps its row's columns in registers (RG * 4
+// packed words, padded with the constant slot) and the gather loop is unrolled in full: no column loads in the step and all
+// gathers of a row in flight at once.
+template <typename T, int IPT, bool ISING, bool WEIGHTED, int SATK, int RG>
+__global__ void __launch_bounds__(RG > 0 ? 512 : 1024, 1) persist_q2_kernel(const __grid_constant__ PersistParams<T> p) {
     namespace cg = cooperative_groups;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int unit_off[kPersistMaxUnits + 1];
-    const int n = p.n;
-    const int gn = n + 1;                                                  // slot n of each buffer stays 0: the ELL padding points at it
-    T *gbuf = reinterpret_cast<T *>(smem_raw);                             // [2][n + 1]
-    float *ws = reinterpret_cast<float *>(gbuf + 2 * (size_t)gn);         // [ell_cap] when WEIGHTED
-    unsigned short *cs = reinterpret_cast<unsigned short *>(WEIGHTED ? (ws + p.ell_cap) : ws);  // [ell_cap] ([SATK][ell_cap])
-    unsigned char *sgn = reinterpret_cast<unsigned char *>(cs + (size_t)(SATK > 0 ? SATK : 1) * p.ell_cap);  // SAT: [ell_cap]
-
+    __shared__ __align__(8) unsigned long long bar[2];
     cg::cluster_group cluster = cg::this_cluster();
     const unsigned CS = cluster.num_blocks();
     const unsigned c = cluster.block_rank();
+    const int n = p.n;
+    const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = nt >> 5;
+    const int cw = IPT * nt;          // slots per CTA
+    const int pad = (int)CS * cw;     // the constant slot the ELL padding points at
+    const int gn = p.gn;              // slots per buffer, >= pad + 1, a multiple of 4 (16-byte alignment of what follows)
+    T *gbuf = reinterpret_cast<T *>(smem_raw);                             // [2][gn]
+    float *ws = reinterpret_cast<float *>(gbuf + 2 * (size_t)gn);         // [ell_cap] when WEIGHTED
+    unsigned short *cs = reinterpret_cast<unsigned short *>(WEIGHTED ? (ws + p.ell_cap) : ws);  // [ell_cap] ([SATK][ell_cap])
+    unsigned char *sgn = reinterpret_cast<unsigned char *>(cs + (size_t)(SATK > 0 ? SATK : 1) * p.ell_cap);  // SAT: [ell_cap]
     const int r = blockIdx.x / CS;  // replica
     const int64_t base = (int64_t)(r / p.Rb) * p.blk_stride + (r % p.Rb);
-    const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = nt >> 5;
-    const int v_begin = c * p.chunk, v_end = min(n, v_begin + p.chunk);
+    auto slot_of = [&](int j) -> int {
+        const int pos = p.rank ? p.rank[j] : j;
+        const int gw = pos >> 5;
+        return (gw % (int)CS) * cw + (gw / (int)CS) * 32 + (pos & 31);
+    };
 
     // ---- state into registers, the whole gathered vector into this CTA's shared memory ----
     T h[IPT], m1[IPT], m2[IPT];
+    int vi[IPT];                                 // the variable, -1 = none
     int e0[IPT], deg[IPT], off[IPT], pdeg[IPT];  // pdeg: the unit's longest row rounded up to kPersistUnroll (warp-uniform)
 #pragma unroll
     for (int k = 0; k < IPT; ++k) {
-        const int i = v_begin + k * nt + tid;
-        const bool ok = i < v_end;
-        const int64_t o = base + (int64_t)(ok ? i : 0) * p.Rb;
+        const int pos = ((k * nwarps + warp) * (int)CS + (int)c) * 32 + lane;
+        const bool ok = pos < n;
+        const int i = ok ? (p.order ? p.order[pos] : pos) : 0;
+        vi[k] = ok ? i : -1;
+        const int64_t o = base + (int64_t)i * p.Rb;
         h[k] = ok ? p.h[o] : (T)0;
         m1[k] = ok ? p.m1[o] : (T)0;
         m2[k] = ok ? p.m2[o] : (T)0;
@@ -100,38 +146,43 @@ __global__ void __launch_bounds__(1024, 1) persist_q2_kernel(const __grid_consta
         pdeg[k] = (mx + kPersistUnroll - 1) / kPersistUnroll * kPersistUnroll;
         if (lane == 0) unit_off[k * nwarps + warp + 1] = pdeg[k] * 32;
     }
-    for (int i = tid; i < n; i += nt)
-        gbuf[i] = p.disc ? (T)(int)p.g8_in[base + (int64_t)i * p.Rb] : p.g_in[base + (int64_t)i * p.Rb];
+    for (int x = tid; x < 2 * gn; x += nt) gbuf[x] = (T)0;  // (slots of no variable travel with the runs: keep them defined)
     if (tid == 0) {
         unit_off[0] = 0;
-        gbuf[n] = SATK > 0 ? (T)1 : (T)0;
-        gbuf[gn + n] = SATK > 0 ? (T)1 : (T)0;
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(ps_smem(&bar[0])));
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(ps_smem(&bar[1])));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
+    for (int i = tid; i < n; i += nt)
+        gbuf[slot_of(i)] = p.disc ? (T)(int)p.g8_in[base + (int64_t)i * p.Rb] : p.g_in[base + (int64_t)i * p.Rb];
+    if (tid < 2) gbuf[tid * gn + pad] = SATK > 0 ? (T)1 : (T)0;
     if (tid == 0)
         for (int u = 1; u <= IPT * nwarps; ++u) unit_off[u] += unit_off[u - 1];
     __syncthreads();
-    // ---- this CTA's CSR rows as a sliced ELL: slot j of lane l of unit (k, warp) at unit_off + j*32 + l ----
+    // ---- this CTA's CSR rows as a sliced ELL ----
 #pragma unroll
     for (int k = 0; k < IPT; ++k) {
-        off[k] = unit_off[k * nwarps + warp] + lane;
-        for (int j = 0; j < pdeg[k]; ++j) {  // rows shorter than the unit are padded with (column n, weight 0): adds +0
+        off[k] = unit_off[k * nwarps + warp] + (SATK > 0 ? lane : lane * kPersistUnroll);
+        for (int j = 0; j < pdeg[k]; ++j) {  // rows shorter than the unit are padded with (pad slot, weight 0): adds +0
             const bool real = j < deg[k];
             if (SATK > 0) {
                 // padding occurrence: first factor 0.5 - 0.5 * 1 = 0, the others 1: contributes +-0
 #pragma unroll
                 for (int x = 0; x < (SATK > 0 ? SATK : 1); ++x) {
                     const unsigned pk = real ? (unsigned)p.col[(int64_t)(e0[k] + j) * p.kst + x] : (((unsigned)n << 1) | (x == 0 ? 0u : 1u));
-                    cs[(size_t)x * p.ell_cap + off[k] + j * 32] = (unsigned short)(pk & 0xffffu);
+                    const unsigned var = (pk & 0x7fffffffu) >> 1;
+                    const unsigned sl = var >= (unsigned)n ? (unsigned)pad : (unsigned)slot_of((int)var);  // (short clauses are padded with variable n)
+                    cs[(size_t)x * p.ell_cap + off[k] + j * 32] = (unsigned short)((sl << 1) | (pk & 1u));
                     if (x == 0) sgn[off[k] + j * 32] = (unsigned char)(pk >> 31);
                 }
                 continue;
             }
-            cs[off[k] + j * 32] = real ? (unsigned short)p.col[e0[k] + j] : (unsigned short)n;
-            if (WEIGHTED) ws[off[k] + j * 32] = real ? p.w[e0[k] + j] : 0.0f;
+            cs[off[k] + (j / kPersistUnroll) * (32 * kPersistUnroll) + (j % kPersistUnroll)] = (unsigned short)(real ? slot_of(p.col[e0[k] + j]) : pad);
+            if (WEIGHTED) ws[unit_off[k * nwarps + warp] + j * 32 + lane] = real ? p.w[e0[k] + j] : 0.0f;
         }
     }
-    if (CS > 1) cluster.sync();  // every CTA of the cluster is running before anyone stores into its shared memory
+    if (CS > 1) cluster.sync();  // every CTA of the cluster is running (and its mbarriers exist) before anyone pushes into it
     else __syncthreads();
 
     Sc<T> sc;
@@ -143,12 +194,25 @@ __global__ void __launch_bounds__(1024, 1) persist_q2_kernel(const __grid_consta
 #pragma unroll
     for (int k = 0; k < IPT; ++k) {
         ci[k] = (T)1;
-        const int i = v_begin + k * nt + tid;
-        if (p.disc && i < v_end) {
+        const int i = vi[k];
+        if (p.disc && i >= 0) {
             const double rs = p.rowsum[i] * (ISING ? 2.0 : 1.0);
             ci[k] = rs > 0.0 ? (T)(1.0 / rs) : (T)0;
         }
     }
+    unsigned creg[RG > 0 ? RG * 4 : 1];
+    if (RG > 0) {
+        __syncthreads();  // (the staged columns of this thread were written by this thread; the barrier is for tidiness only)
+#pragma unroll
+        for (int g = 0; g < RG; ++g) {
+            uint4 pk = make_uint4(0u, 0u, 0u, 0u);
+            if (g * kPersistUnroll < pdeg[0]) pk = *reinterpret_cast<const uint4 *>(cs + off[0] + g * kPersistUnroll * 32);
+            else pk.x = pk.y = pk.z = pk.w = (unsigned)pad | ((unsigned)pad << 16);
+            creg[g * 4 + 0] = pk.x; creg[g * 4 + 1] = pk.y; creg[g * 4 + 2] = pk.z; creg[g * 4 + 3] = pk.w;
+        }
+    }
+    const unsigned run_bytes = (unsigned)cw * (unsigned)sizeof(T);
+    unsigned phase[2] = {0u, 0u};
     int cur = 0;
     for (int t = 0; t < p.nsteps; ++t) {
         const T *__restrict__ gi = gbuf + (size_t)cur * gn;
@@ -159,8 +223,7 @@ __global__ void __launch_bounds__(1024, 1) persist_q2_kernel(const __grid_consta
         sc.first = t == p.first_step;
 #pragma unroll
         for (int k = 0; k < IPT; ++k) {
-            const int i = v_begin + k * nt + tid;
-            if (i < v_end) {
+            if (vi[k] >= 0) {
                 T dU = (T)0;
                 const unsigned short *__restrict__ cp = cs + off[k];
                 if (SATK > 0) {
@@ -177,42 +240,70 @@ __global__ void __launch_bounds__(1024, 1) persist_q2_kernel(const __grid_consta
                         }
                         dU += sp[j * 32] ? -prod : prod;
                     }
-                } else if (WEIGHTED) {
-                    const float *__restrict__ wp = ws + off[k];
-#pragma unroll kPersistUnroll
-                    for (int j = 0; j < pdeg[k]; ++j) dU = fma((T)wp[j * 32], gi[cp[j * 32]], dU);
+                } else if (RG > 0 && !WEIGHTED) {
+                    // no branches: every gather of the row is issued before the first add (rows shorter than 8 * RG read the
+                    // constant slot, a broadcast)
+                    T mv[RG > 0 ? RG * kPersistUnroll : 1];
+#pragma unroll
+                    for (int x = 0; x < RG * kPersistUnroll; ++x) mv[x] = gi[(creg[x >> 1] >> ((x & 1) * 16)) & 0xffffu];
+#pragma unroll
+                    for (int x = 0; x < RG * kPersistUnroll; ++x) dU += mv[x];  // (the padding adds +0 at the end: CSR order kept)
                 } else {
-#pragma unroll kPersistUnroll
-                    for (int j = 0; j < pdeg[k]; ++j) dU += gi[cp[j * 32]];  // == fma(1, m_j, dU) of the stepwise kernel
+                    // eight columns per 16-byte load; the sum runs in CSR order (== the stepwise kernel's fma(w, m_j, dU))
+                    const float *__restrict__ wp = ws + unit_off[k * nwarps + warp] + lane;
+#pragma unroll 2
+                    for (int jg = 0; jg < pdeg[k]; jg += kPersistUnroll) {
+                        const uint4 pk = *reinterpret_cast<const uint4 *>(cp + jg * 32);
+                        const unsigned w4[4] = {pk.x, pk.y, pk.z, pk.w};
+                        T mv[kPersistUnroll];
+#pragma unroll
+                        for (int x = 0; x < kPersistUnroll; ++x) mv[x] = gi[(w4[x >> 1] >> ((x & 1) * 16)) & 0xffffu];
+#pragma unroll
+                        for (int x = 0; x < kPersistUnroll; ++x) {
+                            if (WEIGHTED) dU = fma((T)wp[(jg + x) * 32], mv[x], dU);
+                            else dU += mv[x];
+                        }
+                    }
                 }
                 if (ISING) dU = (T)-2 * dU;
                 const T g = q2_grad(dU, ci[k], h[k], sc);
                 h[k] = opt_update(h[k], g, m1[k], m2[k], sc);
-                const T mg = sc.disc ? sign_of(h[k]) : mag_of(h[k]);
-                if (CS > 1) {
-                    for (unsigned pr = 0; pr < CS; ++pr) cluster.map_shared_rank(go, pr)[i] = mg;
-                } else {
-                    go[i] = mg;
-                }
+                go[(int)c * cw + k * nt + tid] = sc.disc ? sign_of(h[k]) : mag_of(h[k]);
             }
         }
-        // one barrier per step is enough with two buffers: step t+1 overwrites the buffer step t READ, and no
-        // CTA starts step t+1 before all have finished step t
-        if (CS > 1) cluster.sync();
-        else __syncthreads();
+        if (CS > 1) {
+            const int b = cur ^ 1;
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // my stores, before the bulk copies read them
+            __syncthreads();
+            if (tid == 0)
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(ps_smem(&bar[b])), "r"((CS - 1) * run_bytes) : "memory");
+            if (tid < (int)CS && tid != (int)c) {
+                const unsigned src = ps_smem(go + (size_t)c * cw);
+                asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                                 ps_mapa(src, (unsigned)tid)),
+                             "r"(src), "r"(run_bytes), "r"(ps_mapa(ps_smem(&bar[b]), (unsigned)tid))
+                             : "memory");
+            }
+            ps_wait(&bar[b], phase[b]);
+            phase[b] ^= 1u;
+        } else {
+            __syncthreads();
+        }
         cur ^= 1;
     }
+    if (CS > 1) cluster.sync();  // nobody leaves while a peer's last push may still be reading or writing here
 
 #pragma unroll
     for (int k = 0; k < IPT; ++k) {
-        const int i = v_begin + k * nt + tid;
-        if (i < v_end) {
+        const int i = vi[k];
+        if (i >= 0) {
             const int64_t o = base + (int64_t)i * p.Rb;
             p.h[o] = h[k];
             p.m1[o] = m1[k];
             p.m2[o] = m2[k];
-            if (p.disc) p.g8_out[o] = (signed char)(int)gbuf[(size_t)cur * gn + i];
-            else p.g_out[o] = gbuf[(size_t)cur * gn + i];
+            const T mg = gbuf[(size_t)cur * gn + (int)c * cw + k * nt + tid];
+            if (p.disc) p.g8_out[o] = (signed char)(int)mg;
+            else p.g_out[o] = mg;
         }
     }
 }
@@ -234,27 +325,37 @@ static bool persist_geometry(int n, int cs, PersistGeom *g) {
     return true;
 }
 
-// Called by fem_create with the host CSR: sliced-ELL entries per CTA (max over the CTAs of a cluster) for each
-// cluster size; -1 where the mapping does not apply.
-void persist_prepare(Handle *hd, const int64_t *row_ptr) {
+// Slots per buffer of the gathered vector: IPT * threads per CTA of the cluster, the constant slot, rounded up to 4.
+static int persist_gn(int n, int cs) {
+    PersistGeom g;
+    if (!persist_geometry(n, cs, &g)) return 0;
+    return (cs * g.ipt * g.threads + 1 + 3) & ~3;
+}
+
+// Called by fem_create with the host CSR (or occurrence table) and the processing order (nullptr = identity): sliced-ELL
+// entries per CTA (max over the CTAs of a cluster) for each cluster size, with the kernel's unit -> position mapping;
+// -1 where the mapping does not apply.
+void persist_prepare(Handle *hd, const int64_t *row_ptr, const int *order) {
     const int n = hd->dp.n;
     for (int a = 0; a < 4; ++a) {
         hd->persist_ell[a] = -1;
         PersistGeom g;
-        if (n > 65535 || !persist_geometry(n, kClusterSizes[a], &g)) continue;
+        const int cs = kClusterSizes[a];
+        if (n > 65535 || !persist_geometry(n, cs, &g)) continue;
+        const int units = g.ipt * (g.threads / 32);
         int64_t worst = 0;
-        for (int c = 0; c < kClusterSizes[a]; ++c) {
+        for (int c = 0; c < cs; ++c) {
             int64_t entries = 0;
-            const int v_begin = c * g.chunk, v_end = std::min(n, v_begin + g.chunk);
-            for (int k = 0; k < g.ipt; ++k)
-                for (int w0 = 0; w0 < g.threads; w0 += 32) {
-                    int64_t mx = 0;
-                    for (int l = 0; l < 32; ++l) {
-                        const int i = v_begin + k * g.threads + w0 + l;
-                        if (i < v_end) mx = std::max<int64_t>(mx, row_ptr[i + 1] - row_ptr[i]);
-                    }
-                    entries += 32 * ((mx + kPersistUnroll - 1) / kPersistUnroll * kPersistUnroll);
+            for (int u = 0; u < units; ++u) {
+                int64_t mx = 0;
+                for (int l = 0; l < 32; ++l) {
+                    const int64_t pos = ((int64_t)u * cs + c) * 32 + l;
+                    if (pos >= n) break;
+                    const int i = order ? order[pos] : (int)pos;
+                    mx = std::max<int64_t>(mx, row_ptr[i + 1] - row_ptr[i]);
                 }
+                entries += 32 * ((mx + kPersistUnroll - 1) / kPersistUnroll * kPersistUnroll);
+            }
             worst = std::max(worst, entries);
         }
         hd->persist_ell[a] = worst;
@@ -262,8 +363,10 @@ void persist_prepare(Handle *hd, const int64_t *row_ptr) {
 }
 
 static size_t persist_smem_bytes(const Handle *hd, int a, size_t elt) {
-    const size_t per_slot = hd->dp.kind == FEM_MAXSAT ? 2 * (size_t)hd->dp.kstride + 1 : (hd->dp.w ? 6 : 2);
-    return 2 * ((size_t)hd->dp.n + 1) * elt + (size_t)hd->persist_ell[a] * per_slot + 16;
+    const bool sat = hd->dp.kind == FEM_MAXSAT;
+    const size_t per_slot = sat ? 2 * (size_t)hd->dp.kstride + 1 : (hd->dp.w ? 6 : 2);
+    (void)sat;
+    return 2 * (size_t)persist_gn(hd->dp.n, kClusterSizes[a]) * elt + (size_t)hd->persist_ell[a] * per_slot + 16;
 }
 
 // Cluster size index for R replicas: spread a replica over as many SMs as the device has to spare (R * CS <= SMs),
@@ -278,6 +381,7 @@ static int persist_choose(const Handle *hd, int R) {
     int best = -1;
     for (int a = 0; a < 4; ++a) {
         if (hd->persist_ell[a] < 0 || persist_smem_bytes(hd, a, sizeof(double)) > kSmemCap) continue;
+        if (persist_gn(hd->dp.n, kClusterSizes[a]) > (sat ? 32768 : 65536)) continue;  // slots (SAT: slot << 1 | negated) are 16-bit ELL columns
         if (hd->opt_persistent > 1) {  // forced cluster size (tests, experiments)
             if (kClusterSizes[a] == hd->opt_persistent - 1) return a;
             continue;
@@ -317,14 +421,22 @@ static cudaError_t persist_launch_ipt(Handle *hd, const PersistParams<T> &p, int
     const bool ising = hd->dp.kind == FEM_ISING, weighted = hd->dp.w != nullptr;
     if (hd->dp.kind == FEM_MAXSAT) {
         switch (hd->dp.kstride) {
-            case 1: return launch(persist_q2_kernel<T, IPT, false, false, 1>);
-            case 2: return launch(persist_q2_kernel<T, IPT, false, false, 2>);
-            case 3: return launch(persist_q2_kernel<T, IPT, false, false, 3>);
-            default: return launch(persist_q2_kernel<T, IPT, false, false, 4>);
+            case 1: return launch(persist_q2_kernel<T, IPT, false, false, 1, 0>);
+            case 2: return launch(persist_q2_kernel<T, IPT, false, false, 2, 0>);
+            case 3: return launch(persist_q2_kernel<T, IPT, false, false, 3, 0>);
+            default: return launch(persist_q2_kernel<T, IPT, false, false, 4, 0>);
         }
     }
-    if (ising) return weighted ? launch(persist_q2_kernel<T, IPT, true, true, 0>) : launch(persist_q2_kernel<T, IPT, true, false, 0>);
-    return weighted ? launch(persist_q2_kernel<T, IPT, false, true, 0>) : launch(persist_q2_kernel<T, IPT, false, false, 0>);
+    if (IPT == 1 && sizeof(T) == 4 && !weighted && hd->dp.max_deg <= kPersistRegGroups * kPersistUnroll && threads <= 512) {
+        // columns in registers, fp32 steps of unit-weight graphs: 24, 48 or 72 entries per row
+        constexpr bool on = IPT == 1 && sizeof(T) == 4;
+        const int groups = (hd->dp.max_deg + kPersistUnroll - 1) / kPersistUnroll;
+        if (groups <= 3) return ising ? launch(persist_q2_kernel<T, IPT, true, false, 0, on ? 3 : 0>) : launch(persist_q2_kernel<T, IPT, false, false, 0, on ? 3 : 0>);
+        if (groups <= 6) return ising ? launch(persist_q2_kernel<T, IPT, true, false, 0, on ? 6 : 0>) : launch(persist_q2_kernel<T, IPT, false, false, 0, on ? 6 : 0>);
+        return ising ? launch(persist_q2_kernel<T, IPT, true, false, 0, on ? 9 : 0>) : launch(persist_q2_kernel<T, IPT, false, false, 0, on ? 9 : 0>);
+    }
+    if (ising) return weighted ? launch(persist_q2_kernel<T, IPT, true, true, 0, 0>) : launch(persist_q2_kernel<T, IPT, true, false, 0, 0>);
+    return weighted ? launch(persist_q2_kernel<T, IPT, false, true, 0, 0>) : launch(persist_q2_kernel<T, IPT, false, false, 0, 0>);
 }
 
 // Runs steps [t_begin, t_end) of the schedule for all replicas; `scalars(t)` gives the per-step scalars.
@@ -352,6 +464,9 @@ static cudaError_t persist_run_t(Handle *hd, int t_begin, int t_end, F &&scalars
         p.w = sat ? nullptr : hd->dp.w;
         p.kst = 1;
         while (p.kst < hd->dp.kstride) p.kst <<= 1;
+        p.order = sat ? nullptr : hd->dp.order;
+        p.rank = sat ? nullptr : hd->dp.rank;
+        p.gn = persist_gn(hd->dp.n, cs);
         p.n = hd->dp.n;
         p.Rb = hd->Rb;
         p.blk_stride = hd->rows * hd->Rb;
