@@ -191,7 +191,9 @@ fem_status fem_energy_of(fem_handle *h, const int32_t *cfg /* [count][n] */, int
  * "tc_cluster" (int8 step: 1 = 2 x 2 thread-block clusters with operand multicast where the tile grid is even in both
  * directions, the default; 0 = off; bit-identical either way).
  * "persistent" (small sparse MAXCUT / ISING / MAXSAT problems with few enough replicas to run in at most three
- * waves of clusters: 1 = replica-persistent cluster kernel where the problem fits, the default; 0 = one launch per step; 1 + CS = force clusters of CS = 1, 2, 4 or 8 CTAs per replica) and
+ * waves of clusters: 1 = replica-persistent cluster kernel where the problem fits, the default; 0 = one launch per step; 1 + CS = force clusters of CS = 1, 2, 4 or 8 CTAs per replica),
+ * "persist_chunk" (annealing steps per launch of that kernel: 0 = as many as its parameters hold, 2048 in fp32, the default;
+ * 1 .. 2048 = at most that many; no effect on the result) and
  * "long_rows" (two-state graph kinds: 1 = rows with many entries are summed by a CTA each in a fixed order, the default;
  * 0 = one thread per row as for short rows -- this one does change the summation order of those rows),
  * "potts_si" (BMINCUT, q = 4 or 8, replica blocks of 4 / 8 / 16 / 32 with n a multiple of 32 / block: 1 = fp32 steps on

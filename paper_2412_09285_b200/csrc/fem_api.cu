@@ -644,6 +644,9 @@ fem_status fem_set_option(fem_handle *h, const char *key, int64_t value) {
     } else if (!strcmp(key, "persistent")) {
         if (value < 0 || value > 9) return fail(hd, FEM_EINVAL, "persistent must be 0, 1 or 1 + cluster size");
         hd->opt_persistent = value;
+    } else if (!strcmp(key, "persist_chunk")) {
+        if (value < 0 || value > 2048) return fail(hd, FEM_EINVAL, "persist_chunk must be 0 .. 2048");
+        hd->opt_persist_chunk = value;
     } else if (!strcmp(key, "potts_tma")) {
         if (value < 0 || value > 1) return fail(hd, FEM_EINVAL, "potts_tma must be 0 or 1");
         hd->opt_potts_tma = value;

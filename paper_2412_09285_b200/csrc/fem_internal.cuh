@@ -152,6 +152,7 @@ struct Handle {
     // small sparse two-state problems: replica-persistent kernel (k_persist_q2.cu).  0 = off, 1 = automatic cluster
     // size, 1 + CS = force clusters of CS CTAs per replica
     int64_t opt_persistent = 1;
+    int64_t opt_persist_chunk = 0;  // annealing steps per launch of the persistent kernel (0 = as many as the parameters hold)
     int64_t persist_launches = 0, persist_cluster = 0;
     int64_t opt_potts_tma = 1;    // Potts step with TMA-staged rows (k_step_potts_tma.cu) where it applies
     int64_t tma_launches = 0;

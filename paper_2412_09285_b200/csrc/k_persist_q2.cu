@@ -26,7 +26,7 @@ namespace fem {
 
 template <typename T>
 struct PersistChunk {
-    static constexpr int kSteps = sizeof(T) == 4 ? 256 : 96;  // 3 * kSteps * sizeof(T) <= 3 KB of kernel parameters
+    static constexpr int kSteps = sizeof(T) == 4 ? 2048 : 1024;  // 3 * kSteps * sizeof(T) = 24 KB of the 32 KB of kernel parameters
 };
 
 template <typename T>
@@ -449,8 +449,9 @@ static cudaError_t persist_run_t(Handle *hd, int t_begin, int t_end, F &&scalars
     PersistGeom g;
     persist_geometry(hd->dp.n, cs, &g);
     const size_t smem = persist_smem_bytes(hd, a, sizeof(T));
-    for (int ta = t_begin; ta < t_end; ta += PersistChunk<T>::kSteps) {
-        const int tb = std::min(t_end, ta + PersistChunk<T>::kSteps);
+    const int per_launch = hd->opt_persist_chunk > 0 ? (int)std::min<int64_t>(hd->opt_persist_chunk, PersistChunk<T>::kSteps) : PersistChunk<T>::kSteps;
+    for (int ta = t_begin; ta < t_end; ta += per_launch) {
+        const int tb = std::min(t_end, ta + per_launch);
         PersistParams<T> p;
         p.h = S::h(hd);
         p.m1 = S::m1(hd);

@@ -323,7 +323,7 @@ def test_persistent_kernel_bit_identical_to_stepwise(fem, name, mode):
     registers, gathers from shared memory).  Its arithmetic is the stepwise kernel's, so fields, moments and
     energies must be bit-identical, including across a resume (stop_after) and the fp64 wide phase."""
     inst, R = _persist_cases()[name]()
-    steps = 300                                                      # spans two parameter chunks of the fp32 kernel
+    steps = 300                                                      # three launches of the fp32 kernel (persist_chunk below)
     extra = {"adam_exact": {}, "rmsprop_manipulated": dict(optimizer=1, lr=0.03, alpha=0.9, momentum=0.5,
                                                             manipulated=True, gamma_grad=0.9),
              "sgd_exact": dict(optimizer=2, lr=0.3, momentum=0.7, dampening=0.2)}[mode]
@@ -332,6 +332,7 @@ def test_persistent_kernel_bit_identical_to_stepwise(fem, name, mode):
     for persistent in (0, 1, 2, 3, 5, 9):                             # off, automatic, clusters of 1, 2, 4, 8 CTAs per replica
         eng = fem.Fem(inst, R)
         eng.set_option("persistent", persistent)
+        eng.set_option("persist_chunk", 128)
         eng.anneal(sch, R, seed=4, stop_after=5)                      # stops inside the wide phase
         h5 = eng.get_fields()
         eng.anneal(sch, R, seed=4, stop_after=37)
