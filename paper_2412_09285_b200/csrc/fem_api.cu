@@ -429,21 +429,35 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
         // its factor (1 - 1/q) - D is 1
         h_occ.assign((size_t)s.nocc * kst, qs ? n * F : ((n << 1) | 1));
         std::vector<int> fill(h_occ_ptr.begin(), h_occ_ptr.end() - 1);
-        for (int c = 0; c < m; ++c) {  // clause order inside each variable's list == the oracle's summation order
-            const int64_t a = pb->clause_ptr[c], b = pb->clause_ptr[c + 1];
-            for (int64_t x = a; x < b; ++x) {
-                const int lit = pb->lits[x];
-                const int v = (lit > 0 ? lit : -lit) - 1;
-                int *ent = h_occ.data() + (size_t)fill[qs ? v * F + qs[x] : v]++ * kst;
-                int k = 0;
-                for (int64_t y = a; y < b; ++y) {
-                    if (y == x) continue;
-                    const int l2 = pb->lits[y];
-                    if (qs) ent[k++] = (l2 - 1) * F + qs[y];
-                    else ent[k++] = (((l2 > 0 ? l2 : -l2) - 1) << 1) | (l2 < 0 ? 1 : 0);
+        // clause order inside each variable's list == the oracle's summation order.  Large tables: the variables are shared out
+        // over host threads, each scanning all clauses for its own range (the scattered 16-byte writes are what costs:
+        // 14 ms of every end-to-end pass at cfg 3 with one thread)
+        auto fill_range = [&](int vlo, int vhi) {
+            for (int c = 0; c < m; ++c) {
+                const int64_t a = pb->clause_ptr[c], b = pb->clause_ptr[c + 1];
+                for (int64_t x = a; x < b; ++x) {
+                    const int lit = pb->lits[x];
+                    const int v = (lit > 0 ? lit : -lit) - 1;
+                    if (v < vlo || v >= vhi) continue;
+                    int *ent = h_occ.data() + (size_t)fill[qs ? v * F + qs[x] : v]++ * kst;
+                    int k = 0;
+                    for (int64_t y = a; y < b; ++y) {
+                        if (y == x) continue;
+                        const int l2 = pb->lits[y];
+                        if (qs) ent[k++] = (l2 - 1) * F + qs[y];
+                        else ent[k++] = (((l2 > 0 ? l2 : -l2) - 1) << 1) | (l2 < 0 ? 1 : 0);
+                    }
+                    if (!qs && lit > 0) ent[0] |= 0x80000000;
                 }
-                if (!qs && lit > 0) ent[0] |= 0x80000000;
             }
+        };
+        {
+            const unsigned hw = std::max(1u, std::min(16u, std::thread::hardware_concurrency()));
+            const unsigned nt = s.nlits < 200000 ? 1u : hw;
+            std::vector<std::thread> pool;
+            for (unsigned t = 1; t < nt; ++t) pool.emplace_back(fill_range, (int)((int64_t)n * t / nt), (int)((int64_t)n * (t + 1) / nt));
+            fill_range(0, (int)((int64_t)n / nt));
+            for (auto &th : pool) th.join();
         }
         h_cptr.resize((size_t)m + 1);
         for (int c = 0; c <= m; ++c) h_cptr[c] = (int)pb->clause_ptr[c];
