@@ -226,6 +226,31 @@ fem_status fem_probe_l2_read(void *buffer, size_t bytes, int32_t repeats, void *
 fem_status fem_probe_l2_gather(void *buffer, size_t bytes, int32_t row_bytes, int32_t repeats, void *cuda_stream,
                                double *gigabytes_per_second);
 
+/* Cut values without any allocation (Eq.6: cut(sigma) = sum over edges (i, j), i < j, of W_ij [sigma_i != sigma_j]),
+ * for callers that cannot call cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses that forbid it.
+ * No handle, no workspace: the per-chunk partial sums that fem_energy_of keeps in the caller's workspace live in a
+ * file-scope static __device__ array of FEM_CUT_STATIC_SCRATCH_BYTES (2 MiB), which every GPU that loads the library holds
+ * until the process exits.  The call makes no cudaMalloc / cudaFree and calls no allocating library routine; it enqueues two
+ * kernels on `cuda_stream` and returns without synchronising (the first call on a device also looks up the array's device
+ * address, once: make that call before capturing a graph).
+ *   All pointers are DEVICE pointers on the CURRENT device, owned by the caller and neither checked nor kept:
+ *   n        number of nodes (>= 1)
+ *   row_ptr  int32 [n + 1], col_idx int32 [nnz]: the symmetric CSR of fem_problem (both directions of every edge, columns
+ *            ascending, no self loops); weight float [nnz] or NULL (= 1), rounded to the nearest integer per edge as in the
+ *            readout (a7)
+ *   sigma    int8 [n][count], configuration innermost: sigma[i * count + a] in {0, 1} is node i of configuration a
+ *   count    configurations, 1 .. FEM_CUT_STATIC_MAX_COUNT
+ *   cut      int64 [count], written: for the same graph and configurations fem_energy_of reports energy_int = -cut
+ * Returns FEM_EINVAL (count beyond the maximum: split the batch; n or count < 1; a null pointer) or FEM_ECUDA, with the reason
+ * in fem_cut_static_error() (per host thread).  Every call on a device shares the scratch array and finds the previous call's
+ * contents in it; nothing in it has to start at zero (each call writes every partial it reads).  Calls whose kernels may
+ * overlap on the GPU (streams without an ordering between them) RACE on it: order them on one stream or by events. */
+#define FEM_CUT_STATIC_MAX_COUNT 4096
+#define FEM_CUT_STATIC_SCRATCH_BYTES (2u << 20)
+fem_status fem_cut_static(int32_t n, const int32_t *row_ptr, const int32_t *col_idx, const float *weight, const int8_t *sigma,
+                          int32_t count, int64_t *cut, void *cuda_stream);
+const char *fem_cut_static_error(void);
+
 const char *fem_last_error(const fem_handle *h); /* h may be NULL: last create-time error */
 void fem_destroy(fem_handle *h);
 int32_t fem_abi_version(void);

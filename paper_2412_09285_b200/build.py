@@ -9,7 +9,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "libfem_b200.so")
-SOURCES = ["fem_api.cu", "k_init.cu", "k_step_q2.cu", "k_step_potts.cu", "k_readout.cu", "k_dense_tc.cu", "k_dense_i8.cu", "k_persist_q2.cu", "k_step_potts_tma.cu", "k_step_potts_si.cu", "k_step_qsat.cu", "k_probe.cu"]
+SOURCES = ["fem_api.cu", "k_init.cu", "k_step_q2.cu", "k_step_potts.cu", "k_readout.cu", "k_dense_tc.cu", "k_dense_i8.cu", "k_persist_q2.cu", "k_step_potts_tma.cu", "k_step_potts_si.cu", "k_step_qsat.cu", "k_probe.cu", "k_cut_static.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 

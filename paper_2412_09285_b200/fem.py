@@ -26,7 +26,9 @@ EXPORTS = [
     "fem_set_fields", "fem_get_fields", "fem_get_moments", "fem_get_marginals", "fem_get_configs", "fem_energy_of",
     "fem_set_option", "fem_get_info", "fem_last_error", "fem_destroy",
     "fem_schedule_inverse_proportional", "fem_schedule_exponential", "fem_probe_l2_read", "fem_probe_l2_gather",
+    "fem_cut_static", "fem_cut_static_error",
 ]
+CUT_STATIC_MAX_COUNT = 4096   # FEM_CUT_STATIC_MAX_COUNT of include/fem.h
 
 
 class FemError(RuntimeError):
@@ -95,6 +97,8 @@ def load_library():
     lib.fem_schedule_exponential.argtypes = [C.c_double, C.c_double, C.c_int32, C.c_void_p]
     lib.fem_probe_l2_read.argtypes = [C.c_void_p, C.c_size_t, C.c_int32, C.c_void_p, C.POINTER(C.c_double)]
     lib.fem_probe_l2_gather.argtypes = [C.c_void_p, C.c_size_t, C.c_int32, C.c_int32, C.c_void_p, C.POINTER(C.c_double)]
+    lib.fem_cut_static.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
+    lib.fem_cut_static_error.restype = C.c_char_p
     _lib = lib
     return lib
 
@@ -323,6 +327,28 @@ def probe_l2_gather(device: str = "cuda:0", mib: int = 32, row_bytes: int = 128,
     if st != FEM_OK:
         raise FemError(st, "fem_probe_l2_gather")
     return float(out.value)
+
+
+def cut_static(row_ptr, col_idx, weight, sigma, cut, stream=None) -> None:
+    """fem_cut_static on torch CUDA tensors (all on one device): row_ptr int32 [n + 1], col_idx int32 [nnz], weight float32
+    [nnz] or None, sigma int8 [n, count] (configuration innermost), cut int64 [count] (written).  Allocates nothing and does
+    not synchronise; argument marshalling only."""
+    import torch
+    lib = load_library()
+    want = ((row_ptr, torch.int32), (col_idx, torch.int32), (sigma, torch.int8), (cut, torch.int64)) + (((weight, torch.float32),) if weight is not None else ())
+    for t, dt in want:
+        if not (t.is_cuda and t.dtype == dt and t.is_contiguous() and t.device == sigma.device):
+            raise FemError(FEM_EINVAL, "cut_static: tensors must be contiguous CUDA tensors of the documented dtypes on one device")
+    n, count = int(sigma.shape[0]), int(sigma.shape[1])
+    if row_ptr.numel() != n + 1 or cut.numel() < min(count, CUT_STATIC_MAX_COUNT):
+        raise FemError(FEM_EINVAL, "cut_static: row_ptr must have n + 1 entries and cut at least count")
+    with torch.cuda.device(sigma.device):
+        st_ = stream if stream is not None else torch.cuda.current_stream(sigma.device)
+        st = lib.fem_cut_static(n, C.c_void_p(row_ptr.data_ptr()), C.c_void_p(col_idx.data_ptr()),
+                                C.c_void_p(weight.data_ptr()) if weight is not None else None, C.c_void_p(sigma.data_ptr()),
+                                count, C.c_void_p(cut.data_ptr()), C.c_void_p(st_.cuda_stream))
+    if st != FEM_OK:
+        raise FemError(st, (lib.fem_cut_static_error() or b"").decode())
 
 
 def schedule_for(cfg: wl.Config, precise_steps: int = 8) -> Schedule:
