@@ -25,7 +25,8 @@ struct Q2Params {
     unsigned rv;        // Rb / VEC lanes per variable
     int rv_shift;       // log2(rv) when rv is a power of two, else -1
     unsigned total;     // n * rv threads per replica block
-    unsigned main_blocks;  // CTAs that map one thread to (variable, VEC replicas); the CTAs after them take one long row each
+    unsigned long_blocks;  // the first long_blocks CTAs take one long row each (they start first: the longest work of the launch);
+                           // the CTAs after them map one thread to (variable, VEC replicas)
     int long_on;        // rows longer than kLongRow are left to those CTAs (dp.long_rows)
     unsigned long_chunks;  // CTAs per long row: ceil(rv / kLongLanes)
 };
@@ -52,18 +53,19 @@ __global__ void __launch_bounds__(kThreads, GH ? 8 : ((MODE == MODE_MAXCUT || MO
     // other thread.  The hub's own row of the gather array is read by all its neighbours and stays in L1 / L2.
     constexpr bool LONG = (MODE == MODE_MAXCUT || MODE == MODE_ISING) && DEG == 0 && !GH;
     bool long_cta = false;
-    if constexpr (LONG) long_cta = blockIdx.x >= p.main_blocks;
-    const unsigned idx = blockIdx.x * kThreads + threadIdx.x;
+    if constexpr (LONG) long_cta = blockIdx.x < p.long_blocks;
+    const unsigned idx = (blockIdx.x - (LONG && !long_cta ? p.long_blocks : 0u)) * kThreads + threadIdx.x;
     if (!long_cta && idx >= p.total) return;
     unsigned i = p.rv_shift >= 0 ? idx >> p.rv_shift : idx / p.rv;
     unsigned c = (idx - i * p.rv) * VEC;
     if constexpr (LONG) {  // rows of different lengths: threads take the variables in degree-sorted order (fem_create)
-        if (!long_cta && p.dp.order) i = (unsigned)__ldg(p.dp.order + i);
+        // (longest rows first: the order is ascending in degree, and the last CTAs of a launch are its tail)
+        if (!long_cta && p.dp.order) i = (unsigned)__ldg(p.dp.order + (p.dp.n - 1 - i));
     }
     unsigned lane0 = 0, lanes = 1;  // long-row CTA: the lanes of the replica block it serves
     if constexpr (LONG) {
         if (long_cta) {
-            const unsigned L = blockIdx.x - p.main_blocks;
+            const unsigned L = blockIdx.x;
             i = (unsigned)__ldg(p.dp.long_rows + L / p.long_chunks);
             lane0 = (L % p.long_chunks) * kLongLanes;
             lanes = min((unsigned)kLongLanes, p.rv - lane0);
@@ -609,11 +611,12 @@ static void launch_step_q2_t(Handle *hd, const StepScalars &sc, int blk_begin, i
     p.rv = (unsigned)(Rb / VEC);
     p.rv_shift = (p.rv & (p.rv - 1)) == 0 ? __builtin_ctz(p.rv) : -1;
     p.total = (unsigned)hd->dp.n * p.rv;
-    p.main_blocks = (unsigned)ceil_div(p.total, kThreads);
+    const unsigned main_blocks = (unsigned)ceil_div(p.total, kThreads);
     // long rows (CSR kinds without a uniform degree): one extra CTA each, when a row's lanes fit a CTA
     p.long_on = (mode == MODE_MAXCUT || mode == MODE_ISING) && hd->opt_long_rows && hd->dp.n_long > 0 && hd->dp.uniform_deg == 0;
     p.long_chunks = (unsigned)ceil_div(p.rv, kLongLanes);
-    dim3 grid(p.main_blocks + (p.long_on ? (unsigned)hd->dp.n_long * p.long_chunks : 0u), (unsigned)blk_count);
+    p.long_blocks = p.long_on ? (unsigned)hd->dp.n_long * p.long_chunks : 0u;
+    dim3 grid(main_blocks + p.long_blocks, (unsigned)blk_count);
     if (VEC == 4) launch_q2_mode<T, 4>(hd, p, grid, mode);
     else launch_q2_mode<T, 1>(hd, p, grid, mode);
     hd->launches++;
