@@ -198,13 +198,19 @@ fem_status fem_energy_of(fem_handle *h, const int32_t *cfg /* [count][n] */, int
  * 0 = one thread per row as for short rows -- this one does change the summation order of those rows),
  * "potts_si" (BMINCUT, q = 4 or 8, replica blocks of 4 / 8 / 16 / 32 with n a multiple of 32 / block: 1 = fp32 steps on
  * state-innermost replica blocks, k_step_potts_si.cu, the default; 0 = off),
+ * "l2_persist" (state-innermost Potts steps: 1 = the two gather buffers of the replica block(s) a launch works on are kept
+ * in a persisting L2 set-aside under an access-policy window while h, m1, m2 stream past them, the default, used when both
+ * fit in 47% of the L2; 0 = off.  The set-aside is the DEVICE-wide limit cudaLimitPersistingL2CacheSize: fem_anneal raises it
+ * when such steps begin, and fem_result, fem_reset and fem_destroy put the old value back after synchronising; while it is
+ * raised, other work on the device has that much less L2 for ordinary accesses.  A cache policy: no bit of the result
+ * changes),
  * "potts_tma" (BMINCUT shapes the state-innermost kernel does not take, or with "potts_si" = 0: 1 = rows staged by bulk
  * asynchronous copies where the shape allows, the default; 0 = register path).  Apart from "long_rows" and
  * the three "tensor_cores" modes (different roundings of the dense product) none of them changes a single bit of the
  * results.  Unknown key: FEM_EINVAL. */
 fem_status fem_set_option(fem_handle *h, const char *key, int64_t value);
 /* Introspection for benchmarks: "launches" (kernels enqueued so far), "tc_launches" (of which tcgen05
- * dense steps; "tc8_launches": of those, int8 digit steps), "persist_launches", "persist_cluster" (CTAs per replica of the persistent kernel),
+ * dense steps; "tc8_launches": of those, int8 digit steps), "l2_persist_bytes" (persisting L2 set-aside in force, 0 when none), "persist_launches", "persist_cluster" (CTAs per replica of the persistent kernel),
  * "tma_launches" (TMA-staged Potts steps), "si_launches" (state-innermost Potts steps), "t_done", "R", "replica_block", "nnz", "uniform_degree",
  * "max_degree", "long_rows" (rows of a two-state graph kind with more than 96 entries, or more than 32 and four times the mean degree:
  * the stepwise kernel gives each

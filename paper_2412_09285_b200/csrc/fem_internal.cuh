@@ -160,6 +160,10 @@ struct Handle {
     // arrays are re-laid out in place for the fp32 steps of one fem_anneal call (si_live) and back before it returns.
     int64_t opt_long_rows = 1;   // 0: long rows stay with one thread per VEC replicas (measurements only)
     int64_t opt_potts_si = 1;
+    int64_t opt_l2_persist = 1;     // state-innermost Potts steps: keep the two gather buffers of a replica block in a persisting L2 set-aside
+    bool l2_persist_on = false;     // the device limit is raised (fem_api.cu: l2_persist_begin / l2_persist_end)
+    size_t l2_persist_prev = 0;     // cudaLimitPersistingL2CacheSize as found
+    int64_t l2_persist_bytes = 0;   // set-aside in force while on (info)
     int64_t si_launches = 0;
     bool si_live = false;
     int64_t persist_ell[4] = {-1, -1, -1, -1};  // sliced-ELL entries per CTA for cluster sizes 1, 2, 4, 8

@@ -453,11 +453,22 @@ static cudaError_t launch_si_deg(Handle *hd, PottsSiParams &p, int blk_count) {
     cfg.blockDim = dim3(kSiWarps * 32);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = hd->stream;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
+    if (hd->l2_persist_on) {
+        // the gather buffer this step WRITES goes to the persisting set-aside (fem_api.cu: l2_persist_begin); it is the one
+        // the next step gathers from, and the set-aside holds both, so the gathers hit whatever h, m1, m2 stream through
+        attr[1].id = cudaLaunchAttributeAccessPolicyWindow;
+        attr[1].val.accessPolicyWindow.base_ptr = (void *)p.g_out;
+        attr[1].val.accessPolicyWindow.num_bytes = (size_t)blk_count * (size_t)p.blk_stride * sizeof(float);
+        attr[1].val.accessPolicyWindow.hitRatio = 1.0f;
+        attr[1].val.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+        attr[1].val.accessPolicyWindow.missProp = cudaAccessPropertyNormal;
+        cfg.numAttrs = 2;
+    }
     return cudaLaunchKernelEx(&cfg, kernel, p);
 }
 

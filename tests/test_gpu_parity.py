@@ -492,6 +492,55 @@ def test_potts_si_bit_identical_to_team_kernel(fem, case, opt):
     assert np.array_equal(out[1][2]["part_sizes"], out[0][2]["part_sizes"])
 
 
+def test_potts_l2_persistence_changes_no_bit_and_gives_the_set_aside_back(fem):
+    """State-innermost Potts steps keep the gather buffers of a replica block in a persisting L2 set-aside (option
+    "l2_persist", default 1; fem_api.cu l2_persist_begin / l2_persist_end): a cache policy, so every bit of the result is
+    the same with it off; the device-wide limit is raised while the steps run and is back at its old value after
+    fem_result (and after fem_destroy when no result was asked for)."""
+    try:
+        from cuda.bindings import runtime as cudart
+    except Exception:                                     # pragma: no cover - cuda-python is in the image
+        cudart = None
+
+    def limit():
+        if cudart is None:
+            return None
+        err, val = cudart.cudaDeviceGetLimit(cudart.cudaLimit.cudaLimitPersistingL2CacheSize)
+        assert int(err) == 0
+        return int(val)
+
+    q, d, n, R, rb, _ = SI_CASES["q8_reg10_R16_rb8"]
+    inst = wl.random_regular(n, d, 2020 + q, wl.BMINCUT, q, lam=0.03)
+    sch = fem.Schedule(beta=fem.linear_temperature_schedule(1.0, 0.05, 40), precise_steps=4)
+    import torch
+    torch.cuda.synchronize()
+    before = limit()
+    out = {}
+    for persist in (1, 0):
+        eng = fem.Fem(inst, R)
+        eng.set_option("replica_block", rb)
+        eng.set_option("l2_persist", persist)
+        eng.anneal(sch, R, seed=8)
+        bytes_on = eng.info("l2_persist_bytes")
+        assert (bytes_on >= 2 * (inst.n * q + 1) * rb * 4) if persist else bytes_on == 0
+        if persist and before is not None:
+            assert limit() == bytes_on
+        fields = eng.get_fields()
+        res = eng.result()
+        assert eng.info("l2_persist_bytes") == 0 and limit() == before
+        assert eng.info("si_launches") == 36 * (R // rb)
+        out[persist] = (fields, res)
+        eng.close()
+    assert np.array_equal(out[1][0], out[0][0])
+    assert np.array_equal(out[1][1]["energy"], out[0][1]["energy"])
+    eng = fem.Fem(inst, R)                                # no fem_result: fem_destroy gives the set-aside back
+    eng.set_option("replica_block", rb)
+    eng.anneal(sch, R, seed=8)
+    assert eng.info("l2_persist_bytes") > 0
+    eng.close()
+    assert limit() == before
+
+
 def test_two_handles_with_rank_seeds_match_single_runs(fem):
     """The N > 1 path on one device: two handles, seeded as ranks 0 and 1 (multigpu.replica_seed), advanced in turns on
     the same stream, give bit for bit what each seed gives alone -- handles share nothing -- and the Eq.5 pick over the
