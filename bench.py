@@ -260,6 +260,7 @@ def run_workload(args, name, steps, warmup, ctx, with_e2e=True):
     wall_end = time.time()
     clocks = sampler.stop(wall_begin, wall_end) if sampler else None
     launches = eng.info("launches") - launches0
+    l2_persist_bytes = eng.info("l2_persist_bytes")            # (read before fem_result gives the set-aside back)
     res = eng.result()
     bulk_ms = sum(e[0].elapsed_time(e[1]) for e in bulk_events)
     bulk_launches = sum(e[2] for e in bulk_events)
@@ -268,6 +269,7 @@ def run_workload(args, name, steps, warmup, ctx, with_e2e=True):
     # algorithmic bytes of one launch: the whole step's bytes spread over the launches that make up a step
     step_bytes = eng.info("step_bytes") * (N - K) * steps / max(bulk_launches, 1)
     info = {k: eng.info(k) for k in ("tc_launches", "tc8_launches", "persist_launches", "tma_launches", "si_launches", "replica_block", "nnz")}
+    info["l2_persist_bytes"] = l2_persist_bytes
     eng.close()
 
     # ---- e2e through the public API from host buffers (pinned), host<->device copies inside the timed region
@@ -400,6 +402,7 @@ def run_workload(args, name, steps, warmup, ctx, with_e2e=True):
             roofline["note"] = ("the step moves (12 + 4 deg + 16) B per field between SMs and L2 against 24 B of compulsory HBM traffic; "
                                 "with a block footprint beyond one die's half of the L2 the measured SM <-> L2 rate, not HBM, is what "
                                 "binds (l2_gather_probe_gbs: pure random-row reads, footprint-sized vs 32 MiB working set)")
+            roofline["l2_persist_bytes"] = info["l2_persist_bytes"]   # persisting L2 set-aside holding the block's gather buffers
         if info["replica_block"] < R and 20.0 * n * inst.fields_per_var * info["replica_block"] < 0.5 * 126e6:
             roofline["note"] = ("replica block L2-resident for the whole anneal: `achieved` is the ALGORITHMIC-byte rate "
                                 "(24 B per field per step / time) served out of L2, not DRAM utilisation; it is compared with "
