@@ -4,20 +4,21 @@
 // The stepwise kernel (k_step_q2.cu) is launch- and latency-bound when n*R is a few tens of thousands of
 // fields (BASELINE.json configs[0]: n = 800, R = 32: one launch per annealing step, 11 us each, 1% of HBM).
 // Replicas are independent, so here ONE CLUSTER of CS CTAs owns ONE replica for a whole
-// run of annealing steps: CTA c of the cluster owns the variables [c*chunk, (c+1)*chunk); their h, m1, m2 live in
-// registers; every CTA keeps the replica's whole gathered vector m = tanh(h/2) double-buffered in its own shared
-// memory and, after each step, stores its new m values into all CS copies through distributed shared memory;
-// the only synchronisation per annealing step is one cluster barrier (__syncthreads() when CS = 1).  The CTA's
-// rows of the CSR are staged once in shared memory as a sliced ELL (slot-major inside each warp: lane l of a
-// warp reads index/weight slot j at [j*32 + l], conflict-free; 16-bit column indices).  HBM is touched at entry
-// (load state) and exit (store state), so the per-step launch, DRAM and L2 round trips disappear; the binding
-// resource is the shared-memory gather rate of the SMs a replica is spread over.
+// run of annealing steps: the warps of the cluster take the variables in turn along the degree-sorted processing order;
+// their h, m1, m2 live in registers; every CTA keeps the replica's whole gathered vector m = tanh(h/2) double-buffered in
+// its own shared memory, in slot order (what a CTA produces is one contiguous run), and after each step pushes its run
+// into the peers' copies with one bulk copy per peer through distributed shared memory, completing on the peer's
+// mbarrier: no cluster barrier and no per-lane remote store inside the step (__syncthreads() only when CS = 1).  The CTA's
+// rows of the CSR are staged once per launch in shared memory as a sliced ELL of 16-bit slot columns (eight per lane and
+// 16-byte load), or kept in registers (fp32 steps, unit weights, rows of at most 72 entries).  HBM is touched at entry
+// (load state) and exit (store state), so the per-step launch, DRAM and L2 round trips disappear; what binds is the
+// latency of the shared-memory gathers and of the exchange.
 //
 // Arithmetic is the stepwise kernel's, instruction for instruction (same device functions, same CSR-order sum),
 // so the result is bit-identical to the stepwise path (tests/test_gpu_parity.py::test_persistent_bit_identical).
 // Rows a1-a4 of DESIGN.md section 2: S30 coupling sum, S29 entropy gradient and
 // chain rule, Adam; the per-step scalars 1/beta_t and the two bias corrections come from the
-// host (double) in the kernel parameters, kChunk steps per launch.
+// host (double) in the kernel parameters, PersistChunk<T>::kSteps steps per launch.
 #include <cooperative_groups.h>
 
 #include "device_math.cuh"
