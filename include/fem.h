@@ -212,7 +212,7 @@ fem_status fem_set_option(fem_handle *h, const char *key, int64_t value);
 /* Introspection for benchmarks: "launches" (kernels enqueued so far), "tc_launches" (of which tcgen05
  * dense steps; "tc8_launches": of those, int8 digit steps), "l2_persist_bytes" (persisting L2 set-aside in force, 0 when none), "persist_launches", "persist_cluster" (CTAs per replica of the persistent kernel),
  * "tma_launches" (TMA-staged Potts steps), "si_launches" (state-innermost Potts steps), "t_done", "R", "replica_block", "nnz", "uniform_degree",
- * "max_degree", "long_rows" (rows of a two-state graph kind with more than 96 entries, or more than 32 and four times the mean degree:
+ * "max_degree", "long_rows" (rows of a two-state graph kind with more than 80 entries:
  * the stepwise kernel gives each
  * a CTA of its own), "integral_weights", "step_bytes" (algorithmic HBM bytes of one fused step of the last schedule's optimiser,
  * DESIGN.md section 6).  Unknown key: -1. */

@@ -24,12 +24,12 @@ namespace fem {
 constexpr int kThreads = 256;
 constexpr int kMaxQ = 32;
 constexpr int kMaxClauseLen = 8;
-// two-state graph kinds, rows from row_ptr: a "long row" has more than kLongRow entries, or more than kLongRowSkew entries
-// when that is over four times the mean degree (the hubs of a degree-skewed graph) -- the stepwise kernel gives it a
-// whole CTA (k_step_q2.cu) instead of one thread per VEC replicas, and the replica-persistent kernel is not used
-constexpr int kLongRow = 96;
-constexpr int kLongRowSkew = 32;
-__host__ __device__ inline bool is_long_row(int64_t deg, int64_t nnz, int n) { return deg > kLongRow || (deg > kLongRowSkew && deg * n > 4 * nnz); }
+// two-state graph kinds, rows from row_ptr: a "long row" has more than kLongRow entries (the hubs of a degree-skewed graph) --
+// the stepwise kernel gives it a whole CTA (k_step_q2.cu) instead of one thread per VEC replicas, and the replica-persistent
+// kernel is not used.  Measured on the scale-free workload (n = 1e5, hub degree 1167; us per launch of 3.2 M fields):
+// threshold 32 -> 27.5, 64 -> 23.1, 80 -> 21.7, 96 -> 22.0, 128 -> 26.7, 192 -> 34.2.
+constexpr int kLongRow = 80;
+__host__ __device__ inline bool is_long_row(int64_t deg, int64_t /*nnz*/, int /*n*/) { return deg > kLongRow; }
 
 // Per-step scalars, computed on the host in double and narrowed in-kernel.
 struct StepScalars {

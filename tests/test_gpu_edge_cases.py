@@ -60,7 +60,7 @@ def cases():
         "empty_graph": (_graph(wl.MAXCUT, 37, []), 5),
         "isolated_nodes": (_graph(wl.MAXCUT, 50, [(0, 1), (1, 2), (7, 9)], weights=[1.0, -2.0, 3.0]), 1),
         "star_degree_1499": (_graph(wl.MAXCUT, 1500, star), 6),
-        # degree-skewed rows (north_star subsystem 2): hubs of a scale-free graph get a CTA each (rows > 96 entries)
+        # degree-skewed rows (north_star subsystem 2): hubs of a scale-free graph get a CTA each (rows > 80 entries)
         "scalefree_n3000_R12": (wl.preferential_attachment(3000, 3, 31, pm1=True), 12),
         "scalefree_ising_n2000_R64": (wl.sparse_ising_from(wl.preferential_attachment(2000, 4, 32, pm1=False), -0.5), 64),
         "ising_two_spins": (_graph(wl.ISING, 2, [(0, 1)], weights=[0.75]), 4),
@@ -110,7 +110,7 @@ def test_degenerate_inputs_against_the_oracle(fem, name, manipulated):
 
 @pytest.mark.parametrize("name", ["star_degree_1499", "scalefree_n3000_R12", "scalefree_ising_n2000_R64"])
 def test_long_rows_take_the_cta_path_and_are_deterministic(fem, name):
-    """Rows with more than 96 entries are summed by a CTA in a fixed order: the counter shows the path is taken (and the
+    """Rows with more than 80 entries are summed by a CTA in a fixed order: the counter shows the path is taken (and the
     replica-persistent kernel, which has no such path, is not), two runs agree bit for bit, and the replica blocking
     changes nothing (a long row is always cut into the same 16 interleaved slices)."""
     inst, R = CASES[name]
