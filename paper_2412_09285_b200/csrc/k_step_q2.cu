@@ -41,7 +41,7 @@ enum { MODE_MAXCUT = 0, MODE_ISING = 1, MODE_SAT = 3, MODE_FIELD = 4 };
 // would have used, so the results are bit-identical while no gather array is written: 24 B of HBM traffic per field
 // and step instead of 28, for DEG more exp / rcp per field (cfg 4a is DRAM-bound: profiles/r02_cfg4a_step.md).
 template <typename T, int VEC, int MODE, int DEG, bool GH = false, int KB = 4>
-__global__ void __launch_bounds__(kThreads, GH ? 8 : ((MODE == MODE_MAXCUT || MODE == MODE_ISING) && DEG == 0 && sizeof(T) == 4 ? 4 : 1)) step_q2_kernel(const Q2Params<T> p) {
+__global__ void __launch_bounds__(kThreads, GH ? 8 : (((MODE == MODE_MAXCUT || MODE == MODE_ISING) && DEG == 0 || MODE == MODE_SAT) && sizeof(T) == 4 ? 4 : 1)) step_q2_kernel(const Q2Params<T> p) {
     using R = Row<T, VEC>;
     pdl_trigger();
     // Degree-skewed rows (north_star subsystem 2; the paper's scale-free MaxCut instances, and the reason c_i
