@@ -118,7 +118,7 @@ static Layout make_layout(const fem_problem *pb, const ProblemShape &s, int R_ca
     L.rowsum = take(s.nnz > 0 || pb->row_ptr ? (size_t)pb->n * 8 : 0);
     L.long_rows = take((size_t)s.n_long * 4);
     L.vw = take(pb->node_weight ? (size_t)pb->n * 4 : 0);
-    L.order = take(pb->kind != FEM_BMINCUT && pb->row_ptr ? (size_t)pb->n * 4 : 0);
+    L.order = take((pb->kind != FEM_BMINCUT && pb->row_ptr) || (pb->kind == FEM_MAXSAT && !pb->lit_state) ? (size_t)pb->n * 4 : 0);
     L.rank = take(pb->kind != FEM_BMINCUT && pb->row_ptr ? (size_t)pb->n * 4 : 0);
     L.J = take(s.dense ? (size_t)pb->n * pb->n * 4 : 0);
     L.Jlo = take(s.dense ? (size_t)pb->n * pb->n * 4 : 0);
@@ -510,6 +510,20 @@ fem_status fem_create(const fem_problem *pb, int32_t R_cap, void *workspace, siz
         }
         hd->integral_weights = true;
         hd->structure_bytes = 4 * ((int64_t)n * F + 1) + 4 * (int64_t)s.nocc * kst;
+        if (!qs && n > 1) {
+            // processing order of the stepwise kernel: the variables by ascending number of occurrences (counting sort, stable);
+            // its threads take them from the end, so the last CTAs of a launch -- its tail -- hold the variables with the
+            // fewest occurrences.  Which thread takes which variable changes no arithmetic.
+            int mx = 0;
+            for (int v = 0; v < n; ++v) mx = std::max(mx, h_occ_ptr[(size_t)v + 1] - h_occ_ptr[v]);
+            std::vector<int> cnt((size_t)mx + 2, 0);
+            h_ord.resize((size_t)n);
+            for (int v = 0; v < n; ++v) cnt[(size_t)(h_occ_ptr[(size_t)v + 1] - h_occ_ptr[v]) + 1]++;
+            for (size_t d = 1; d < cnt.size(); ++d) cnt[d] += cnt[d - 1];
+            for (int v = 0; v < n; ++v) h_ord[(size_t)cnt[(size_t)(h_occ_ptr[(size_t)v + 1] - h_occ_ptr[v])]++] = v;
+            up(at(L.order), h_ord.data(), h_ord.size() * 4, "upload order");
+            dp.order = reinterpret_cast<int *>(at(L.order));
+        }
         if (!qs) {   // sliced-ELL sizes of the replica-persistent kernel, from the occurrence counts
             hd->dp = dp;
             std::vector<int64_t> optr(h_occ_ptr.begin(), h_occ_ptr.end());

@@ -56,7 +56,7 @@ struct DevProblem {
     const float *vw;       // BMINCUT: node weights V_i of the balance term (S33-S35), or nullptr (= all 1)
     double vtotal;         // sum_i V_i (= n without node weights)
     const int *rank;       // [n] inverse of `order` (the position of each variable), nullptr with it
-    const int *order;      // [n] two-state graph kinds with rows of different lengths: the variables sorted by degree (ascending), the
+    const int *order;      // [n] (Boolean Max-SAT: the variables by ascending number of occurrences.)  Two-state graph kinds with rows of different lengths: the variables sorted by degree (ascending), the
                            // order in which the stepwise kernel's threads take them, so that the variables of a warp have rows of
                            // (nearly) the same length; nullptr = index order
     const int *long_rows;  // [n_long] variables whose row has more than kLongRow entries (two-state graph kinds), ascending

@@ -73,6 +73,9 @@ __global__ void __launch_bounds__(Q2Block<T, MODE>::kTpb, GH ? 8 : (Q2Block<T, M
         // (longest rows first: the order is ascending in degree, and the last CTAs of a launch are its tail)
         if (!long_cta && p.dp.order) i = (unsigned)__ldg(p.dp.order + (p.dp.n - 1 - i));
     }
+    if constexpr (MODE == MODE_SAT) {  // variables with the most occurrences first (fem_create)
+        if (p.dp.order) i = (unsigned)__ldg(p.dp.order + (p.dp.n - 1 - i));
+    }
     unsigned lane0 = 0, lanes = 1;  // long-row CTA: the lanes of the replica block it serves
     if constexpr (LONG) {
         if (long_cta) {
