@@ -34,25 +34,29 @@ struct Q2Params {
 constexpr int kLongSlices = 32;  // interleaved slices a long row is cut into (fixed: the summation order depends on the row only)
 constexpr int kLongLanes = 32;   // lanes (VEC replicas each) one long-row CTA serves; a wider replica block takes several CTAs per row
 
-#ifndef SAT_TPB
-#define SAT_TPB 64
-#endif
 enum { MODE_MAXCUT = 0, MODE_ISING = 1, MODE_SAT = 3, MODE_FIELD = 4 };
+
+// Threads per CTA and the register cap (as CTAs per SM) of each instantiation.  Max-SAT fp32 steps use CTAs of 64 threads:
+// at R = 128 a warp is one variable's replicas, the time of a CTA is that of its slowest variable, and the finer the CTAs the
+// shorter the tail of a launch (cfg 3: 85.9 -> 82.4 us); 16 of them per SM = 64 registers, four resident CTAs' worth of warps
+// more than the 68 registers the compiler would take (93.9 -> 85.9 us).  CSR graphs without a uniform degree: 64 registers too
+// (skew workload 31.0 -> 28.3 us).  Gather-the-fields: 32 registers, eight CTAs of 256 (six: 193 us against 184 at cfg 4a).
+constexpr int kSatThreads = 64;
+template <typename T, int MODE, int DEG, bool GH>
+struct Q2Block {
+    static constexpr bool kSat32 = MODE == MODE_SAT && sizeof(T) == 4;
+    static constexpr bool kCsr32 = (MODE == MODE_MAXCUT || MODE == MODE_ISING) && DEG == 0 && !GH && sizeof(T) == 4;
+    static constexpr int kTpb = kSat32 ? kSatThreads : kThreads;
+    static constexpr int kMinBlocks = GH ? 8 : (kSat32 ? 1024 / kSatThreads : (kCsr32 ? 4 : 1));
+};
 
 // GH ("gather the fields", fp32 MaxCut / sparse Ising, regular degree 3 or 4): neighbours are gathered from the FIELD
 // array (p.a.g_in == p.a.h) and m_j = tanh(h_j / 2) is recomputed per neighbour with the very function the owner
 // would have used, so the results are bit-identical while no gather array is written: 24 B of HBM traffic per field
 // and step instead of 28, for DEG more exp / rcp per field (cfg 4a is DRAM-bound: profiles/r02_cfg4a_step.md).
-// threads per CTA: Max-SAT fp32 steps use small CTAs (a warp is one variable's replicas there and the time of a CTA is that of
-// its slowest variable: the finer the CTAs, the shorter the tail of a launch)
-template <typename T, int MODE>
-struct Q2Block {
-    static constexpr int kTpb = (MODE == 3 && sizeof(T) == 4) ? SAT_TPB : kThreads;
-    static constexpr int kMinBlocks = (MODE == 3 && sizeof(T) == 4) ? 1024 / SAT_TPB : 0;
-};
 template <typename T, int VEC, int MODE, int DEG, bool GH = false, int KB = 4>
-__global__ void __launch_bounds__(Q2Block<T, MODE>::kTpb, GH ? 8 : (Q2Block<T, MODE>::kMinBlocks ? Q2Block<T, MODE>::kMinBlocks : ((MODE == MODE_MAXCUT || MODE == MODE_ISING) && DEG == 0 && sizeof(T) == 4 ? 4 : 1))) step_q2_kernel(const Q2Params<T> p) {
-    constexpr unsigned TPB = Q2Block<T, MODE>::kTpb;
+__global__ void __launch_bounds__(Q2Block<T, MODE, DEG, GH>::kTpb, Q2Block<T, MODE, DEG, GH>::kMinBlocks) step_q2_kernel(const Q2Params<T> p) {
+    constexpr unsigned TPB = Q2Block<T, MODE, DEG, GH>::kTpb;
     using R = Row<T, VEC>;
     pdl_trigger();
     // Degree-skewed rows (north_star subsystem 2; the paper's scale-free MaxCut instances, and the reason c_i
@@ -527,13 +531,13 @@ template <typename T, int VEC, int MODE>
 static void launch_q2_deg(Handle *hd, const Q2Params<T> &p, dim3 grid) {
     if constexpr (MODE == MODE_SAT) {
         switch (hd->dp.kstride) {
-            case 1: launch_pdl(step_q2_kernel<T, VEC, MODE, 1>, grid, dim3(Q2Block<T, MODE>::kTpb), hd->stream, p); break;
-            case 2: launch_pdl(step_q2_kernel<T, VEC, MODE, 2>, grid, dim3(Q2Block<T, MODE>::kTpb), hd->stream, p); break;
-            case 3: launch_pdl(step_q2_kernel<T, VEC, MODE, 3>, grid, dim3(Q2Block<T, MODE>::kTpb), hd->stream, p); break;
-            case 4: launch_pdl(step_q2_kernel<T, VEC, MODE, 4>, grid, dim3(Q2Block<T, MODE>::kTpb), hd->stream, p); break;
-            case 5: launch_pdl(step_q2_kernel<T, VEC, MODE, 5>, grid, dim3(Q2Block<T, MODE>::kTpb), hd->stream, p); break;
-            case 6: launch_pdl(step_q2_kernel<T, VEC, MODE, 6>, grid, dim3(Q2Block<T, MODE>::kTpb), hd->stream, p); break;
-            default: launch_pdl(step_q2_kernel<T, VEC, MODE, 7>, grid, dim3(Q2Block<T, MODE>::kTpb), hd->stream, p); break;
+            case 1: launch_pdl(step_q2_kernel<T, VEC, MODE, 1>, grid, dim3(Q2Block<T, MODE, 1, false>::kTpb), hd->stream, p); break;
+            case 2: launch_pdl(step_q2_kernel<T, VEC, MODE, 2>, grid, dim3(Q2Block<T, MODE, 2, false>::kTpb), hd->stream, p); break;
+            case 3: launch_pdl(step_q2_kernel<T, VEC, MODE, 3>, grid, dim3(Q2Block<T, MODE, 3, false>::kTpb), hd->stream, p); break;
+            case 4: launch_pdl(step_q2_kernel<T, VEC, MODE, 4>, grid, dim3(Q2Block<T, MODE, 4, false>::kTpb), hd->stream, p); break;
+            case 5: launch_pdl(step_q2_kernel<T, VEC, MODE, 5>, grid, dim3(Q2Block<T, MODE, 5, false>::kTpb), hd->stream, p); break;
+            case 6: launch_pdl(step_q2_kernel<T, VEC, MODE, 6>, grid, dim3(Q2Block<T, MODE, 6, false>::kTpb), hd->stream, p); break;
+            default: launch_pdl(step_q2_kernel<T, VEC, MODE, 7>, grid, dim3(Q2Block<T, MODE, 7, false>::kTpb), hd->stream, p); break;
         }
     } else {
         const int d = (MODE == MODE_MAXCUT || MODE == MODE_ISING) ? hd->dp.uniform_deg : 0;
@@ -625,7 +629,7 @@ static void launch_step_q2_t(Handle *hd, const StepScalars &sc, int blk_begin, i
     p.rv = (unsigned)(Rb / VEC);
     p.rv_shift = (p.rv & (p.rv - 1)) == 0 ? __builtin_ctz(p.rv) : -1;
     p.total = (unsigned)hd->dp.n * p.rv;
-    const unsigned main_blocks = (unsigned)ceil_div(p.total, mode == MODE_SAT ? Q2Block<T, MODE_SAT>::kTpb : kThreads);
+    const unsigned main_blocks = (unsigned)ceil_div(p.total, mode == MODE_SAT ? Q2Block<T, MODE_SAT, 1, false>::kTpb : kThreads);
     // long rows (CSR kinds without a uniform degree): one extra CTA each, when a row's lanes fit a CTA
     p.long_on = (mode == MODE_MAXCUT || mode == MODE_ISING) && hd->opt_long_rows && hd->dp.n_long > 0 && hd->dp.uniform_deg == 0;
     p.long_chunks = (unsigned)ceil_div(p.rv, kLongLanes);
